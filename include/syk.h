@@ -1,0 +1,179 @@
+/* syk.h -- C ABI of libsyk_b200: the data-parallel hot path of the sparse-SYK OTOC method of
+ * arXiv 2311.00639 on one NVIDIA B200 (sm_100a).
+ *
+ * Citations "PAPER.md:<line>" refer to the paper text; "R-xxx" to the readings listed in DESIGN.md section 2.
+ *
+ * Conventions common to every call
+ *   - Every function returns an int: SYK_OK (0) or a negative error code.  Nothing throws, prints or exits.
+ *   - N = number of Majorana fermions, even, 4 <= N <= 64.  L = N/2 qubits, D = 2^L amplitudes.
+ *   - A state vector is a contiguous array of D complex numbers, interleaved (re, im); `dtype` says whether the
+ *     components are float (SYK_C64, 8 bytes per amplitude) or double (SYK_C128, 16 bytes per amplitude).
+ *     Basis index b = sum_q bit_q 2^q, qubit 0 = least significant bit (R-ENDIAN).
+ *   - Pointers named d_* are DEVICE pointers owned by the caller, 16-byte aligned; pointers named h_* and all
+ *     other pointers are HOST pointers.  The library never allocates device vectors: work space is passed in
+ *     (the memory discipline is part of the method).  The only device memory the library
+ *     owns is the per-Hamiltonian term table (a few KB for sparse H, <= ~8 MB for dense N=48), allocated on
+ *     first device use of a handle and released by syk_free_hamiltonian.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and return, except
+ *     where they hand back host scalars (syk_krylov_evolve, syk_otoc, syk_lanczos_run, *_host): those
+ *     synchronise that stream only.
+ *   - There is no CPU fallback: a compute call on a machine without a CUDA device returns SYK_ECUDA.
+ *   - Results are bitwise reproducible run to run: no atomics on data, fixed reduction trees.
+ */
+#ifndef SYK_B200_H
+#define SYK_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { SYK_OK = 0,
+       SYK_EINVAL = -1,   /* bad argument: N odd / out of range, p outside (0,1], index >= N, i == j, null or
+                             unaligned pointer, in == out where forbidden, unsorted quartet or t_grid */
+       SYK_ENOMEM = -2,   /* work space too small (ask the *_workspace_bytes query) or host allocation failed */
+       SYK_ECUDA = -3,    /* CUDA runtime error or no device; text via syk_last_cuda_error() */
+       SYK_ENOCONV = -4   /* Krylov sub-step limit reached; the result is written, stats->err_est says how bad */ };
+
+enum { SYK_C64 = 0, SYK_C128 = 1 };
+enum { SYK_GAMMA_PAULI = 0,  /* gamma_n = Pauli string, {g_m,g_n} = 2 delta; benchmark default */
+       SYK_GAMMA_HALF = 1    /* gamma_n = Pauli string / sqrt(2), {g_m,g_n} = delta; R-NORM      */ };
+
+typedef struct syk_ham syk_ham;   /* opaque, library-owned: host term tables + lazily created device copy */
+
+const char* syk_strerror(int code);
+const char* syk_last_cuda_error(void);           /* text of the last CUDA error seen by this thread ("" if none) */
+int syk_version(void);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * a-1  Term compiler (host).  Eq. (1); <bits, coeff> encoding PAPER.md:257-267; operator
+ *      product and sum PAPER.md:299.
+ *
+ * syk_build_hamiltonian samples H = sum_{i<j<k<l} p_ijkl J_ijkl g_i g_j g_k g_l: each quartet (lexicographic rank
+ * r) is kept with probability p and gets J ~ N(0, 3/(8 p N^3)) from the counter-based generator R-RNG keyed
+ * (seed, realization, r).  Each kept quartet becomes one Pauli string c Z^z X^x (Jordan-Wigner, R-JW; acting as
+ * (O v)[b] = c (-1)^popcount(b & z) v[b xor x], R-SIGN) with c = J s^4 times a phase in {1,-1,i,-i}; strings
+ * are grouped by X-mask; canonical order: groups by ascending x, terms inside a group by ascending z.
+ * syk_build_from_terms does the same for caller-supplied quartets (each i<j<k<l, all distinct) and couplings.
+ * *out receives a new handle; release it with syk_free_hamiltonian.  No device is needed for these calls.
+ */
+int syk_build_hamiltonian(int N, double p, uint64_t seed, uint32_t realization, int gamma_norm, syk_ham** out);
+int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets /* [n_terms][4] */,
+                         const double* J /* [n_terms] */, int gamma_norm, syk_ham** out);
+void syk_free_hamiltonian(syk_ham* h);
+
+/* Sizes: any output pointer may be NULL. dim = 2^(N/2). */
+int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, int64_t* dim);
+
+/* Copies the canonical tables to caller arrays (any may be NULL): x[n_xmasks], group_off[n_xmasks+1],
+ * z[n_terms], c_re_im[n_terms][2], quartet_of_term[n_terms][4], J_of_term[n_terms]. */
+int syk_ham_tables(const syk_ham* h, uint64_t* x, uint32_t* group_off, uint64_t* z, double* c_re_im,
+                   int32_t* quartet_of_term, double* J_of_term);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * a-2  apply_H (device).  Algorithm 1, in gather form:
+ *        out[b] = sum_g in[b xor x_g] * sum_{t in g} c_t (-1)^popcount(b & z_t),      0 <= b < D.
+ * d_in and d_out are distinct, non-overlapping device vectors of `dtype`.  SYK_C64 multiplies and accumulates
+ * in fp32 (R-C64), SYK_C128 in fp64.  An empty Hamiltonian (no terms) gives out = 0.
+ */
+int syk_apply_H(const syk_ham* h, int dtype, const void* d_in, void* d_out, void* stream);
+
+/* Batched over disorder realizations: n_batch handles with the same N; vector r of the batch
+ * starts at element offset r*batch_stride (batch_stride >= D) of d_in / d_out. */
+int syk_apply_H_batched(const syk_ham* const* hams, int n_batch, int dtype, const void* d_in, void* d_out,
+                        int64_t batch_stride, void* stream);
+
+/* The same product with HOST vectors: copies h_in to the device work space, applies H, copies the result to
+ * h_out; synchronises.  d_work must hold 2*D amplitudes of `dtype`. */
+int syk_apply_H_host(const syk_ham* h, int dtype, const void* h_in, void* h_out, void* d_work, size_t work_bytes,
+                     void* stream);
+
+/* out = gamma_n in (one Pauli string: flip qubit n/2, sign from the lower qubits, R-JW).
+ * d_out may equal d_in (in place). */
+int syk_apply_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, void* stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * a-5 (input)  Normalised complex Gaussian ("Haar-random") state from R-RNG stream 2, written to
+ * d_psi.  d_scratch: at least syk_reduce_scratch_bytes() bytes of device memory. */
+size_t syk_reduce_scratch_bytes(void);
+int syk_random_state(int N, uint64_t seed, uint32_t realization, int dtype, void* d_psi, void* d_scratch,
+                     void* stream);
+
+/* <a|b> = sum conj(a[k]) b[k] in fp64 (deterministic); synchronises; result to host re_im[2]. */
+int syk_dot(int N, int dtype, const void* d_a, const void* d_b, void* d_scratch, double* re_im, void* stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * a-3 / a-4  Lanczos and the Krylov exponential, PAPER.md:301 ("restarted Krylov subspace method for
+ * exp(-iHt)|Psi>"), R-KRYLOV.
+ *
+ * syk_lanczos_run: m steps of the Hermitian Lanczos recurrence from v_1 = psi/|psi| with the fused kernels
+ * (apply_H with the -beta_j v_{j-1} term and the <v_j|w> partial sums fused; then w - alpha_j v_j with |.|^2
+ * fused; scalars stay on the device between steps).  Outputs (host): alpha[m], beta[m+1] with beta[0] = |psi|
+ * and beta[j] (j>=1) the off-diagonal element / residual norm after step j.  d_psi is not modified.  Work
+ * space: syk_krylov_workspace_bytes with two_pass = 0 and krylov_dim = m.  Synchronises.
+ */
+typedef struct {
+    int krylov_dim;     /* m: Lanczos steps per sub-step (2..128); 0 = default 24 */
+    double tol;         /* relative error target for the whole call; 0 = default 1e-12 (C128) / 1e-6 (C64) */
+    int two_pass;       /* 0: store the m Lanczos vectors (m work vectors); 1: two-pass Lanczos (2 work vectors) */
+    int max_substeps;   /* 0 = default 100000 */
+} syk_krylov_opts;
+
+typedef struct {
+    int64_t n_matvec;   /* apply_H launches */
+    int n_substeps;     /* time sub-steps taken */
+    int krylov_dim_used;/* smallest effective m over sub-steps (happy breakdown shortens it) */
+    double err_est;     /* accumulated a-posteriori error estimate, relative */
+    double model_bytes; /* bytes the byte model of DESIGN.md section 6 attributes to the call */
+    double elapsed_ms;  /* device time of the call (CUDA events on `stream`) */
+} syk_stats;
+
+int syk_krylov_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes);
+
+int syk_lanczos_run(const syk_ham* h, int dtype, const void* d_psi, int m, double* alpha, double* beta,
+                    void* d_work, size_t work_bytes, syk_stats* stats, void* stream);
+
+/* psi <- exp(-i (tau_re + i tau_im) H) psi, in place (R-TAU).  Real time t: (t, 0).  exp(-beta H/4): (0, -beta/4).
+ * exp(-(it + beta/4)H): (t, -beta/4).  The result is NOT renormalised.  opts/stats may be NULL. */
+int syk_krylov_evolve(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im,
+                      const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream);
+
+/* Same with a HOST vector (in/out): d_work must hold one extra vector in front of the Krylov work space, i.e.
+ * D*elem_bytes + syk_krylov_workspace_bytes(). */
+int syk_krylov_evolve_host(const syk_ham* h, int dtype, void* h_psi, double tau_re, double tau_im,
+                           const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                           void* stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * a-5  Regularised OTOC, PAPER.md:230 (R-EQ2, R-WV, R-F):
+ *   F(t) = <psi| e^{(it-b/8)H} g_W e^{-(it+b/4)H} g_V e^{(it-b/4)H} g_W e^{-(it+b/4)H} g_V e^{-bH/8} |psi>
+ * for t in t_grid (non-decreasing, >= 0), W = gamma_{i_W}, V = gamma_{j_V}, b = beta >= 0.  F_out[n_t][2] (host)
+ * receives the un-normalised complex values; OTOC(t) = F(t)/F(0) is the caller's division.
+ * d_psi is used as work space and destroyed.  Work space: syk_otoc_workspace_bytes (2 vectors + Krylov work).
+ * stats (may be NULL) accumulates over all evolutions. */
+int syk_otoc_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes);
+int syk_otoc(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
+             void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
+             syk_stats* stats, void* stream);
+
+/* Batched over disorder realizations: realization r uses hams[r], state d_psi + r*batch_stride elements, and
+ * writes F_out[r][n_t][2].  One work space is shared (realizations run back to back on `stream`). */
+int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,
+                     const double* t_grid, int n_t, void* d_psi, int64_t batch_stride, double* F_out,
+                     const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Introspection for tests and the benchmark. */
+/* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined tile gather. */
+int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
+/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 as above. */
+int syk_set_apply_H_kernel(syk_ham* h, int kind);
+/* Number of kernels launched by this library on the calling thread since the last reset. */
+int64_t syk_launch_count(int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SYK_B200_H */

@@ -1,0 +1,165 @@
+// Internal declarations of libsyk_b200 (not part of the C ABI; see include/syk.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <complex>
+#include <vector>
+
+#include "../../include/syk.h"
+
+namespace syk {
+
+// ---------------------------------------------------------------------------------------------------------
+// Host tables of one Hamiltonian in canonical order (a-1) and their device copy.
+// ---------------------------------------------------------------------------------------------------------
+struct DeviceTables {
+    uint32_t* gx = nullptr;        // [n_groups]    X-mask of each group
+    uint32_t* goff = nullptr;      // [n_groups+1]  first term of each group
+    uint32_t* tz = nullptr;        // [n_terms]     Z-mask of each term
+    double2* tc128 = nullptr;      // [n_terms]     coefficient (re, im), fp64
+    float2* tc64 = nullptr;        // [n_terms]     coefficient rounded once to fp32 (R-C64)
+    // tile-load lists of the TMA kernel, one per tile size: distinct values of x >> tile_log2 in ascending
+    // order, each with the range of groups it serves
+    uint32_t* load_hi[2] = {nullptr, nullptr};     // [n_loads]    x >> tile_log2
+    uint32_t* load_g0[2] = {nullptr, nullptr};     // [n_loads+1]  first group of each load
+    int n_loads[2] = {0, 0};
+    int device = -1;
+    void* blob = nullptr;          // single allocation holding all of the above
+};
+
+}  // namespace syk
+
+struct syk_ham {
+    int N = 0;
+    int L = 0;
+    int gamma_norm = 0;
+    std::vector<uint64_t> x;                   // [n_groups]
+    std::vector<uint32_t> group_off;           // [n_groups+1]
+    std::vector<uint64_t> z;                   // [n_terms]
+    std::vector<std::complex<double>> c;       // [n_terms]
+    std::vector<int32_t> quartet;              // [n_terms*4]
+    std::vector<double> J;                     // [n_terms]
+    int forced_kernel = -1;                    // syk_set_apply_H_kernel
+    mutable syk::DeviceTables dev;             // created on first device use
+    int64_t n_terms() const { return (int64_t)z.size(); }
+    int64_t n_groups() const { return (int64_t)x.size(); }
+};
+
+namespace syk {
+
+// tile sizes of the TMA kernel (amplitudes per tile), index by dtype (SYK_C64 = 0, SYK_C128 = 1): 16 KiB tiles
+constexpr int kTileLog2[2] = {11, 10};
+constexpr int kMaxKrylov = 128;
+constexpr int kMaxPartials = 4096;            // upper bound on the grid size of any reducing kernel
+
+inline size_t elem_bytes(int dtype) { return dtype == SYK_C128 ? 16 : 8; }
+
+// error plumbing ------------------------------------------------------------------------------------------
+void set_cuda_error(cudaError_t e, const char* what);
+#define SYK_CUDA(call)                                          \
+    do {                                                        \
+        cudaError_t e__ = (call);                               \
+        if (e__ != cudaSuccess) {                               \
+            ::syk::set_cuda_error(e__, #call);                  \
+            return SYK_ECUDA;                                   \
+        }                                                       \
+    } while (0)
+#define SYK_TRY(call)                   \
+    do {                                \
+        int r__ = (call);               \
+        if (r__ != SYK_OK) return r__;  \
+    } while (0)
+
+void count_launch(int n = 1);
+int num_sms();                                 // SM count of the current device (cached); <= 0 on error
+
+// device table management (device_tables.cu)
+int ensure_device_tables(const syk_ham* h);
+void free_device_tables(const syk_ham* h);
+
+// ---------------------------------------------------------------------------------------------------------
+// Scalars of a Lanczos run, resident on the device (a-3): everything the fused kernels need between steps.
+// ---------------------------------------------------------------------------------------------------------
+struct LanczosScalars {
+    double alpha[kMaxKrylov + 2];   // alpha[j], j = 1..m
+    double nrm[kMaxKrylov + 2];     // nrm[j] = |u_j|, u_1 = psi, u_{j+1} = w - alpha_j v_j  (nrm[j+1] = beta_{j+1})
+    double2 coef[kMaxKrylov + 2];   // coef[j] = [exp(-i tau T_m) e_1]_j * nrm[1], uploaded by the host
+    double partial_dot[kMaxPartials];   // per-CTA partial sums of Re<u_j|w> written by apply_H
+    double partial_nrm[kMaxPartials];   // per-CTA partial sums of |.|^2 written by the vector kernels
+    double2 partial_cdot[kMaxPartials]; // per-CTA partial sums of a complex dot product
+    int n_partial_dot;              // how many entries of partial_dot are valid
+    int n_partial_nrm;
+    int n_partial_cdot;
+    int pad;
+};
+
+// What the fused epilogue of apply_H does (all pointers device):
+//   plain : out[b] = acc
+//   fused : out[b] = acc / nrm[j] - (nrm[j]/nrm[j-1]) prev[b]   (second term absent when j == 1)
+//           and partial_dot[cta] = sum_b Re(conj(in[b]) out[b]);
+//           nrm[j] is first reduced from partial_nrm (written by the preceding vector kernel).
+struct FusedArgs {
+    LanczosScalars* sc = nullptr;   // nullptr = plain
+    const void* prev = nullptr;     // u_{j-1}; may alias out; nullptr when j == 1
+    int j = 0;
+};
+
+// apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
+int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                   cudaStream_t stream);
+
+// vector kernels (vector_ops.cu); all reductions go through LanczosScalars partial arrays
+int launch_norm2(int dtype, uint64_t D, const void* d_v, LanczosScalars* sc, cudaStream_t stream);
+// u_next = w - (alpha_j / nrm[j]) u_j in place on w, |u_next|^2 partials; alpha_j reduced from partial_dot.
+// When y != nullptr also y = y_scale * y + (coef[j]/nrm[j]) u_j  with y_scale = coef[1]/nrm[1] if first_y else 1.
+int launch_axpy_norm(int dtype, uint64_t D, void* d_w, const void* d_u, int j, LanczosScalars* sc, void* d_y,
+                     int first_y, cudaStream_t stream);
+// finalises nrm[j] from partial_nrm (used after the last vector kernel of a run); 1 block
+int launch_finalize_nrm(int j, LanczosScalars* sc, cudaStream_t stream);
+// psi = sum_{j=1..m} (coef[j]/nrm[j]) u_j, u_1 = psi itself (in place), u_j (j >= 2) = vecs + (j-2)*stride_elems
+int launch_combine(int dtype, uint64_t D, void* d_psi, const void* d_vecs, uint64_t stride_elems, int m,
+                   LanczosScalars* sc, cudaStream_t stream);
+// y = ys*y + (coef[j]/nrm[j]) u, ys = first_y ? coef[1]/nrm[1] : 1; u == nullptr drops the second term
+int launch_axpy_coef(int dtype, uint64_t D, void* d_y, const void* d_u, int j, int first_y, LanczosScalars* sc,
+                     cudaStream_t stream);
+int launch_cdot(int dtype, uint64_t D, const void* d_a, const void* d_b, LanczosScalars* sc, cudaStream_t stream);
+int fetch_cdot(LanczosScalars* sc, double* re_im, cudaStream_t stream);   // host sum of the partials; synchronises
+int launch_normalise(int dtype, uint64_t D, void* d_v, LanczosScalars* sc, cudaStream_t stream);
+int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, cudaStream_t stream);
+int launch_random_fill(int N, uint64_t seed, uint32_t realization, int dtype, void* d_psi, LanczosScalars* sc,
+                       cudaStream_t stream);
+int apply_h_kernel_kind(const syk_ham* h, int dtype);
+
+// Krylov driver internals shared with the OTOC pipeline (krylov.cu)
+int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im,
+                       const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                       cudaStream_t stream);
+size_t krylov_header_bytes();
+
+// ---------------------------------------------------------------------------------------------------------
+// The counter-based generator R-RNG, host and device.
+// ---------------------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+#define SYK_HD __host__ __device__ __forceinline__
+#else
+#define SYK_HD inline
+#endif
+constexpr uint64_t kGold = 0x9E3779B97F4A7C15ull;
+SYK_HD uint64_t rng_fmix(uint64_t z) {
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return z;
+}
+SYK_HD uint64_t rng_absorb(uint64_t h, uint64_t w) { return rng_fmix((h ^ w) + kGold); }
+SYK_HD uint64_t rng_key(uint64_t seed, uint64_t realization, uint64_t stream) {
+    return rng_absorb(rng_absorb(rng_absorb(0, seed), realization), stream);
+}
+SYK_HD uint64_t rng_draw(uint64_t key, uint64_t index, uint64_t d) {
+    return rng_absorb(rng_absorb(key, index), d) >> 11;
+}
+constexpr uint64_t kStreamHamiltonian = 1, kStreamState = 2;
+
+}  // namespace syk

@@ -1,0 +1,357 @@
+// a-4  Krylov driver: psi <- exp(-i tau H) psi for complex tau (R-TAU, R-KRYLOV).
+//
+// Hermitian Lanczos builds T_m (real symmetric tridiagonal; alpha_j, beta_j) with the fused kernels; the small
+// exponential exp(-i tau T_m) e_1 is taken on the host through a Jacobi eigen-decomposition of T_m; the result is
+// |psi| V_m exp(-i tau T_m) e_1.  T_m does not depend on tau, so after one build the driver picks the longest
+// sub-step h along the ray tau = |tau| e^{i phi} whose a-posteriori error estimate
+//        err(h) = int_0^h beta_{m+1} |e_m^T exp(-i e^{i phi} s T_m) e_1| ds / |exp(-i e^{i phi} h T_m) e_1|
+// (the time integral of the residual norm of y' = -iHy, relative to the result) stays below its share
+// tol * h/|tau| of the budget, applies it, and repeats on the remainder.
+//
+//  one-pass : keeps u_2..u_{m+1} (m work vectors), then psi = sum_j c_j v_j in one fused pass.
+//  two-pass : 2 work vectors P, Q.  Pass 1 runs the recurrence for T_m only; from step 3 on the new vector
+//             overwrites u_{j-1} in place (out aliases prev in the fused apply_H), so psi is untouched.  Pass 2
+//             repeats the identical recurrence (bitwise: fixed reduction trees) and accumulates
+//             y += c_j v_j into psi's own buffer as soon as u_1 is no longer needed.  Replaces the restarted
+//             scheme of PAPER.md:301 as the bounded-memory mode (PAPER.md:249 counts v+3 vectors; this is 3).
+#include <algorithm>
+#include <cmath>
+#include <complex>
+
+#include "common.h"
+
+namespace syk {
+
+size_t krylov_header_bytes() { return (sizeof(LanczosScalars) + 4095) & ~(size_t)4095; }
+
+namespace {
+
+using cplx = std::complex<double>;
+
+// Cyclic Jacobi for a real symmetric matrix A (m x m, row-major, destroyed): eigenvalues theta, eigenvectors in
+// the columns of Q (row-major).  Small m only (<= 128).
+void jacobi_eig(int m, std::vector<double>& A, std::vector<double>& theta, std::vector<double>& Q) {
+    Q.assign((size_t)m * m, 0.0);
+    for (int i = 0; i < m; ++i) Q[(size_t)i * m + i] = 1.0;
+    auto a = [&](int i, int j) -> double& { return A[(size_t)i * m + j]; };
+    for (int sweep = 0; sweep < 100; ++sweep) {
+        double off = 0.0, diag = 0.0;
+        for (int i = 0; i < m; ++i) {
+            diag += a(i, i) * a(i, i);
+            for (int j = i + 1; j < m; ++j) off += a(i, j) * a(i, j);
+        }
+        if (off <= 1e-34 * (diag + off) || off == 0.0) break;
+        for (int p = 0; p < m - 1; ++p)
+            for (int q = p + 1; q < m; ++q) {
+                const double apq = a(p, q);
+                if (apq == 0.0) continue;
+                const double th = (a(q, q) - a(p, p)) / (2.0 * apq);
+                const double t = (th >= 0.0 ? 1.0 : -1.0) / (std::fabs(th) + std::sqrt(th * th + 1.0));
+                const double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
+                for (int k = 0; k < m; ++k) {   // columns p, q
+                    const double akp = a(k, p), akq = a(k, q);
+                    a(k, p) = c * akp - s * akq;
+                    a(k, q) = s * akp + c * akq;
+                }
+                for (int k = 0; k < m; ++k) {   // rows p, q
+                    const double apk = a(p, k), aqk = a(q, k);
+                    a(p, k) = c * apk - s * aqk;
+                    a(q, k) = s * apk + c * aqk;
+                }
+                for (int k = 0; k < m; ++k) {
+                    const double qkp = Q[(size_t)k * m + p], qkq = Q[(size_t)k * m + q];
+                    Q[(size_t)k * m + p] = c * qkp - s * qkq;
+                    Q[(size_t)k * m + q] = s * qkp + c * qkq;
+                }
+            }
+    }
+    theta.resize(m);
+    for (int i = 0; i < m; ++i) theta[i] = a(i, i);
+}
+
+struct SmallExp {
+    int m = 0;
+    std::vector<double> theta, Q;
+    double beta_next = 0.0;   // beta_{m+1}
+    cplx dir;                 // tau / |tau|
+    // component j (0-based) of exp(-i dir s T) e_1
+    cplx comp(int j, double s) const {
+        cplx acc = 0.0;
+        for (int k = 0; k < m; ++k)
+            acc += Q[(size_t)j * m + k] * std::exp(cplx(0.0, -1.0) * dir * (s * theta[k])) * Q[k];
+        return acc;
+    }
+    double result_norm(double s) const {
+        double n2 = 0.0;
+        for (int j = 0; j < m; ++j) n2 += std::norm(comp(j, s));
+        return std::sqrt(n2);
+    }
+    double residual(double s) const { return beta_next * std::abs(comp(m - 1, s)); }
+    // Simpson estimate of int_0^h residual ds / |result(h)|
+    double err(double h) const {
+        if (beta_next == 0.0 || h == 0.0) return 0.0;
+        const int n = 32;
+        double sum = residual(0.0) + residual(h);
+        for (int i = 1; i < n; ++i) sum += residual(h * i / n) * ((i & 1) ? 4.0 : 2.0);
+        const double rn = result_norm(h);
+        return (sum * h / (3.0 * n)) / (rn > 0.0 ? rn : 1.0);
+    }
+};
+
+struct Ctx {
+    const syk_ham* h;
+    int dtype;
+    uint64_t D;
+    size_t vbytes;
+    char* psi;
+    char* vecs;
+    LanczosScalars* sc;
+    bool two_pass;
+    cudaStream_t st;
+    syk_stats* stats;
+    char* buf(int j) const {   // buffer holding u_j
+        if (j == 1) return psi;
+        if (two_pass) return vecs + ((j & 1) ? vbytes : 0);
+        return vecs + (size_t)(j - 2) * vbytes;
+    }
+};
+
+// steps j = 1..n_steps of the recurrence; with_y: two-pass second pass, accumulate y into psi's buffer
+int run_recurrence(const Ctx& c, int n_steps, bool with_y) {
+    SYK_TRY(launch_norm2(c.dtype, c.D, c.psi, c.sc, c.st));
+    for (int j = 1; j <= n_steps; ++j) {
+        FusedArgs fa;
+        fa.sc = c.sc;
+        fa.j = j;
+        fa.prev = j > 1 ? c.buf(j - 1) : nullptr;
+        SYK_TRY(launch_apply_h(c.h, c.dtype, c.buf(j), c.buf(j + 1), fa, c.st));
+        void* y = (with_y && j >= 2) ? c.psi : nullptr;
+        SYK_TRY(launch_axpy_norm(c.dtype, c.D, c.buf(j + 1), c.buf(j), j, c.sc, y, j == 2, c.st));
+        if (c.stats) c.stats->n_matvec += 1;
+    }
+    return SYK_OK;
+}
+
+int fetch_scalars(const Ctx& c, int m, double* alpha, double* nrm) {
+    SYK_CUDA(cudaMemcpyAsync(alpha, c.sc->alpha, sizeof(double) * (size_t)(m + 2), cudaMemcpyDeviceToHost, c.st));
+    SYK_CUDA(cudaMemcpyAsync(nrm, c.sc->nrm, sizeof(double) * (size_t)(m + 2), cudaMemcpyDeviceToHost, c.st));
+    SYK_CUDA(cudaStreamSynchronize(c.st));
+    return SYK_OK;
+}
+
+int effective_dim(int m, const double* alpha, const double* nrm, double eps) {
+    double scale = 0.0;
+    for (int j = 1; j <= m; ++j) {
+        scale = std::max(scale, std::fabs(alpha[j]));
+        if (j >= 2) scale = std::max(scale, nrm[j]);
+        const double b = nrm[j + 1];
+        if (!(b > eps * scale) || !std::isfinite(b)) return j;   // happy breakdown: invariant subspace reached
+    }
+    return m;
+}
+
+bool valid_args(const syk_ham* h, int dtype, const void* psi, const void* work) {
+    return h && (dtype == SYK_C64 || dtype == SYK_C128) && psi && work && ((uintptr_t)psi & 15) == 0 &&
+           ((uintptr_t)work & 15) == 0;
+}
+
+int resolve_dim(const syk_ham* h, const syk_krylov_opts* o) {
+    int m = (o && o->krylov_dim > 0) ? o->krylov_dim : 24;
+    const uint64_t D = 1ull << h->L;
+    if (m > kMaxKrylov) m = kMaxKrylov;
+    if ((uint64_t)m > D) m = (int)D;
+    return m;
+}
+
+}  // namespace
+
+int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im,
+                       const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                       cudaStream_t st) {
+    if (!valid_args(h, dtype, d_psi, d_work) || !std::isfinite(tau_re) || !std::isfinite(tau_im)) return SYK_EINVAL;
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->tol < 0 || opts->max_substeps < 0))
+        return SYK_EINVAL;
+    const int m = resolve_dim(h, opts);
+    const bool two_pass = opts && opts->two_pass;
+    const double tol = (opts && opts->tol > 0) ? opts->tol : (dtype == SYK_C128 ? 1e-12 : 1e-6);
+    const int max_sub = (opts && opts->max_substeps > 0) ? opts->max_substeps : 100000;
+
+    Ctx c;
+    c.h = h;
+    c.dtype = dtype;
+    c.D = 1ull << h->L;
+    c.vbytes = (size_t)c.D * elem_bytes(dtype);
+    c.psi = (char*)d_psi;
+    c.sc = (LanczosScalars*)d_work;
+    c.vecs = (char*)d_work + krylov_header_bytes();
+    c.two_pass = two_pass;
+    c.st = st;
+    c.stats = stats;
+    const size_t need = krylov_header_bytes() + (size_t)(two_pass ? 2 : m) * c.vbytes;
+    if (work_bytes < need) return SYK_ENOMEM;
+    {   // psi must not overlap the work space
+        const uintptr_t a = (uintptr_t)d_psi, b = (uintptr_t)d_work;
+        if (a < b + need && b < a + c.vbytes) return SYK_EINVAL;
+    }
+
+    const double len = std::hypot(tau_re, tau_im);
+    if (len == 0.0 || h->n_terms() == 0) return SYK_OK;
+    const cplx dir(tau_re / len, tau_im / len);
+    const double eps_break = dtype == SYK_C128 ? 1e-13 : 2e-6;
+    const double V = (double)c.vbytes, Dx = (double)h->n_groups();
+
+    double remaining = len;
+    int rc = SYK_OK;
+    std::vector<double> alpha(kMaxKrylov + 2), nrm(kMaxKrylov + 2), A;
+    std::vector<double2> coef(kMaxKrylov + 2);
+    int n_sub = 0;
+    while (remaining > 1e-15 * len) {
+        ++n_sub;
+        SYK_TRY(run_recurrence(c, m, false));
+        SYK_TRY(launch_finalize_nrm(m + 1, c.sc, st));
+        SYK_TRY(fetch_scalars(c, m, alpha.data(), nrm.data()));
+        if (!(nrm[1] > 0.0)) return SYK_OK;   // zero vector stays zero
+        const int me = effective_dim(m, alpha.data(), nrm.data(), eps_break);
+
+        SmallExp se;
+        se.m = me;
+        se.dir = dir;
+        se.beta_next = me < m ? 0.0 : nrm[m + 1];
+        A.assign((size_t)me * me, 0.0);
+        for (int j = 1; j <= me; ++j) {
+            A[(size_t)(j - 1) * me + (j - 1)] = alpha[j];
+            if (j < me) A[(size_t)(j - 1) * me + j] = A[(size_t)j * me + (j - 1)] = nrm[j + 1];
+        }
+        jacobi_eig(me, A, se.theta, se.Q);
+
+        // longest sub-step whose error estimate fits its share of the budget
+        auto fits = [&](double hs) { return se.err(hs) <= tol * hs / len; };
+        double hs = remaining;
+        if (!fits(hs)) {
+            if (n_sub >= max_sub) {
+                rc = SYK_ENOCONV;   // forced: take the remainder in one step
+            } else {
+                double lo = 0.0, hi = remaining;
+                for (int it = 0; it < 60; ++it) {
+                    const double mid = 0.5 * (lo + hi);
+                    if (fits(mid)) lo = mid; else hi = mid;
+                }
+                hs = lo;
+                if (!(hs > 1e-9 * len)) {   // estimate never fits: Krylov space too small for this tolerance
+                    rc = SYK_ENOCONV;
+                    hs = std::min(remaining, std::max(hi, 1e-6 * len));
+                }
+            }
+        }
+        if (stats) {
+            stats->err_est += se.err(hs);
+            stats->krylov_dim_used = stats->krylov_dim_used == 0 ? me : std::min(stats->krylov_dim_used, me);
+            stats->n_substeps += 1;
+        }
+        for (int j = 1; j <= me; ++j) {
+            const cplx v = se.comp(j - 1, hs) * nrm[1];
+            coef[j] = make_double2(v.real(), v.imag());
+        }
+        SYK_CUDA(cudaMemcpyAsync(c.sc->coef, coef.data(), sizeof(double2) * (size_t)(me + 1), cudaMemcpyHostToDevice, st));
+        if (!two_pass) {
+            SYK_TRY(launch_combine(dtype, c.D, c.psi, c.vecs, c.D, me, c.sc, st));
+            if (stats) stats->model_bytes += m * ((Dx + 3.0) * V + 3.0 * V) + V + (me + 1.0) * V;
+        } else {
+            if (me == 1) {
+                SYK_TRY(launch_axpy_coef(dtype, c.D, c.psi, nullptr, 1, 1, c.sc, st));
+            } else {
+                SYK_TRY(run_recurrence(c, me - 1, true));
+                SYK_TRY(launch_axpy_coef(dtype, c.D, c.psi, c.buf(me), me, me == 2, c.sc, st));
+            }
+            if (stats) stats->model_bytes += (m + me - 1) * ((Dx + 3.0) * V + 3.0 * V) + 2.0 * V + 2.0 * me * V;
+        }
+        remaining -= hs;
+    }
+    return rc;
+}
+
+}  // namespace syk
+
+extern "C" {
+
+int syk_krylov_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes) {
+    if (!h || !bytes || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1)) return SYK_EINVAL;
+    const int m = syk::resolve_dim(h, opts);
+    const size_t v = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+    *bytes = syk::krylov_header_bytes() + (size_t)((opts && opts->two_pass) ? 2 : m) * v;
+    return SYK_OK;
+}
+
+int syk_krylov_evolve(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im,
+                      const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (stats) {
+        *stats = syk_stats{};
+        SYK_CUDA(cudaEventCreate(&e0));
+        SYK_CUDA(cudaEventCreate(&e1));
+        SYK_CUDA(cudaEventRecord(e0, st));
+    }
+    int rc = syk::krylov_evolve_impl(h, dtype, d_psi, tau_re, tau_im, opts, d_work, work_bytes, stats, st);
+    if (stats) {
+        if (rc == SYK_OK || rc == SYK_ENOCONV) {
+            float ms = 0.f;
+            if (cudaEventRecord(e1, st) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+                cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess)
+                stats->elapsed_ms = ms;
+        }
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+    }
+    return rc;
+}
+
+int syk_lanczos_run(const syk_ham* h, int dtype, const void* d_psi, int m, double* alpha, double* beta,
+                    void* d_work, size_t work_bytes, syk_stats* stats, void* stream) {
+    if (!syk::valid_args(h, dtype, d_psi, d_work) || !alpha || !beta || m < 1 || m > syk::kMaxKrylov)
+        return SYK_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    syk::Ctx c;
+    c.h = h;
+    c.dtype = dtype;
+    c.D = 1ull << h->L;
+    c.vbytes = (size_t)c.D * syk::elem_bytes(dtype);
+    c.psi = (char*)const_cast<void*>(d_psi);
+    c.sc = (syk::LanczosScalars*)d_work;
+    c.vecs = (char*)d_work + syk::krylov_header_bytes();
+    c.two_pass = false;
+    c.st = st;
+    c.stats = stats;
+    if (work_bytes < syk::krylov_header_bytes() + (size_t)m * c.vbytes) return SYK_ENOMEM;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (stats) {
+        *stats = syk_stats{};
+        SYK_CUDA(cudaEventCreate(&e0));
+        SYK_CUDA(cudaEventCreate(&e1));
+        SYK_CUDA(cudaEventRecord(e0, st));
+    }
+    int rc = syk::run_recurrence(c, m, false);
+    if (rc == SYK_OK) rc = syk::launch_finalize_nrm(m + 1, c.sc, st);
+    if (rc == SYK_OK && stats) {
+        float ms = 0.f;
+        if (cudaEventRecord(e1, st) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+            cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess)
+            stats->elapsed_ms = ms;
+        const double V = (double)c.vbytes;
+        stats->model_bytes = m * ((double)h->n_groups() + 6.0) * V + V;
+        stats->krylov_dim_used = m;
+    }
+    if (stats) {
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+    }
+    SYK_TRY(rc);
+    std::vector<double> a(syk::kMaxKrylov + 2), n(syk::kMaxKrylov + 2);
+    SYK_TRY(syk::fetch_scalars(c, m, a.data(), n.data()));
+    for (int j = 1; j <= m; ++j) alpha[j - 1] = a[j];
+    for (int j = 0; j <= m; ++j) beta[j] = n[j + 1];
+    return SYK_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,145 @@
+// a-5  OTOC pipeline (R-EQ2; random state -> Krylov evolution -> inner product).
+//
+//   F(t) = <psi| E(-t - ib/8) g_W E(t - ib/4) g_V E(-t - ib/4) g_W E(t - ib/4) g_V E(-ib/8) |psi>,  E(tau) = exp(-i tau H)
+//
+// Right to left on the ket, with the bra side l(t) = E(t - ib/8) psi.  Both l(t) and phi(t) = E(t - ib/4) g_V E(-ib/8) psi
+// are advanced incrementally along the (non-decreasing) t grid by E(dt); the two middle evolutions of length t act on
+// t-dependent states and are redone for every grid point:
+//   l    <- E(-ib/8) psi                     (in psi's own buffer; psi is destroyed)
+//   phi  <- E(-ib/4) g_V l
+//   for each t_k:  l <- E(dt) l ; phi <- E(dt) phi
+//                  r <- g_W phi ; r <- E(-t - ib/4) r ; r <- g_V r ; r <- E(t - ib/4) r ; r <- g_W r ;  F_k = <l|r>
+// Resident vectors: l, phi, r + Krylov work (2 in two-pass mode: 5 in total, PAPER.md:249's v+3 with v = 2).
+#include "common.h"
+
+namespace syk {
+
+static int otoc_one(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
+                    void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
+                    syk_stats* stats, cudaStream_t st) {
+    const uint64_t D = 1ull << h->L;
+    const size_t vbytes = (size_t)D * elem_bytes(dtype);
+    size_t kbytes = 0;
+    SYK_TRY(syk_krylov_workspace_bytes(h, dtype, opts, &kbytes));
+    if (work_bytes < 2 * vbytes + kbytes) return SYK_ENOMEM;
+    char* l = (char*)d_psi;
+    char* phi = (char*)d_work;
+    char* r = phi + vbytes;
+    char* kwork = r + vbytes;
+    LanczosScalars* sc = (LanczosScalars*)kwork;   // the Krylov header doubles as reduction scratch between evolutions
+    const int N = h->N, gn = h->gamma_norm;
+    int rc_soft = SYK_OK;
+    auto evolve = [&](void* v, double tre, double tim) -> int {
+        int rc = krylov_evolve_impl(h, dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+        if (rc == SYK_ENOCONV) {
+            rc_soft = rc;
+            return SYK_OK;
+        }
+        return rc;
+    };
+    SYK_TRY(evolve(l, 0.0, -beta / 8.0));
+    SYK_TRY(launch_gamma(N, j_V, gn, dtype, l, phi, st));
+    SYK_TRY(evolve(phi, 0.0, -beta / 4.0));
+    double t_prev = 0.0;
+    for (int k = 0; k < n_t; ++k) {
+        const double t = t_grid[k], dt = t - t_prev;
+        if (dt > 0.0) {
+            SYK_TRY(evolve(l, dt, 0.0));
+            SYK_TRY(evolve(phi, dt, 0.0));
+        }
+        t_prev = t;
+        SYK_TRY(launch_gamma(N, i_W, gn, dtype, phi, r, st));
+        SYK_TRY(evolve(r, -t, -beta / 4.0));
+        SYK_TRY(launch_gamma(N, j_V, gn, dtype, r, r, st));
+        SYK_TRY(evolve(r, t, -beta / 4.0));
+        SYK_TRY(launch_gamma(N, i_W, gn, dtype, r, r, st));
+        SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
+        SYK_TRY(fetch_cdot(sc, F_out + 2 * k, st));
+    }
+    return rc_soft;
+}
+
+static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
+                         const void* d_psi, const double* F_out, const void* d_work) {
+    if (!h || (dtype != SYK_C64 && dtype != SYK_C128) || !d_psi || !d_work || n_t < 0 || (n_t > 0 && (!t_grid || !F_out)))
+        return false;
+    if (((uintptr_t)d_psi & 15) || ((uintptr_t)d_work & 15)) return false;
+    if (i_W < 0 || i_W >= h->N || j_V < 0 || j_V >= h->N || i_W == j_V || !(beta >= 0.0)) return false;
+    double prev = 0.0;
+    for (int k = 0; k < n_t; ++k) {
+        if (!(t_grid[k] >= prev)) return false;
+        prev = t_grid[k];
+    }
+    return true;
+}
+
+}  // namespace syk
+
+extern "C" {
+
+int syk_otoc_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes) {
+    size_t k = 0;
+    SYK_TRY(syk_krylov_workspace_bytes(h, dtype, opts, &k));
+    *bytes = k + 2 * ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+    return SYK_OK;
+}
+
+int syk_otoc(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t, void* d_psi,
+             double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+             void* stream) {
+    if (!syk::otoc_args_ok(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, d_work)) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    return syk::otoc_one(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, opts, d_work, work_bytes, stats,
+                         (cudaStream_t)stream);
+}
+
+int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,
+                     const double* t_grid, int n_t, void* d_psi, int64_t batch_stride, double* F_out,
+                     const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream) {
+    if (!hams || n_batch < 0) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    int rc_soft = SYK_OK;
+    for (int r = 0; r < n_batch; ++r) {
+        if (!hams[r] || hams[r]->N != hams[0]->N || batch_stride < ((int64_t)1 << hams[r]->L)) return SYK_EINVAL;
+        char* psi = (char*)d_psi + (size_t)r * (size_t)batch_stride * syk::elem_bytes(dtype);
+        if (!syk::otoc_args_ok(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out, d_work)) return SYK_EINVAL;
+        int rc = syk::otoc_one(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out + (size_t)r * 2 * n_t, opts,
+                               d_work, work_bytes, stats, (cudaStream_t)stream);
+        if (rc == SYK_ENOCONV) rc_soft = rc;
+        else if (rc != SYK_OK) return rc;
+    }
+    return rc_soft;
+}
+
+// ---- HOST-buffer entry points: the same calls with the host<->device copies inside ---------------------------
+int syk_apply_H_host(const syk_ham* h, int dtype, const void* h_in, void* h_out, void* d_work, size_t work_bytes,
+                     void* stream) {
+    if (!h || !h_in || !h_out || !d_work || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    const size_t v = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+    if (work_bytes < 2 * v) return SYK_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* din = (char*)d_work;
+    char* dout = din + v;
+    SYK_CUDA(cudaMemcpyAsync(din, h_in, v, cudaMemcpyHostToDevice, st));
+    SYK_TRY(syk_apply_H(h, dtype, din, dout, stream));
+    SYK_CUDA(cudaMemcpyAsync(h_out, dout, v, cudaMemcpyDeviceToHost, st));
+    SYK_CUDA(cudaStreamSynchronize(st));
+    return SYK_OK;
+}
+
+int syk_krylov_evolve_host(const syk_ham* h, int dtype, void* h_psi, double tau_re, double tau_im,
+                           const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                           void* stream) {
+    if (!h || !h_psi || !d_work || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    const size_t v = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+    if (work_bytes < v) return SYK_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    SYK_CUDA(cudaMemcpyAsync(d_work, h_psi, v, cudaMemcpyHostToDevice, st));
+    int rc = syk_krylov_evolve(h, dtype, d_work, tau_re, tau_im, opts, (char*)d_work + v, work_bytes - v, stats, stream);
+    if (rc != SYK_OK && rc != SYK_ENOCONV) return rc;
+    SYK_CUDA(cudaMemcpyAsync(h_psi, d_work, v, cudaMemcpyDeviceToHost, st));
+    SYK_CUDA(cudaStreamSynchronize(st));
+    return rc;
+}
+
+}  // extern "C"
