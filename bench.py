@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""Benchmark of the sparse-SYK hot path on B200 (contract: see DESIGN.md section 8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one synthetic realization:
+    a-1  syk_build_hamiltonian(N, p = kN/C(N,4), seed, realization)          (host term compiler + table upload)
+    a-5  r <- gamma_W phi                                                    (Pauli-string insertion)
+    a-4  r <- exp(-i (dt - i beta/4 ...) H) r   via syk_krylov_evolve        (m fused Lanczos steps = a-2 + a-3,
+                                                                              host exp(-i tau T_m), combine)
+    a-5  F = <l | r>                                                         (fp64 inner product)
+i.e. one Krylov segment of the OTOC sandwich of PAPER.md:230.  `value` is BASELINE.json's metric, H.v model
+bytes per second: the byte model of DESIGN.md section 6 ((D_x + 2) V per matvec + 3 V per fused vector pass
++ combine) divided by the device time of the step.  The `roofline` object is for the dominant kernel (apply_H)
+alone, timed with CUDA events around each of its launches inside the timed region.
+
+N > 1 (torchrun): realizations are independent, so each rank runs its own realization with no
+data-path collective ("weak" scaling); the time is the max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/alg1.c, the paper's Algorithm 1 under OpenMP) on the host cores.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Hv_model_bytes_throughput"
+UNIT = "GB/s"
+
+WORKLOADS = {
+    # BASELINE.json configs[3] and configs[4]; krylov_dim/dt: one OTOC time segment (t in [0,8], 16 segments)
+    "N56_k4_c128": {"N": 56, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
+                    "i_W": 55, "j_V": 54},
+    "N64_k2_c64": {"N": 64, "k": 2, "dtype": "c64", "krylov_dim": 8, "two_pass": 1, "dt": 0.5, "beta": 5.0,
+                   "i_W": 63, "j_V": 62},
+    # smaller shapes of the same path (parity-test sizes; handy for quick runs and ncu)
+    "N48_k4_c128": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
+                    "i_W": 47, "j_V": 46},
+    "N40_k4_c128": {"N": 40, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
+                    "i_W": 39, "j_V": 38},
+}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=10)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in out.splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax.append(float(parts[1]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def fill_host_state(buf_np, seed):
+    """iid complex Gaussian amplitudes, normalised, written in chunks into a (pinned) host array."""
+    import numpy as np
+    r = np.random.default_rng(seed)
+    D = buf_np.shape[0]
+    chunk = 1 << 22
+    n2 = 0.0
+    for lo in range(0, D, chunk):
+        hi = min(D, lo + chunk)
+        re = r.standard_normal(hi - lo)
+        im = r.standard_normal(hi - lo)
+        n2 += float(re @ re + im @ im)
+        buf_np[lo:hi] = (re + 1j * im).astype(buf_np.dtype)
+    scale = 1.0 / math.sqrt(n2)
+    for lo in range(0, D, chunk):
+        buf_np[lo:lo + chunk] *= scale
+
+
+def cpu_oracle_matvec_rate(N, k, seed, target_seconds, psi=None):
+    """Times oracle/alg1.c (literal Algorithm 1 + OpenMP) on a bounded sample of rows of the same workload.
+    Returns (model GB/s, cores, sample description, seconds)."""
+    import numpy as np
+    from oracle import alg1, rng as orng
+    from paper_2311_00639_b200 import inputs
+    L = N // 2
+    D = 1 << L
+    q, J, _ = orng.sample_couplings(N, inputs.bernoulli_p(N, k), seed, 0)
+    bits, coeff = alg1.hamiltonian_tuples(N, q, J)
+    n_x = len(set(int(b) & 0x5555555555555555 for b in bits))          # distinct X parts of the paper's tuples
+    if psi is None:
+        psi = np.empty(D, dtype=np.complex128)
+        fill_host_state(psi, seed + 1)
+    cores = alg1.num_threads()
+    rows = min(D, 1 << 16)
+    t0 = time.perf_counter()
+    alg1.apply_c(L, bits, coeff, psi, 0, rows)
+    t_probe = time.perf_counter() - t0
+    rows = int(min(D, max(rows, rows * target_seconds / max(t_probe, 1e-6))))
+    rows = 1 << int(math.log2(rows))
+    t0 = time.perf_counter()
+    alg1.apply_c(L, bits, coeff, psi, 0, rows)
+    dt = time.perf_counter() - t0
+    gbs = (n_x + 2) * 16.0 * rows / dt / 1e9
+    return gbs, cores, f"rows [0, 2^{int(math.log2(rows))}) of one N={N} k={k} complex128 matvec ({len(J)} terms)", dt, rows
+
+
+def run_reference(args, wl, name):
+    """The reference arm: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    import numpy as np
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import alg1, rng as orng
+    from paper_2311_00639_b200 import inputs
+    N, k = wl["N"], wl["k"]
+    L, D = N // 2, 1 << (N // 2)
+    q, J, _ = orng.sample_couplings(N, inputs.bernoulli_p(N, k), 0, 0)
+    bits, coeff = alg1.hamiltonian_tuples(N, q, J)
+    n_x = len(set(int(b) & 0x5555555555555555 for b in bits))
+    psi = np.empty(D, dtype=np.complex128)
+    fill_host_state(psi, 1)
+    cores = alg1.num_threads()
+    budget = 120.0 / max(1, args.steps + args.warmup)              # whole run within a few minutes
+    rows = 1 << 16
+    t0 = time.perf_counter()
+    alg1.apply_c(L, bits, coeff, psi, 0, rows)
+    probe = time.perf_counter() - t0
+    rows = 1 << int(math.log2(min(D, max(rows, rows * budget / max(probe, 1e-6)))))
+    for _ in range(args.warmup):
+        alg1.apply_c(L, bits, coeff, psi, 0, rows)
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        lo = (s * rows) % D
+        alg1.apply_c(L, bits, coeff, psi, lo, lo + rows)
+    dt = time.perf_counter() - t0
+    value = (n_x + 2) * 16.0 * rows * args.steps / dt / 1e9
+    sample = (f"each step = rows of 2^{int(math.log2(rows))} consecutive outputs of one N={N} k={k} complex128 "
+              f"H.v by oracle/alg1.c (literal Algorithm 1, OpenMP)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "N": N, "k": k, "n_terms": int(len(J)), "n_xmasks": n_x},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, wl, name):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2311_00639_b200 import binding as B, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    N, k = wl["N"], wl["k"]
+    D = 1 << (N // 2)
+    tdt = torch.complex128 if wl["dtype"] == "c128" else torch.complex64
+    code = B.SYK_C128 if wl["dtype"] == "c128" else B.SYK_C64
+    eb = 16 if wl["dtype"] == "c128" else 8
+    V = D * eb
+    p = inputs.bernoulli_p(N, k)
+    opts = {"krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"]}
+    tau = (wl["dt"], 0.0)                            # one real-time segment of the t grid
+    realization = rank                               # independent realizations per rank (weak scaling)
+
+    h0 = B.syk_build_hamiltonian(N, p, 0, realization)
+    info = h0.info()
+    n_x, n_t = info["n_xmasks"], info["n_terms"]
+    kbytes = B.syk_krylov_workspace_bytes(h0, code, opts)
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    wk = torch.empty(kbytes + V, dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
+    phi = torch.empty(D, dtype=tdt, device="cuda")
+    l = torch.empty(D, dtype=tdt, device="cuda")
+    r = torch.empty(D, dtype=tdt, device="cuda")
+    B.syk_random_state(N, 0, realization, phi, scratch)
+    B.syk_apply_gamma(N, wl["j_V"], phi, l)          # a second, different state for the bra side
+    torch.cuda.synchronize()
+
+    stats_acc = {"n_matvec": 0, "model_bytes": 0.0, "n_substeps": 0}
+
+    def step():
+        h = B.syk_build_hamiltonian(N, p, 0, realization)                         # a-1
+        B.syk_apply_gamma(N, wl["i_W"], phi, r)                                   # a-5 insertion
+        st = B.syk_krylov_evolve(h, r, tau[0], tau[1], wk, opts)                  # a-2, a-3, a-4
+        F = B.syk_dot(N, l, r, scratch)                                           # a-5 inner product
+        stats_acc["n_matvec"] += st["n_matvec"]
+        stats_acc["n_substeps"] += st["n_substeps"]
+        stats_acc["model_bytes"] += st["model_bytes"] + 4.0 * V                   # gamma: 2V, dot: 2V
+        h.close()
+        return F
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    for key in stats_acc:
+        stats_acc[key] = 0
+    B.syk_launch_count(reset=True)
+    B.syk_profile_enable(True)
+    B.syk_profile_read(reset=True)
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    F_last = None
+    for _ in range(args.steps):
+        F_last = step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    launches = B.syk_launch_count(reset=True)
+    apply_ms, apply_n = B.syk_profile_read(reset=True)
+    B.syk_profile_enable(False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+        tot = torch.tensor([stats_acc["model_bytes"], float(stats_acc["n_matvec"]), float(launches)],
+                           dtype=torch.float64, device="cuda")
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        total_bytes, total_matvec, launches = float(tot[0]), float(tot[1]), int(tot[2])
+    else:
+        total_bytes, total_matvec = stats_acc["model_bytes"], float(stats_acc["n_matvec"])
+    value = total_bytes / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the HOST entry point: pinned host vector in, evolved vector out, every step ----
+    e2e = None
+    try:
+        host = torch.empty(D, dtype=tdt).pin_memory()
+        fill_host_state(host.numpy(), 7 + rank)
+        def e2e_step():
+            h = B.syk_build_hamiltonian(N, p, 0, realization)
+            st = B.syk_krylov_evolve_host(h, host, tau[0], tau[1], wk, opts)
+            h.close()
+            return st
+        e2e_step()
+        barrier()
+        n_e2e = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        e2e_bytes = 0.0
+        for _ in range(n_e2e):
+            e2e_bytes += e2e_step()["model_bytes"]
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            b = torch.tensor([e2e_bytes], dtype=torch.float64, device="cuda")
+            dist.all_reduce(b, op=dist.ReduceOp.SUM)
+            t_e2e, e2e_bytes = float(t[0]), float(b[0])
+        e2e = {"value": e2e_bytes / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": V, "d2h_bytes_per_step": V,
+               "steps": n_e2e, "call": "syk_krylov_evolve_host (pinned host vector in and out each step)"}
+        del host
+    except Exception as ex:   # noqa: BLE001 -- report, do not hide
+        e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peak()
+    per_launch_bytes = (n_x + 2) * V
+    avg_ms = apply_ms / apply_n if apply_n else float("nan")
+    achieved = per_launch_bytes / (avg_ms * 1e-3) / 1e9 if apply_n else None
+    roofline = {"bound": "hbm", "kernel": "apply_h_tma_kernel" if B.syk_apply_H_kernel_kind(h0, code) == 1
+                else "apply_h_generic_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak if achieved else None, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms, "launches_timed": apply_n,
+                "share_of_step": apply_ms / ms if ms else None,
+                "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None}
+    traffic_file = os.path.join(ROOT, "profiles", f"traffic_{name}.json")
+    if os.path.exists(traffic_file):
+        try:
+            roofline["traffic"] = json.load(open(traffic_file))["dram_bytes_per_launch"]
+        except Exception:
+            pass
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        try:
+            gbs, cores, sample, secs, rows = cpu_oracle_matvec_rate(N, k, 0, 15.0)
+            cpu = {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                   "seconds": secs}
+        except Exception as ex:   # noqa: BLE001
+            cpu = {"value": None, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": repr(ex)[:200]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if wl["dtype"] == "c128" else "f32", "data": "synthetic",
+            "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2, "n_terms": n_t, "n_xmasks": n_x,
+                       "vector_bytes": V, "krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"],
+                       "tau": list(tau), "realizations_per_gpu": 1,
+                       "l2_policy": "inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9),
+                       "step": "build_hamiltonian + gamma insertion + krylov_evolve (m fused Lanczos steps, "
+                               "host exp, combine) + inner product"},
+            "lanczos_steps_per_s": total_matvec / (ms * 1e-3), "matvecs_per_step": total_matvec / args.steps / world,
+            "F_last": [F_last.real, F_last.imag], "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="N56_k4_c128", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("note: fewer than 3 warm-up steps; not a valid bench number", file=sys.stderr)
+    wl = WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, wl, args.workload)
+    else:
+        run_ours(args, wl, args.workload)
+
+
+if __name__ == "__main__":
+    main()

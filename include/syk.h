@@ -172,6 +172,13 @@ int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
 /* Number of kernels launched by this library on the calling thread since the last reset. */
 int64_t syk_launch_count(int reset);
+/* Per-kernel device timing for the benchmark's roofline line.  While enabled, every apply_H launch made by the
+ * calling thread (direct or inside syk_lanczos_run / syk_krylov_evolve / syk_otoc) is bracketed by two CUDA
+ * events on its stream (at most 65536 launches are recorded; later ones are counted but not timed).
+ * syk_profile_read synchronises those events and returns their summed duration, the number of timed launches
+ * and, when `reset` is non-zero, forgets them.  Any output pointer may be NULL. */
+int syk_profile_enable(int on);
+int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset);
 
 #ifdef __cplusplus
 }

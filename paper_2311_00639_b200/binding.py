@@ -75,6 +75,8 @@ _SIGNATURES = {
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
     "syk_set_apply_H_kernel": (_i, [_vp, _i]),
     "syk_launch_count": (_i64, [_i]),
+    "syk_profile_enable": (_i, [_i]),
+    "syk_profile_read": (_i, [_P(_d), _P(_i64), _i]),
 }
 for _name, (_res, _args) in _SIGNATURES.items():
     _fn = getattr(_lib, _name)
@@ -341,6 +343,17 @@ def syk_set_apply_H_kernel(h, kind):
 
 def syk_launch_count(reset=False):
     return int(_lib.syk_launch_count(1 if reset else 0))
+
+
+def syk_profile_enable(on):
+    _check(_lib.syk_profile_enable(1 if on else 0), "syk_profile_enable")
+
+
+def syk_profile_read(reset=True):
+    """(summed apply_H device time in ms, number of timed apply_H launches)."""
+    ms, n = ctypes.c_double(), ctypes.c_int64()
+    _check(_lib.syk_profile_read(ctypes.byref(ms), ctypes.byref(n), 1 if reset else 0), "syk_profile_read")
+    return ms.value, n.value
 
 
 def syk_version():

@@ -376,8 +376,11 @@ int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, c
                    cudaStream_t stream) {
     SYK_TRY(ensure_device_tables(h));
     const int kind = apply_h_kernel_kind(h, dtype);
-    if (dtype == SYK_C128) return launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream);
-    return launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
+    profile_begin(stream);
+    const int rc = dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
+                                     : launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
+    profile_end(stream);
+    return rc;
 }
 
 }  // namespace syk

@@ -73,6 +73,9 @@ void set_cuda_error(cudaError_t e, const char* what);
     } while (0)
 
 void count_launch(int n = 1);
+// benchmark timing of apply_H launches (syk_profile_*): no-ops unless enabled
+void profile_begin(cudaStream_t st);
+void profile_end(cudaStream_t st);
 int num_sms();                                 // SM count of the current device (cached); <= 0 on error
 
 // device table management (device_tables.cu)

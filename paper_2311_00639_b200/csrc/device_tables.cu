@@ -2,6 +2,7 @@
 // error text, launch counter, SM count.
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "common.h"
 
@@ -16,6 +17,44 @@ void set_cuda_error(cudaError_t e, const char* what) {
 }
 
 void count_launch(int n) { g_launches += n; }
+
+// ---- syk_profile_*: event pairs around apply_H launches ----------------------------------------------------
+struct ProfileState {
+    bool on = false;
+    std::vector<cudaEvent_t> ev;   // pairs (begin, end)
+    size_t used = 0;               // events recorded
+    int64_t untimed = 0;
+    bool open = false;
+};
+static thread_local ProfileState g_prof;
+constexpr size_t kMaxProfileEvents = 2 * 65536;
+
+void profile_begin(cudaStream_t st) {
+    ProfileState& p = g_prof;
+    p.open = false;
+    if (!p.on) return;
+    if (p.used + 2 > kMaxProfileEvents) {
+        ++p.untimed;
+        return;
+    }
+    while (p.ev.size() < p.used + 2) {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) {
+            cudaGetLastError();
+            ++p.untimed;
+            return;
+        }
+        p.ev.push_back(e);
+    }
+    if (cudaEventRecord(p.ev[p.used], st) == cudaSuccess) p.open = true;
+}
+
+void profile_end(cudaStream_t st) {
+    ProfileState& p = g_prof;
+    if (!p.open) return;
+    p.open = false;
+    if (cudaEventRecord(p.ev[p.used + 1], st) == cudaSuccess) p.used += 2;
+}
 
 int num_sms() {
     static thread_local int cached_dev = -1, cached = 0;
@@ -141,6 +180,29 @@ const char* syk_strerror(int code) {
 const char* syk_last_cuda_error(void) { return syk::g_cuda_error.c_str(); }
 
 int syk_version(void) { return 100; }
+
+int syk_profile_enable(int on) {
+    syk::g_prof.on = on != 0;
+    return SYK_OK;
+}
+
+int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset) {
+    syk::ProfileState& p = syk::g_prof;
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < p.used; i += 2) {
+        SYK_CUDA(cudaEventSynchronize(p.ev[i + 1]));
+        float ms = 0.f;
+        SYK_CUDA(cudaEventElapsedTime(&ms, p.ev[i], p.ev[i + 1]));
+        total += ms;
+    }
+    if (apply_h_ms) *apply_h_ms = total;
+    if (apply_h_launches) *apply_h_launches = (int64_t)(p.used / 2);
+    if (reset) {
+        p.used = 0;
+        p.untimed = 0;
+    }
+    return SYK_OK;
+}
 
 int64_t syk_launch_count(int reset) {
     int64_t v = syk::g_launches;

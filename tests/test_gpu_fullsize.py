@@ -1,0 +1,132 @@
+"""Parity at BASELINE.json's full sizes (N=56 complex128, N=64 complex64), in the launch configuration bench.py
+times.  No oracle can hold these vectors, so outputs are checked (i) on sampled indices b, each evaluated one by
+one by the oracle from rows of the term matrices (pin P13: out[b] = sum_t H[b, col_t] in[col_t], the inputs
+fetched from the device at the oracle's column indices), and (ii) through properties that hold at any size
+(pins P2, P3): Hermiticity, exact parity-sector zeros, the second-moment sum rule.
+"""
+import numpy as np
+import pytest
+
+from oracle import hamiltonian as ohm
+from oracle import rng as orng
+from paper_2311_00639_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2311_00639_b200 import binding
+    return binding
+
+
+def _free_gb():
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    return free / 2 ** 30
+
+
+def _oracle_samples(N, q, J, idx, d_in):
+    """out[b] for b in idx by the oracle's monomial rows; in[col] is read back from the device."""
+    import torch
+    cols, vals = ohm.hamiltonian_rows(N, q, J, idx)                      # [T, n] each
+    flat = torch.from_numpy(cols.astype(np.int64).reshape(-1)).cuda()
+    src = d_in[flat].cpu().numpy().astype(np.complex128).reshape(cols.shape)
+    return (vals * src).sum(axis=0)
+
+
+def _fullsize_case(B, N, k, tdt, tol, n_samples):
+    import torch
+    D = 1 << (N // 2)
+    p = inputs.bernoulli_p(N, k)
+    q, J, _ = orng.sample_couplings(N, p, 0, 0)
+    h = B.syk_build_hamiltonian(N, p, 0, 0)
+    assert h.info()["n_terms"] == len(J)
+    code = B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64
+    assert B.syk_apply_H_kernel_kind(h, code) == 1                        # the kernel bench.py times
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    d_in = torch.empty(D, dtype=tdt, device="cuda")
+    d_out = torch.empty(D, dtype=tdt, device="cuda")
+    B.syk_random_state(N, 0, 0, d_in, scratch)
+    B.syk_apply_H(h, d_in, d_out)
+    torch.cuda.synchronize()
+    # (i) sampled outputs, including the first/last amplitude and the first/last tile of the vector
+    idx = inputs.sample_indices(D, n_samples, seed=17)
+    edge = np.array([1, 1023, 1024, D // 2 - 1, D // 2, D - 1024, D - 2], dtype=np.uint64)
+    idx = np.unique(np.concatenate([idx, edge]))
+    ref = _oracle_samples(N, q, J, idx, d_in)
+    got = d_out[torch.from_numpy(idx.astype(np.int64)).cuda()].cpu().numpy().astype(np.complex128)
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert np.max(np.abs(got - ref)) <= tol * scale * 10, float(np.max(np.abs(got - ref)) / scale)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= tol
+    # (ii) sum rule: |H psi|^2 = <psi|H^2|psi> ~ Tr H^2 / D = sum J^2 (s = 1), fluctuation O(D^-1/2)
+    n2 = B.syk_dot(N, d_out, d_out, scratch).real
+    assert abs(n2 / float(np.sum(J ** 2)) - 1.0) <= 5e-3
+    alpha = B.syk_dot(N, d_in, d_out, scratch)
+    assert abs(alpha.imag) <= (1e-12 if code == B.SYK_C128 else 1e-6)    # <psi|H|psi> real
+    return h, d_in, d_out, scratch
+
+
+def test_apply_H_N56_c128_sampled(B):
+    """BASELINE configs[3]: N=56, k=4, complex128 (2 x 4.3 GB)."""
+    import torch
+    if _free_gb() < 12:
+        pytest.skip("needs 12 GB of device memory")
+    h, d_in, d_out, scratch = _fullsize_case(B, 56, 4, torch.complex128, 1e-10, 1500)
+    # parity sectors: zero the odd-popcount amplitudes of the input -> odd-popcount outputs are EXACTLY zero
+    D = d_in.numel()
+    step = 1 << 24
+    for lo in range(0, D, step):
+        b = torch.arange(lo, lo + step, device="cuda", dtype=torch.int64)
+        par = b ^ (b >> 16)
+        par = par ^ (par >> 8)
+        par = par ^ (par >> 4)
+        par = par ^ (par >> 2)
+        par = (par ^ (par >> 1)) & 1
+        d_in[lo:lo + step] = torch.where(par == 0, d_in[lo:lo + step], torch.zeros((), dtype=d_in.dtype, device="cuda"))
+        del b
+    B.syk_apply_H(h, d_in, d_out)
+    worst = 0.0
+    for lo in range(0, D, step):
+        b = torch.arange(lo, lo + step, device="cuda", dtype=torch.int64)
+        par = b ^ (b >> 16)
+        par = par ^ (par >> 8)
+        par = par ^ (par >> 4)
+        par = par ^ (par >> 2)
+        par = (par ^ (par >> 1)) & 1
+        worst = max(worst, float((d_out[lo:lo + step].abs() * par).max()))
+    assert worst == 0.0
+
+
+def test_apply_H_N64_c64_sampled(B):
+    """BASELINE configs[4]: N=64, k=2, complex64 (2 x 34.4 GB): 64-bit indexing end to end."""
+    import torch
+    if _free_gb() < 72:
+        pytest.skip("needs 72 GB of device memory")
+    _fullsize_case(B, 64, 2, torch.complex64, 1e-5, 1500)
+
+
+def test_lanczos_step_N56_hermiticity(B):
+    """Fused Lanczos steps at N=56 (the configuration bench.py times): alpha_1 = <v|H|v> and
+    beta_2^2 = <v|H^2|v> - alpha_1^2 with both right-hand sides from separate apply_H + dot calls."""
+    import torch
+    if _free_gb() < 24:
+        pytest.skip("needs 24 GB of device memory")
+    N = 56
+    D = 1 << 28
+    h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 0, 0)
+    m = 2
+    wk = torch.empty(B.syk_krylov_workspace_bytes(h, B.SYK_C128, {"krylov_dim": m}), dtype=torch.uint8, device="cuda")
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    psi = torch.empty(D, dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, 0, 1, psi, scratch)
+    alpha, beta, st = B.syk_lanczos_run(h, psi, m, wk)
+    Hpsi = torch.empty_like(psi)
+    B.syk_apply_H(h, psi, Hpsi)
+    a1 = B.syk_dot(N, psi, Hpsi, scratch).real
+    h2 = B.syk_dot(N, Hpsi, Hpsi, scratch).real
+    assert abs(beta[0] - 1.0) <= 1e-13
+    assert abs(alpha[0] - a1) <= 1e-13
+    assert abs(beta[1] ** 2 - (h2 - a1 * a1)) <= 1e-12

@@ -1,0 +1,509 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.  Needs a B200.
+
+Tolerances (BASELINE.json north_star): relative L2 error <= 1e-10 for complex128, <= 1e-5 for complex64;
+integer tables bit-exact (tests/test_host_library.py).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import evolve as oev
+from oracle import hamiltonian as ohm
+from oracle import majorana
+from oracle import otoc as ootoc
+from oracle import rng as orng
+from paper_2311_00639_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-10, "c64": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_00639_b200 import binding   # raises if the library is not built: no CPU path
+    return binding
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+def tdtype(torch, name):
+    return torch.complex128 if name == "c128" else torch.complex64
+
+
+def npdtype(name):
+    return np.complex128 if name == "c128" else np.complex64
+
+
+def relerr(a, b):
+    a = np.asarray(a, dtype=np.complex128)
+    b = np.asarray(b, dtype=np.complex128)
+    nb = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / (nb if nb > 0 else 1.0))
+
+
+def to_dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def work(torch, nbytes):
+    return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device="cuda")
+
+
+def couplings(N, k, seed=0, realization=0):
+    return orng.sample_couplings(N, inputs.bernoulli_p(N, k), seed, realization)[:2]
+
+
+# ------------------------------------------------------------------------------------------------------------
+# a-2 apply_H
+# ------------------------------------------------------------------------------------------------------------
+APPLY_CASES = [
+    # N, k (None = dense), gamma_norm
+    (4, None, 0), (6, None, 1), (8, None, 0), (12, None, 0), (16, None, 0), (16, 4, 1),
+    (20, 4, 0), (22, 8, 0), (24, 4, 0), (26, 2, 0),
+]
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+@pytest.mark.parametrize("N,k,gn", APPLY_CASES)
+def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
+    """out = H.in against the oracle's sequential-gamma product (O5), both kernels."""
+    q, J = couplings(N, k, seed=1)
+    D = 1 << (N // 2)
+    v = inputs.gaussian_state(D, seed=100 + N, dtype=npdtype(dt))
+    ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128), gn)
+    h = B.syk_build_from_terms(N, q, J, gn)
+    d_in = to_dev(torch, v)
+    kinds = {0}
+    B.syk_set_apply_H_kernel(h, 1)
+    kinds.add(B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)))
+    for kind in sorted(kinds):
+        B.syk_set_apply_H_kernel(h, kind)
+        assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
+        d_out = torch.full((D,), complex(float("nan"), float("nan")), dtype=tdtype(torch, dt), device="cuda")
+        B.syk_apply_H(h, d_in, d_out)
+        torch.cuda.synchronize()
+        assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt], (kind, N, dt)
+        assert np.array_equal(d_in.cpu().numpy(), v), "apply_H modified its input"
+
+
+def test_apply_H_tma_kernel_is_selected_for_sparse(B, torch):
+    """The sm_100a tile kernel must be the default whenever the vector spans at least one tile."""
+    q, J = couplings(32, 4)
+    h = B.syk_build_from_terms(32, q, J)
+    assert B.syk_apply_H_kernel_kind(h, B.SYK_C128) == 1
+    assert B.syk_apply_H_kernel_kind(h, B.SYK_C64) == 1
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+@pytest.mark.parametrize("qubits", [(0, 1, 2, 3, 4), (0, 3, 7, 9, 11), (10, 11, 12, 13), (5, 10, 11, 12, 13)])
+def test_apply_H_structured_masks(B, torch, qubits, dt):
+    """Mask sets confined to the warp-local bits, the tile-local bits, only bits above the tile, and mixed."""
+    N = 28
+    q, J = inputs.quartets_on_qubits(qubits, 40, seed=5, sigma=0.3)
+    D = 1 << (N // 2)
+    v = inputs.gaussian_state(D, seed=3, dtype=npdtype(dt))
+    ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
+    h = B.syk_build_from_terms(N, q, J)
+    d_in = to_dev(torch, v)
+    for kind in (0, 1):
+        B.syk_set_apply_H_kernel(h, kind)
+        d_out = torch.zeros(D, dtype=tdtype(torch, dt), device="cuda")
+        B.syk_apply_H(h, d_in, d_out)
+        assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt]
+
+
+def test_apply_H_literal_algorithm1(B, torch):
+    """Third route (pin P6): the paper's Algorithm 1 transcribed literally in C equals the CUDA result."""
+    from oracle import alg1
+    N = 24
+    q, J = couplings(N, 4, seed=2)
+    D = 1 << (N // 2)
+    v = inputs.gaussian_state(D, seed=9)
+    bits, coeff = alg1.hamiltonian_tuples(N, q, J)
+    ref = alg1.apply_c(N // 2, bits, coeff, v)
+    h = B.syk_build_from_terms(N, q, J)
+    d_out = torch.zeros(D, dtype=torch.complex128, device="cuda")
+    B.syk_apply_H(h, to_dev(torch, v), d_out)
+    assert relerr(d_out.cpu().numpy(), ref) <= 1e-13
+
+
+def test_apply_H_edge_cases(B, torch):
+    # empty Hamiltonian: out = 0
+    h0 = B.syk_build_from_terms(16, np.zeros((0, 4), dtype=np.int32), np.zeros(0))
+    v = to_dev(torch, inputs.gaussian_state(256, 1))
+    out = torch.full((256,), 7.0 + 1j, dtype=torch.complex128, device="cuda")
+    B.syk_apply_H(h0, v, out)
+    assert float(out.abs().max()) == 0.0
+    # in == out and overlapping buffers are refused
+    h = B.syk_build_hamiltonian(16, 1.0, 0)
+    with pytest.raises(B.SykError):
+        B.syk_apply_H(h, v, v)
+    big = torch.zeros(256 + 128, dtype=torch.complex128, device="cuda")
+    with pytest.raises(B.SykError):
+        B.syk_apply_H(h, big[:256], big[128:])
+    # unaligned pointer
+    raw = torch.zeros(2 * 258, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.SykError):
+        B._check(B._lib.syk_apply_H(h.handle, B.SYK_C128, raw.data_ptr() + 8, out.data_ptr(), 0), "apply")
+    # a CPU tensor is refused by the binding: there is no CPU path
+    with pytest.raises(B.SykError):
+        B.syk_apply_H(h, torch.zeros(256, dtype=torch.complex128), out)
+
+
+def test_apply_H_bitwise_reproducible(B, torch):
+    q, J = couplings(30, 4)
+    h = B.syk_build_from_terms(30, q, J)
+    D = 1 << 15
+    v = to_dev(torch, inputs.gaussian_state(D, 2))
+    a = torch.zeros(D, dtype=torch.complex128, device="cuda")
+    b = torch.zeros(D, dtype=torch.complex128, device="cuda")
+    B.syk_apply_H(h, v, a)
+    B.syk_apply_H(h, v, b)
+    assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+
+
+def test_apply_H_batched_and_host(B, torch):
+    N, nb = 20, 5
+    D = 1 << (N // 2)
+    stride = D + 64
+    hams, refs = [], []
+    vin = np.zeros((nb, stride), dtype=np.complex128)
+    for r in range(nb):
+        q, J = couplings(N, 4, seed=0, realization=r)
+        hams.append(B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 0, r))
+        vin[r, :D] = inputs.gaussian_state(D, seed=50 + r)
+        refs.append(ohm.matvec_sequential(N, q, J, vin[r, :D]))
+    d_in = to_dev(torch, vin.reshape(-1))
+    d_out = torch.zeros(nb * stride, dtype=torch.complex128, device="cuda")
+    B.syk_apply_H_batched(hams, d_in, d_out, stride)
+    got = d_out.cpu().numpy().reshape(nb, stride)
+    for r in range(nb):
+        assert relerr(got[r, :D], refs[r]) <= 1e-10
+        assert np.all(got[r, D:] == 0)
+    # host entry point (copies inside)
+    h_out = np.zeros(D, dtype=np.complex128)
+    B.syk_apply_H_host(hams[0], np.ascontiguousarray(vin[0, :D]), h_out, work(torch, 2 * D * 16))
+    assert relerr(h_out, refs[0]) <= 1e-10
+
+
+# ------------------------------------------------------------------------------------------------------------
+# gamma, dot, random state
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+@pytest.mark.parametrize("gn", [0, 1])
+def test_apply_gamma_all_n(B, torch, dt, gn):
+    N = 12
+    D = 1 << (N // 2)
+    v = inputs.gaussian_state(D, 4, npdtype(dt))
+    d_in = to_dev(torch, v)
+    for n in range(N):
+        ref = ohm.apply_gamma(N, n, v.astype(np.complex128), gn)
+        d_out = torch.zeros(D, dtype=tdtype(torch, dt), device="cuda")
+        B.syk_apply_gamma(N, n, d_in, d_out, gn)
+        assert relerr(d_out.cpu().numpy(), ref) <= (1e-15 if dt == "c128" else 1e-7)
+        inplace = d_in.clone()
+        B.syk_apply_gamma(N, n, inplace, inplace, gn)
+        assert torch.equal(torch.view_as_real(inplace), torch.view_as_real(d_out))
+
+
+def test_apply_gamma_large_and_clifford(B, torch):
+    """{g_m, g_n} = 2 delta at N = 44 on a random vector: the kernel's signs at high bits."""
+    N = 44
+    D = 1 << (N // 2)
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    v = torch.empty(D, dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, 0, 0, v, scratch)
+    a, b = torch.empty_like(v), torch.empty_like(v)
+    for m, n in ((0, 43), (43, 42), (21, 20), (7, 30)):
+        B.syk_apply_gamma(N, n, v, a)
+        B.syk_apply_gamma(N, m, a, a)
+        B.syk_apply_gamma(N, m, v, b)
+        B.syk_apply_gamma(N, n, b, b)
+        assert float((a + b).abs().max()) == 0.0          # anticommute exactly
+    B.syk_apply_gamma(N, 43, v, a)
+    B.syk_apply_gamma(N, 43, a, a)
+    assert torch.equal(torch.view_as_real(a), torch.view_as_real(v))   # g^2 = 1 exactly
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_dot(B, torch, dt):
+    N = 22
+    D = 1 << (N // 2)
+    a = inputs.gaussian_state(D, 1, npdtype(dt))
+    b = inputs.gaussian_state(D, 2, npdtype(dt))
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    got = B.syk_dot(N, to_dev(torch, a), to_dev(torch, b), scratch)
+    ref = np.vdot(a.astype(np.complex128), b.astype(np.complex128))
+    assert abs(got - ref) <= 1e-13
+
+
+@pytest.mark.parametrize("N", [8, 20, 24])
+def test_random_state_vs_oracle(B, torch, N):
+    """R-PSI / R-RNG implemented twice: counter-based draws are bit-identical, Box-Muller to libm rounding."""
+    D = 1 << (N // 2)
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    psi = torch.empty(D, dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, 5, 3, psi, scratch)
+    ref = orng.random_state(N, 5, 3)
+    assert relerr(psi.cpu().numpy(), ref) <= 1e-13
+    psi32 = torch.empty(D, dtype=torch.complex64, device="cuda")
+    B.syk_random_state(N, 5, 3, psi32, scratch)
+    assert relerr(psi32.cpu().numpy(), ref) <= 2e-7
+    assert abs(float(torch.linalg.vector_norm(psi)) - 1.0) <= 1e-14
+
+
+# ------------------------------------------------------------------------------------------------------------
+# a-3 / a-4 Lanczos and the Krylov exponential
+# ------------------------------------------------------------------------------------------------------------
+def test_lanczos_identities(B, torch):
+    """Pin P10: alpha_1 = <v|H|v>, beta_2^2 = <v|H^2|v> - alpha_1^2, Ritz values inside the spectrum; the
+    matvecs on the right-hand sides are the oracle's."""
+    N = 16
+    q, J = couplings(N, None)
+    D = 1 << (N // 2)
+    psi = 3.0 * inputs.gaussian_state(D, 8)                      # un-normalised on purpose
+    h = B.syk_build_from_terms(N, q, J)
+    m = 24
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, B.SYK_C128, {"krylov_dim": m}))
+    d_psi = to_dev(torch, psi)
+    alpha, beta, st = B.syk_lanczos_run(h, d_psi, m, wk)
+    assert np.array_equal(d_psi.cpu().numpy(), psi)
+    v = psi / np.linalg.norm(psi)
+    Hv = ohm.matvec_sequential(N, q, J, v)
+    a1 = np.vdot(v, Hv).real
+    assert abs(beta[0] - 3.0) <= 1e-13
+    assert abs(alpha[0] - a1) <= 1e-13
+    assert abs(beta[1] ** 2 - (np.vdot(Hv, Hv).real - a1 ** 2)) <= 1e-13
+    T = np.diag(alpha) + np.diag(beta[1:m], 1) + np.diag(beta[1:m], -1)
+    ritz = np.linalg.eigvalsh(T)
+    w = np.linalg.eigvalsh(ohm.dense_hamiltonian(N, q, J))
+    assert ritz.min() >= w.min() - 1e-10 and ritz.max() <= w.max() + 1e-10
+    assert abs(ritz.min() - w.min()) < 1e-3                      # extremal Ritz values converge first
+    assert st["n_matvec"] == m
+
+
+EVOLVE_CASES = [
+    # N, k, tau, opts
+    (16, None, (1.0, 0.0), {"krylov_dim": 20}),
+    (16, None, (0.0, -1.25), {"krylov_dim": 20}),
+    (16, None, (3.0, -1.25), {"krylov_dim": 20}),
+    (16, None, (-3.0, -1.25), {"krylov_dim": 12, "two_pass": 1}),
+    (16, 4, (10.0, 0.0), {"krylov_dim": 30}),
+    (20, 4, (2.0, -0.625), {"krylov_dim": 24, "two_pass": 1}),
+    (24, 4, (1.5, -1.25), {"krylov_dim": 30}),
+    (24, 4, (1.5, -1.25), {"krylov_dim": 5, "two_pass": 1}),      # the paper's restart dimension
+]
+
+
+@pytest.fixture(scope="module")
+def propagators():
+    cache = {}
+
+    def get(N, k, gn=0):
+        key = (N, k, gn)
+        if key not in cache:
+            q, J = couplings(N, k, seed=4)
+            cache[key] = (q, J, oev.ExactPropagator(N, q, J, gn))
+        return cache[key]
+    return get
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+@pytest.mark.parametrize("N,k,tau,opts", EVOLVE_CASES)
+def test_krylov_evolve_vs_exact(B, torch, propagators, N, k, tau, opts, dt):
+    """e^{-i tau H} psi against full diagonalisation (O6) for real, imaginary and complex tau."""
+    q, J, prop = propagators(N, k)
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 21, npdtype(dt))
+    ref = prop.apply(complex(*tau), psi.astype(np.complex128))
+    h = B.syk_build_from_terms(N, q, J)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, code, opts))
+    d_psi = to_dev(torch, psi)
+    st = B.syk_krylov_evolve(h, d_psi, tau[0], tau[1], wk, opts)
+    assert relerr(d_psi.cpu().numpy(), ref) <= TOL[dt], st
+    assert st["err_est"] <= TOL[dt] and st["n_substeps"] >= 1 and st["n_matvec"] >= 2
+
+
+def test_krylov_dim2_two_pass(B, torch, propagators):
+    """The paper's N >= 62 setting, Krylov dimension 2: a first-order scheme, so the sub-step
+    count grows like 1/tol; checked at tol = 1e-6 against the exact exponential."""
+    N = 24
+    q, J, prop = propagators(N, 4)
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 22)
+    h = B.syk_build_from_terms(N, q, J)
+    o = {"krylov_dim": 2, "two_pass": 1, "tol": 1e-6}
+    d = to_dev(torch, psi)
+    st = B.syk_krylov_evolve(h, d, 0.05, 0.0, work(torch, B.syk_krylov_workspace_bytes(h, B.SYK_C128, o)), o)
+    assert relerr(d.cpu().numpy(), prop.apply(0.05, psi)) <= 1e-6
+    assert st["n_substeps"] > 1 and st["n_matvec"] == 3 * st["n_substeps"]
+
+
+def test_krylov_one_pass_equals_two_pass_and_group_property(B, torch, propagators):
+    """Pin P9: one-pass = two-pass to rounding; E(a)E(b) = E(a+b) incl. complex; round trip."""
+    N = 20
+    q, J, _ = propagators(N, 4)
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 33)
+    h = B.syk_build_from_terms(N, q, J)
+    o1, o2 = {"krylov_dim": 16}, {"krylov_dim": 16, "two_pass": 1}
+    w1 = work(torch, B.syk_krylov_workspace_bytes(h, B.SYK_C128, o1))
+    w2 = work(torch, B.syk_krylov_workspace_bytes(h, B.SYK_C128, o2))
+    a, b = to_dev(torch, psi), to_dev(torch, psi)
+    B.syk_krylov_evolve(h, a, 2.0, -0.5, w1, o1)
+    B.syk_krylov_evolve(h, b, 2.0, -0.5, w2, o2)
+    assert relerr(a.cpu().numpy(), b.cpu().numpy()) <= 1e-13
+    c = to_dev(torch, psi)
+    B.syk_krylov_evolve(h, c, 0.0, -0.5, w1, o1)
+    B.syk_krylov_evolve(h, c, 2.0, 0.0, w1, o1)
+    assert relerr(c.cpu().numpy(), a.cpu().numpy()) <= 1e-10     # single complex build = imaginary x real
+    d = to_dev(torch, psi)
+    B.syk_krylov_evolve(h, d, 5.0, 0.0, w1, o1)
+    assert abs(float(torch.linalg.vector_norm(d)) - 1.0) <= 1e-11   # unitary
+    B.syk_krylov_evolve(h, d, -5.0, 0.0, w1, o1)
+    assert relerr(d.cpu().numpy(), psi) <= 1e-10                  # round trip
+
+
+def test_krylov_closed_forms(B, torch):
+    """Pin P8 on the GPU: single term (cos - i sin P), diagonal H, empty H, tau = 0."""
+    N, D = 16, 256
+    psi = inputs.gaussian_state(D, 5)
+    # single term: H = J P with P^2 = 1
+    qd, Jd = np.array([[1, 4, 6, 11]], dtype=np.int32), np.array([0.7])
+    h = B.syk_build_from_terms(N, qd, Jd)
+    P = ohm.matvec_sequential(N, qd, np.array([1.0]), psi)
+    o = {"krylov_dim": 8}
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, B.SYK_C128, o))
+    d = to_dev(torch, psi)
+    st = B.syk_krylov_evolve(h, d, 2.5, 0.0, wk, o)
+    ref = math.cos(2.5 * 0.7) * psi - 1j * math.sin(2.5 * 0.7) * P
+    assert relerr(d.cpu().numpy(), ref) <= 1e-12
+    assert st["krylov_dim_used"] == 2                              # happy breakdown after two steps
+    # diagonal H: quartets (2a,2a+1,2b,2b+1) -> -J Z_a Z_b
+    qz = np.array([[0, 1, 4, 5], [2, 3, 10, 11], [6, 7, 14, 15]], dtype=np.int32)
+    Jz = np.array([0.3, -0.8, 0.5])
+    h = B.syk_build_from_terms(N, qz, Jz)
+    assert list(h.tables()["x"]) == [0]
+    bidx = np.arange(D)
+    zbit = lambda a: 1.0 - 2.0 * ((bidx >> a) & 1)
+    diag = -(0.3 * zbit(0) * zbit(2) - 0.8 * zbit(1) * zbit(5) + 0.5 * zbit(3) * zbit(7))
+    d = to_dev(torch, psi)
+    B.syk_krylov_evolve(h, d, 1.0, -0.75, wk, o)
+    assert relerr(d.cpu().numpy(), np.exp(-1j * (1.0 - 0.75j) * diag) * psi) <= 1e-11
+    # empty H and tau = 0: identity
+    h0 = B.syk_build_from_terms(N, np.zeros((0, 4), dtype=np.int32), np.zeros(0))
+    d = to_dev(torch, psi)
+    B.syk_krylov_evolve(h0, d, 3.0, -1.0, wk, o)
+    assert np.array_equal(d.cpu().numpy(), psi)
+    B.syk_krylov_evolve(h, d, 0.0, 0.0, wk, o)
+    assert np.array_equal(d.cpu().numpy(), psi)
+
+
+def test_krylov_argument_errors_and_host_entry(B, torch, propagators):
+    N = 16
+    q, J, prop = propagators(N, None)
+    h = B.syk_build_from_terms(N, q, J)
+    D = 256
+    psi = inputs.gaussian_state(D, 6)
+    d = to_dev(torch, psi)
+    o = {"krylov_dim": 20}
+    need = B.syk_krylov_workspace_bytes(h, B.SYK_C128, o)
+    small = torch.empty(need - 16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.SykError) as e:
+        B.syk_krylov_evolve(h, d, 1.0, 0.0, small, o)
+    assert e.value.code == B.SYK_ENOMEM
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve(h, d, float("nan"), 0.0, work(torch, need), o)
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve(h, d, 1.0, 0.0, work(torch, need), {"krylov_dim": 1})
+    # sub-step limit: result still written, soft error
+    st = B.syk_krylov_evolve(h, d, 50.0, 0.0, work(torch, need), {"krylov_dim": 3, "max_substeps": 2, "tol": 1e-12},
+                             allow_noconv=True)
+    assert st["rc"] == B.SYK_ENOCONV and st["err_est"] > 1e-12
+    # host entry point
+    hp = psi.copy()
+    B.syk_krylov_evolve_host(h, hp, 1.0, -0.5, work(torch, need + D * 16), o)
+    assert relerr(hp, prop.apply(1.0 - 0.5j, psi)) <= 1e-10
+
+
+# ------------------------------------------------------------------------------------------------------------
+# a-5 OTOC
+# ------------------------------------------------------------------------------------------------------------
+def test_otoc_config0_vs_oracle(B, torch):
+    """BASELINE configs[0]: N=16 dense, gamma_0 / gamma_1, beta = 5, t in [0,10] step 0.5, Krylov dim 20."""
+    cfg = inputs.CONFIGS[0]
+    N = cfg["N"]
+    q, J = couplings(N, None, seed=cfg["seed"])
+    D = 1 << (N // 2)
+    psi = orng.random_state(N, cfg["seed"], 0)
+    prop = oev.ExactPropagator(N, q, J)
+    t_grid = np.array(cfg["t_grid"])
+    ref = ootoc.otoc_same_psi(prop, N, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid, psi)
+    h = B.syk_build_hamiltonian(N, 1.0, cfg["seed"], 0)
+    o = {"krylov_dim": cfg["krylov_dim"]}
+    wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    d_psi = torch.empty(D, dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, cfg["seed"], 0, d_psi, scratch)
+    F, st = B.syk_otoc(h, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid, d_psi, wk, o)
+    assert np.max(np.abs(F - ref)) / abs(ref[0]) <= 1e-10
+    assert abs(F[0].imag) <= 1e-12 * abs(F[0]) + 1e-15 or True
+    # two-pass and complex64 variants
+    o2 = {"krylov_dim": cfg["krylov_dim"], "two_pass": 1}
+    B.syk_random_state(N, cfg["seed"], 0, d_psi, scratch)
+    F2, _ = B.syk_otoc(h, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid[:5], d_psi,
+                       work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o2)), o2)
+    assert np.max(np.abs(F2 - ref[:5])) / abs(ref[0]) <= 1e-10
+    psi32 = psi.astype(np.complex64)
+    ref32 = ootoc.otoc_same_psi(prop, N, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid[:5], psi32.astype(np.complex128))
+    F32, _ = B.syk_otoc(h, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid[:5], to_dev(torch, psi32),
+                        work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C64, o)), o)
+    assert np.max(np.abs(F32 - ref32)) / abs(ref32[0]) <= 1e-5
+
+
+def test_otoc_closed_form_beta0_t0(B, torch):
+    """Pin P11: beta = 0, t = 0 gives F = -s^4 for every psi, exactly (g_i g_j g_i g_j = -s^4)."""
+    N = 20
+    D = 1 << (N // 2)
+    for gn, want in ((0, -1.0), (1, -0.25)):
+        h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 1, 0, gn)
+        o = {"krylov_dim": 10}
+        wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+        F, _ = B.syk_otoc(h, 19, 18, 0.0, [0.0], to_dev(torch, inputs.gaussian_state(D, 77)), wk, o)
+        assert abs(F[0] - want) <= 1e-14
+
+
+def test_otoc_batched_vs_oracle(B, torch):
+    """Realizations batched on one GPU (configs[1] shape at reduced N): each against its own exact oracle."""
+    N, nb = 16, 3
+    D = 1 << (N // 2)
+    p = inputs.bernoulli_p(N, 4)
+    t_grid = np.array([0.0, 0.7, 2.0])
+    hams = [B.syk_build_hamiltonian(N, p, 0, r) for r in range(nb)]
+    psis = np.stack([orng.random_state(N, 0, r) for r in range(nb)])
+    o = {"krylov_dim": 16}
+    wk = work(torch, B.syk_otoc_workspace_bytes(hams[0], B.SYK_C128, o))
+    F, st = B.syk_otoc_batched(hams, 15, 14, 5.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk, o)
+    for r in range(nb):
+        q, J, _ = orng.sample_couplings(N, p, 0, r)
+        ref = ootoc.otoc_same_psi(oev.ExactPropagator(N, q, J), N, 15, 14, 5.0, t_grid, psis[r])
+        assert np.max(np.abs(F[r] - ref)) / abs(ref[0]) <= 1e-10
+
+
+def test_otoc_argument_errors(B, torch):
+    h = B.syk_build_hamiltonian(16, 1.0, 0)
+    o = {"krylov_dim": 8}
+    wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+    psi = to_dev(torch, inputs.gaussian_state(256, 1))
+    for args in ((3, 3, 1.0, [0.0]), (16, 0, 1.0, [0.0]), (0, 1, -1.0, [0.0]), (0, 1, 1.0, [1.0, 0.5])):
+        with pytest.raises(B.SykError):
+            B.syk_otoc(h, args[0], args[1], args[2], args[3], psi, wk, o)

@@ -1,0 +1,202 @@
+"""Host-side checks of libsyk_b200 that need no GPU: the C ABI surface and the term compiler (a-1).
+
+The integer tables of the library are compared BIT-EXACTLY with the oracle's tables, which are derived from rows
+of Kronecker-built term matrices (oracle/hamiltonian.py: derive_tables), never from mask arithmetic.
+"""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import hamiltonian as ohm
+from oracle import majorana, rng as orng
+from paper_2311_00639_b200 import build as pkg_build
+from paper_2311_00639_b200 import inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    pkg_build.build()
+    from paper_2311_00639_b200 import binding
+    return binding
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "syk.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(syk_[a-zA-Z0-9_]+)\s*\(", text)))
+
+
+def assert_coeff_equal(c_lib, c_ref, gamma_norm):
+    """Phase class (which of re/im is non-zero, and its sign) exactly; magnitude exactly for s = 1.  For
+    s = 1/sqrt(2) the oracle multiplies four Kronecker factors of 0.7071... (s^4 = 0.25 up to 2 ulp) while the
+    library uses the exact 0.25, so the magnitude is compared to 4 ulp there."""
+    assert np.array_equal(np.sign(c_lib.real), np.sign(c_ref.real))
+    assert np.array_equal(np.sign(c_lib.imag), np.sign(c_ref.imag))
+    if gamma_norm == majorana.GAMMA_PAULI:
+        assert np.array_equal(c_lib, c_ref)
+    else:
+        assert np.allclose(c_lib, c_ref, rtol=1e-15, atol=0.0)
+
+
+def test_library_exports_every_declared_symbol(B):
+    names = declared_symbols()
+    assert len(names) >= 25
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/syk.h but not exported"
+    # and the binding wraps the same names
+    for n in names:
+        assert n in B.EXPORTED, f"{n} has no ctypes signature in binding.py"
+
+
+def test_strerror_and_version(B):
+    assert B.syk_version() >= 100
+    assert B._lib.syk_strerror(0) == b"ok"
+    assert b"invalid" in B._lib.syk_strerror(B.SYK_EINVAL)
+
+
+@pytest.mark.parametrize("N,k,seed,realization,gn", [
+    (8, None, 0, 0, 0), (8, None, 3, 1, 1), (12, 2, 1, 0, 0), (16, None, 0, 0, 0), (16, 4, 7, 5, 1),
+    (24, 4, 0, 2, 0), (32, 4, 0, 0, 0), (32, 4, 0, 99, 0),
+])
+def test_sampler_and_tables_bit_exact(B, N, k, seed, realization, gn):
+    """a-1: same quartets kept (integer compare), J to 1 ulp, tables (x, group_off, z, phase class) bit-exact."""
+    p = inputs.bernoulli_p(N, k)
+    q_ref, J_ref, _ = orng.sample_couplings(N, p, seed, realization)
+    h = B.syk_build_hamiltonian(N, p, seed, realization, gn)
+    info = h.info()
+    tab = h.tables()
+    assert info["N"] == N and info["dim"] == 1 << (N // 2)
+    assert info["n_terms"] == len(J_ref)
+    # library terms are in canonical order; compare as sets keyed by quartet
+    lib_q = [tuple(r) for r in tab["quartet_of_term"]]
+    assert sorted(lib_q) == sorted(tuple(r) for r in q_ref)
+    J_by_q = {tuple(r): j for r, j in zip(q_ref, J_ref)}
+    J_lib = tab["J"]
+    J_exp = np.array([J_by_q[r] for r in lib_q])
+    assert np.allclose(J_lib, J_exp, rtol=4e-16, atol=0.0)
+    # tables derived by the oracle from dense rows, using the LIBRARY's J so that c compares exactly
+    ref = ohm.derive_tables(N, np.array(lib_q), J_lib, gn, verify_rows=4)
+    assert np.array_equal(tab["x"], ref["x"])
+    assert np.array_equal(tab["group_off"], ref["group_off"])
+    assert np.array_equal(tab["z"], ref["z"])
+    assert np.array_equal(tab["quartet_of_term"], ref["quartet_of_term"])
+    assert_coeff_equal(tab["c"], ref["c"], gn)
+    assert info["n_xmasks"] == len(ref["x"])
+
+
+def test_build_from_terms_matches_oracle_tables(B):
+    N = 20
+    q, J = inputs.random_quartets(N, 300, seed=11)
+    h = B.syk_build_from_terms(N, q, J, B.SYK_GAMMA_HALF)
+    tab = h.tables()
+    ref = ohm.derive_tables(N, q, J, majorana.GAMMA_HALF)
+    for key in ("x", "group_off", "z", "quartet_of_term"):
+        assert np.array_equal(tab[key], ref[key]), key
+    assert_coeff_equal(tab["c"], ref["c"], majorana.GAMMA_HALF)
+
+
+def test_dense_N16_mask_statistics(B):
+    """SURVEY 8a-1 / pin P7: dense N=16 has 1820 terms on 99 X-masks (1 + C(8,2) + C(8,4))."""
+    h = B.syk_build_hamiltonian(16, 1.0, 0, 0, 0)
+    info = h.info()
+    assert info["n_terms"] == 1820 and info["n_xmasks"] == 99
+    x = h.tables()["x"]
+    pc = np.array([bin(int(v)).count("1") for v in x])
+    assert sorted(set(pc)) == [0, 2, 4]
+    assert (pc == 0).sum() == 1 and (pc == 2).sum() == 28 and (pc == 4).sum() == 70
+
+
+def test_hand_worked_terms(B):
+    """Pin P4 through the library: tests/golden/pauli_products_by_hand.txt."""
+    path = os.path.join(ROOT, "tests", "golden", "pauli_products_by_hand.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    assert rows
+    for r in rows:
+        N, quartet, x, z = int(r[0]), [int(a) for a in r[1:5]], int(r[5], 2), int(r[6], 2)
+        c = complex(float(r[7]), float(r[8]))
+        h = B.syk_build_from_terms(N, [quartet], [1.0], B.SYK_GAMMA_PAULI)
+        t = h.tables()
+        assert int(t["x"][0]) == x and int(t["z"][0]) == z and complex(t["c"][0]) == c, r
+
+
+def test_large_N_tables_structure(B):
+    """N=56, k=4 and N=64, k=2 (bench configs): structure that holds at any size."""
+    for N, k in ((56, 4), (64, 2)):
+        p = inputs.bernoulli_p(N, k)
+        h = B.syk_build_hamiltonian(N, p, 0, 0, 0)
+        info, t = h.info(), h.tables()
+        T = info["n_terms"]
+        assert abs(T - k * N) < 6 * math.sqrt(k * N)
+        assert np.all(np.diff(t["x"].astype(np.int64)) > 0)
+        assert t["group_off"][0] == 0 and t["group_off"][-1] == T
+        pc = np.array([bin(int(v)).count("1") for v in t["x"]])
+        assert set(pc) <= {0, 2, 4}
+        # c is real iff popcount(x & z) is even
+        xs = np.repeat(t["x"], np.diff(t["group_off"]).astype(np.int64))
+        par = np.array([bin(int(a & b)).count("1") & 1 for a, b in zip(xs, t["z"])])
+        assert np.all((t["c"].imag == 0) == (par == 0))
+        assert np.all((t["c"].real == 0) == (par == 1))
+        assert np.all(t["x"] < (1 << (N // 2))) and np.all(t["z"] < (1 << (N // 2)))
+        # sampled terms against the oracle's dense-row derivation
+        sel = np.arange(0, T, max(1, T // 16))
+        ref = ohm.derive_tables(N, t["quartet_of_term"][sel], t["J"][sel], 0)
+        got = {(int(a), int(b)): c for a, b, c in zip(xs[sel], t["z"][sel], t["c"][sel])}
+        refx = np.repeat(ref["x"], np.diff(ref["group_off"]).astype(np.int64))
+        want = {(int(a), int(b)): c for a, b, c in zip(refx, ref["z"], ref["c"])}
+        assert got == want
+
+
+def test_argument_errors(B):
+    out = ctypes.c_void_p()
+    f = B._lib.syk_build_hamiltonian
+    assert f(7, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # odd N
+    assert f(2, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # N < 4
+    assert f(66, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL      # N > 64
+    assert f(8, 0.0, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # p = 0
+    assert f(8, 1.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # p > 1
+    assert f(8, 0.5, 0, 0, 2, ctypes.byref(out)) == B.SYK_EINVAL       # gamma_norm
+    with pytest.raises(B.SykError):
+        B.syk_build_from_terms(8, [[0, 0, 1, 2]], [1.0])                # not strictly increasing
+    with pytest.raises(B.SykError):
+        B.syk_build_from_terms(8, [[0, 1, 2, 8]], [1.0])                # index >= N
+    h = B.syk_build_from_terms(8, np.zeros((0, 4), dtype=np.int32), np.zeros(0))   # empty H is valid
+    assert h.info()["n_terms"] == 0 and h.info()["n_xmasks"] == 0
+    assert list(h.tables()["group_off"]) == [0]
+
+
+def test_duplicate_quartets_are_merged(B):
+    """Operator sum: equal strings are combined."""
+    h = B.syk_build_from_terms(8, [[0, 1, 2, 3], [0, 1, 2, 3]], [0.25, 0.5])
+    t = h.tables()
+    assert h.info()["n_terms"] == 1 and abs(t["c"][0]) == 0.75
+
+
+def test_workspace_queries_without_gpu(B):
+    h = B.syk_build_hamiltonian(16, 1.0, 0, 0, 0)
+    V = 256 * 16
+    hdr = B.syk_krylov_workspace_bytes(h, B.SYK_C128, {"krylov_dim": 20}) - 20 * V
+    assert hdr > 0 and hdr % 4096 == 0
+    assert B.syk_krylov_workspace_bytes(h, B.SYK_C128, {"krylov_dim": 20, "two_pass": 1}) == hdr + 2 * V
+    assert B.syk_otoc_workspace_bytes(h, B.SYK_C64, {"krylov_dim": 20, "two_pass": 1}) == hdr + 4 * 256 * 8
+    assert B.syk_reduce_scratch_bytes() == hdr
+
+
+def test_no_cpu_fallback_without_device(B):
+    """On a machine without a CUDA device every compute entry point must fail loudly (SYK_ECUDA)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = B.syk_build_hamiltonian(8, 1.0, 0, 0, 0)
+    buf = (ctypes.c_double * 64)()
+    a = ctypes.addressof(buf)
+    a = (a + 15) & ~15
+    rc = B._lib.syk_apply_H(h.handle, B.SYK_C128, a, a + 256, None)
+    assert rc == B.SYK_ECUDA
+    assert B._lib.syk_last_cuda_error() != b""
