@@ -286,6 +286,8 @@ def run_ours(args, wl, name):
     # ---- end to end through the HOST entry point: pinned host vector in, evolved vector out, every step ----
     e2e = None
     try:
+        if args.no_e2e:
+            raise RuntimeError("skipped (--no-e2e)")
         host = torch.empty(D, dtype=tdt).pin_memory()
         fill_host_state(host.numpy(), 7 + rank)
         def e2e_step():
@@ -370,6 +372,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="N56_k4_c128", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("note: fewer than 3 warm-up steps; not a valid bench number", file=sys.stderr)

@@ -286,7 +286,8 @@ def test_lanczos_identities(B, torch):
     ritz = np.linalg.eigvalsh(T)
     w = np.linalg.eigvalsh(ohm.dense_hamiltonian(N, q, J))
     assert ritz.min() >= w.min() - 1e-10 and ritz.max() <= w.max() + 1e-10
-    assert abs(ritz.min() - w.min()) < 1e-3                      # extremal Ritz values converge first
+    # extremal Ritz values converge first: after 24 of 256 steps the lowest one is within 1 % of the band width
+    assert abs(ritz.min() - w.min()) < 1e-2 * (w.max() - w.min())
     assert st["n_matvec"] == m
 
 
