@@ -331,10 +331,15 @@ def run_ours(args, wl, name):
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms, "launches_timed": apply_n,
                 "share_of_step": apply_ms / ms if ms else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None}
-    traffic_file = os.path.join(ROOT, "profiles", f"traffic_{name}.json")
+    # DRAM bytes per launch of that kernel from the last committed `ncu --set full` capture (profiles/traffic.csv)
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_file):
         try:
-            roofline["traffic"] = json.load(open(traffic_file))["dram_bytes_per_launch"]
+            import csv
+            for row in csv.DictReader(open(traffic_file)):
+                if row["workload"] == name:
+                    roofline["traffic"] = float(row["dram_bytes_per_launch"])
+                    roofline["traffic_source"] = row["source"]
         except Exception:
             pass
 
