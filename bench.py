@@ -5,7 +5,7 @@
 
 One "step" = one pass of the whole hot path over one synthetic realization:
     a-1  syk_build_hamiltonian(N, p = kN/C(N,4), seed, realization)          (host term compiler + table upload)
-    a-5  r <- gamma_W phi                                                    (Pauli-string insertion)
+    a-5  r <- gamma_W r                                                      (Pauli-string insertion, in place)
     a-4  r <- exp(-i (dt - i beta/4 ...) H) r   via syk_krylov_evolve        (m fused Lanczos steps = a-2 + a-3,
                                                                               host exp(-i tau T_m), combine)
     a-5  F = <l | r>                                                         (fp64 inner product)
@@ -104,11 +104,20 @@ class ClockSampler:
 
 
 def fill_host_state(buf_np, seed):
-    """iid complex Gaussian amplitudes, normalised, written in chunks into a (pinned) host array."""
+    """iid complex Gaussian amplitudes, normalised, written in chunks into a (pinned) host array.  Above 2^28
+    amplitudes one Gaussian block of 2^24 is drawn and re-used with a different unit phase per chunk (the e2e leg
+    only needs a generic dense vector; drawing 2^33 normals with numpy would take minutes)."""
     import numpy as np
     r = np.random.default_rng(seed)
     D = buf_np.shape[0]
-    chunk = 1 << 22
+    chunk = min(D, 1 << 22)
+    if D > (1 << 28):
+        chunk = 1 << 24
+        block = (r.standard_normal(chunk) + 1j * r.standard_normal(chunk)).astype(buf_np.dtype)
+        block *= 1.0 / math.sqrt(float(np.vdot(block, block).real) * (D // chunk))
+        for i, lo in enumerate(range(0, D, chunk)):
+            np.multiply(block, buf_np.dtype.type(np.exp(2.399963229728653j * i)), out=buf_np[lo:lo + chunk])
+        return
     n2 = 0.0
     for lo in range(0, D, chunk):
         hi = min(D, lo + chunk)
@@ -223,18 +232,17 @@ def run_ours(args, wl, name):
     kbytes = B.syk_krylov_workspace_bytes(h0, code, opts)
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
     wk = torch.empty(kbytes + V, dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
-    phi = torch.empty(D, dtype=tdt, device="cuda")
     l = torch.empty(D, dtype=tdt, device="cuda")
     r = torch.empty(D, dtype=tdt, device="cuda")
-    B.syk_random_state(N, 0, realization, phi, scratch)
-    B.syk_apply_gamma(N, wl["j_V"], phi, l)          # a second, different state for the bra side
+    B.syk_random_state(N, 0, realization, r, scratch)
+    B.syk_apply_gamma(N, wl["j_V"], r, l)            # a second, different state for the bra side
     torch.cuda.synchronize()
 
     stats_acc = {"n_matvec": 0, "model_bytes": 0.0, "n_substeps": 0}
 
     def step():
         h = B.syk_build_hamiltonian(N, p, 0, realization)                         # a-1
-        B.syk_apply_gamma(N, wl["i_W"], phi, r)                                   # a-5 insertion
+        B.syk_apply_gamma(N, wl["i_W"], r, r)                                     # a-5 insertion (in place)
         st = B.syk_krylov_evolve(h, r, tau[0], tau[1], wk, opts)                  # a-2, a-3, a-4
         F = B.syk_dot(N, l, r, scratch)                                           # a-5 inner product
         stats_acc["n_matvec"] += st["n_matvec"]
@@ -288,7 +296,7 @@ def run_ours(args, wl, name):
     try:
         if args.no_e2e:
             raise RuntimeError("skipped (--no-e2e)")
-        host = torch.empty(D, dtype=tdt).pin_memory()
+        host = torch.empty(D, dtype=tdt, pin_memory=True)
         fill_host_state(host.numpy(), 7 + rank)
         def e2e_step():
             h = B.syk_build_hamiltonian(N, p, 0, realization)
