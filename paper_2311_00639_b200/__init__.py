@@ -4,4 +4,4 @@
 names.  Importing `binding` fails loudly when `libsyk_b200.so` has not been built (`build.build()`): there is
 no CPU path.
 """
-__all__ = ["binding", "build", "inputs"]
+__all__ = ["binding", "build", "inputs", "replicas"]
