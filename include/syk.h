@@ -166,9 +166,11 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
 
 /* ------------------------------------------------------------------------------------------------------------
  * Introspection for tests and the benchmark. */
-/* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined tile gather. */
+/* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined 16 KiB-tile gather,
+ * 2 = TMA-pipelined register-tile gather (64 KiB tiles; sparse H with <= 1024 terms and D >= 2^22 / 2^23). */
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
-/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 as above. */
+/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 as above
+ * (a kind the handle cannot use falls back to the next lower one). */
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
 /* Number of kernels launched by this library on the calling thread since the last reset. */
 int64_t syk_launch_count(int reset);

@@ -369,6 +369,7 @@ int apply_h_kernel_kind(const syk_ham* h, int dtype) {
     const int avail = tma_stages(h, dtype) >= 3 ? 1 : 0;
     if (h->forced_kernel == 0) return 0;
     if (h->forced_kernel == 1) return avail;
+    if (regtile_tile_log2(h, dtype, h->forced_kernel == 2) > 0) return 2;
     return avail;
 }
 
@@ -377,7 +378,7 @@ int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, c
     SYK_TRY(ensure_device_tables(h));
     const int kind = apply_h_kernel_kind(h, dtype);
     profile_begin(stream);
-    const int rc = dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
+    const int rc = kind == 2 ? launch_apply_h_regtile(h, dtype, d_in, d_out, fa, stream) : dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
                                      : launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
     profile_end(stream);
     return rc;
@@ -419,7 +420,7 @@ int syk_apply_H_kernel_kind(const syk_ham* h, int dtype) {
 }
 
 int syk_set_apply_H_kernel(syk_ham* h, int kind) {
-    if (!h || kind < -1 || kind > 1) return SYK_EINVAL;
+    if (!h || kind < -1 || kind > 2) return SYK_EINVAL;
     h->forced_kernel = kind;
     return SYK_OK;
 }

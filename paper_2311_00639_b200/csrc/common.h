@@ -31,6 +31,26 @@ struct DeviceTables {
 
 }  // namespace syk
 
+namespace syk {
+// Term/load table of the register-tile kernel (apply_h_regtile.cu), passed BY VALUE as a __grid_constant__ kernel
+// parameter so that every per-term quantity is warp-uniform by construction (constant bank, uniform datapath).
+constexpr int kRtMaxTerms = 1024;
+constexpr int kRtMaxLoads = 1024;
+struct RtTable {
+    // term t: .x = tile-local X-mask | (coefficient is imaginary) << 31 ; .y = Z-mask ;
+    //         (.z, .w) = bits of the signed magnitude a (double), or .z = bits of (float) a for complex64
+    uint4 term[kRtMaxTerms];
+    uint32_t load_hi[kRtMaxLoads];         // x >> tile_log2 of each load; the hi == 0 load is LAST
+    uint16_t load_t0[kRtMaxLoads + 2];     // first term of each load
+    int n_loads;
+    int tile_log2;
+};
+struct RtCache {
+    RtTable tab;
+    int valid_for = -1;                    // dtype * 64 + tile_log2 the table was built for
+};
+}  // namespace syk
+
 struct syk_ham {
     int N = 0;
     int L = 0;
@@ -43,6 +63,7 @@ struct syk_ham {
     std::vector<double> J;                     // [n_terms]
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable syk::DeviceTables dev;             // created on first device use
+    mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
     int64_t n_terms() const { return (int64_t)z.size(); }
     int64_t n_groups() const { return (int64_t)x.size(); }
 };
@@ -108,6 +129,12 @@ struct FusedArgs {
     const void* prev = nullptr;     // u_{j-1}; may alias out; nullptr when j == 1
     int j = 0;
 };
+
+// register-tile kernel (apply_h_regtile.cu): 0 if the handle cannot use it, else the tile_log2 it would use
+int regtile_tile_log2(const syk_ham* h, int dtype, bool forced);
+int launch_apply_h_regtile(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                           cudaStream_t stream);
+void free_regtile_tables(const syk_ham* h);
 
 // apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

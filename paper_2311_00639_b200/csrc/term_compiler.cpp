@@ -162,6 +162,7 @@ int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets, const 
 void syk_free_hamiltonian(syk_ham* h) {
     if (!h) return;
     syk::free_device_tables(h);
+    syk::free_regtile_tables(h);
     delete h;
 }
 

@@ -45,22 +45,29 @@ def _fullsize_case(B, N, k, tdt, tol, n_samples):
     h = B.syk_build_hamiltonian(N, p, 0, 0)
     assert h.info()["n_terms"] == len(J)
     code = B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64
-    assert B.syk_apply_H_kernel_kind(h, code) == 1                        # the kernel bench.py times
+    assert B.syk_apply_H_kernel_kind(h, code) == 2                        # the kernel bench.py times
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
     d_in = torch.empty(D, dtype=tdt, device="cuda")
     d_out = torch.empty(D, dtype=tdt, device="cuda")
     B.syk_random_state(N, 0, 0, d_in, scratch)
-    B.syk_apply_H(h, d_in, d_out)
-    torch.cuda.synchronize()
-    # (i) sampled outputs, including the first/last amplitude and the first/last tile of the vector
+    # (i) sampled outputs, including the first/last amplitude and the first/last tiles of the vector (16 KiB and
+    #     64 KiB tiles), for both TMA kernels; the default (register-tile) kernel runs last and feeds (ii)
     idx = inputs.sample_indices(D, n_samples, seed=17)
-    edge = np.array([1, 1023, 1024, D // 2 - 1, D // 2, D - 1024, D - 2], dtype=np.uint64)
+    edge = np.array([1, 1023, 1024, 4095, 4096, 8191, 8192, D // 2 - 1, D // 2, D - 8192, D - 4097, D - 1024, D - 2],
+                    dtype=np.uint64)
     idx = np.unique(np.concatenate([idx, edge]))
     ref = _oracle_samples(N, q, J, idx, d_in)
-    got = d_out[torch.from_numpy(idx.astype(np.int64)).cuda()].cpu().numpy().astype(np.complex128)
     scale = np.sqrt(np.mean(np.abs(ref) ** 2))
-    assert np.max(np.abs(got - ref)) <= tol * scale * 10, float(np.max(np.abs(got - ref)) / scale)
-    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= tol
+    for kind in (1, 2):
+        B.syk_set_apply_H_kernel(h, kind)
+        assert B.syk_apply_H_kernel_kind(h, code) == kind
+        d_out.zero_()
+        B.syk_apply_H(h, d_in, d_out)
+        torch.cuda.synchronize()
+        got = d_out[torch.from_numpy(idx.astype(np.int64)).cuda()].cpu().numpy().astype(np.complex128)
+        assert np.max(np.abs(got - ref)) <= tol * scale * 10, (kind, float(np.max(np.abs(got - ref)) / scale))
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= tol, kind
+    B.syk_set_apply_H_kernel(h, -1)
     # (ii) sum rule: |H psi|^2 = <psi|H^2|psi> ~ Tr H^2 / D = sum J^2 (s = 1), fluctuation O(D^-1/2)
     n2 = B.syk_dot(N, d_out, d_out, scratch).real
     assert abs(n2 / float(np.sum(J ** 2)) - 1.0) <= 5e-3

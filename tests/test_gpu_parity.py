@@ -67,14 +67,15 @@ def couplings(N, k, seed=0, realization=0):
 APPLY_CASES = [
     # N, k (None = dense), gamma_norm
     (4, None, 0), (6, None, 1), (8, None, 0), (12, None, 0), (16, None, 0), (16, 4, 1),
-    (20, 4, 0), (22, 8, 0), (24, 4, 0), (26, 2, 0),
+    (20, 4, 0), (22, 8, 0), (24, 4, 0), (26, 2, 0), (28, 4, 1), (30, 8, 0), (32, 4, 0),
 ]
 
 
 @pytest.mark.parametrize("dt", ["c128", "c64"])
 @pytest.mark.parametrize("N,k,gn", APPLY_CASES)
 def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
-    """out = H.in against the oracle's sequential-gamma product (O5), both kernels."""
+    """out = H.in against the oracle's sequential-gamma product (O5), every kernel the handle can use
+    (0 generic, 1 16 KiB-tile TMA, 2 register-tile TMA)."""
     q, J = couplings(N, k, seed=1)
     D = 1 << (N // 2)
     v = inputs.gaussian_state(D, seed=100 + N, dtype=npdtype(dt))
@@ -82,8 +83,11 @@ def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
     h = B.syk_build_from_terms(N, q, J, gn)
     d_in = to_dev(torch, v)
     kinds = {0}
-    B.syk_set_apply_H_kernel(h, 1)
-    kinds.add(B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)))
+    for want in (1, 2):
+        B.syk_set_apply_H_kernel(h, want)
+        kinds.add(B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)))
+    if N >= 28:
+        assert kinds == {0, 1, 2}
     for kind in sorted(kinds):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
@@ -113,11 +117,12 @@ def test_apply_H_structured_masks(B, torch, qubits, dt):
     ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
     h = B.syk_build_from_terms(N, q, J)
     d_in = to_dev(torch, v)
-    for kind in (0, 1):
+    for kind in (0, 1, 2):
         B.syk_set_apply_H_kernel(h, kind)
+        assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
         d_out = torch.zeros(D, dtype=tdtype(torch, dt), device="cuda")
         B.syk_apply_H(h, d_in, d_out)
-        assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt]
+        assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt], kind
 
 
 def test_apply_H_literal_algorithm1(B, torch):
