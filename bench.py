@@ -333,8 +333,12 @@ def run_ours(args, wl, name):
     per_launch_bytes = (n_x + 2) * V
     avg_ms = apply_ms / apply_n if apply_n else float("nan")
     achieved = per_launch_bytes / (avg_ms * 1e-3) / 1e9 if apply_n else None
-    kernel_names = {0: "apply_h_generic_kernel", 1: "apply_h_tma_kernel", 2: "apply_h_regtile_kernel"}
-    roofline = {"bound": "hbm", "kernel": kernel_names[B.syk_apply_H_kernel_kind(h0, code)], "achieved": achieved, "peak": peak, "unit": "GB/s",
+    kernel_names = {0: "apply_h_generic_kernel", 1: "apply_h_tma_kernel", 2: "apply_h_regtile_kernel",
+                    3: "apply_h_scatter_kernel"}
+    kind = B.syk_apply_H_kernel_kind(h0, code)
+    layout = B.syk_apply_H_layout(h0, code) if kind == 3 else None
+    roofline = {"bound": "hbm", "kernel": kernel_names[kind], "layout": layout, "achieved": achieved, "peak": peak,
+                "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms, "launches_timed": apply_n,
                 "share_of_step": apply_ms / ms if ms else None,

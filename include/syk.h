@@ -167,11 +167,25 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
 /* ------------------------------------------------------------------------------------------------------------
  * Introspection for tests and the benchmark. */
 /* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined 16 KiB-tile gather,
- * 2 = TMA-pipelined register-tile gather (64 KiB tiles; sparse H with <= 1024 terms and D >= 2^22 / 2^23). */
+ * 2 = TMA-pipelined register-tile gather (64 KiB tiles; sparse H with <= 1024 terms and D >= 2^22 / 2^23),
+ * 3 = TMA-pipelined scatter-tile gather (128 KiB tiles on index bits chosen per Hamiltonian; sparse H with
+ *     1..1024 terms and D >= 2^23 / 2^24). */
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
-/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 as above
+/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 as above
  * (a kind the handle cannot use falls back to the next lower one). */
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
+/* Tile layout the scatter-tile kernel (kind 3) chose for this Hamiltonian: n_loads = source tiles fetched per
+ * output tile (L2 -> SM transfers of the whole vector per product), n_passes = distinct X-masks outside tile and
+ * L2-window bits (DRAM reads of the whole vector per product, if L2 reuse were perfect), tile_mask / window_mask =
+ * the index bits of a tile / of tile + window.  Any output pointer may be NULL.  SYK_EINVAL if kind 3 cannot be used. */
+int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
+                       uint32_t* window_mask);
+/* Pacing of the register-tile / scatter-tile kernels' persistent CTAs (process-wide; a tuning knob, results do not depend on it):
+ * producers count their tile loads in epochs of `epoch_len` loads and may start an epoch only when every CTA has
+ * issued the epoch `lag`+1 before it, which keeps the CTAs at the same place of the sorted load list so that source
+ * tiles shared between neighbouring output tiles are still in L2.  epoch_len = 0 lets the CTAs run free.
+ * Default (8, 1).  Used only for vectors larger than L2.  0 <= lag <= 30. */
+int syk_set_lockstep(int epoch_len, int lag);
 /* Number of kernels launched by this library on the calling thread since the last reset. */
 int64_t syk_launch_count(int reset);
 /* Per-kernel device timing for the benchmark's roofline line.  While enabled, every apply_H launch made by the

@@ -74,6 +74,8 @@ _SIGNATURES = {
                               _P(syk_stats), _vp]),
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
     "syk_set_apply_H_kernel": (_i, [_vp, _i]),
+    "syk_set_lockstep": (_i, [_i, _i]),
+    "syk_apply_H_layout": (_i, [_vp, _i, _P(_i), _P(_i), _P(_u32), _P(_u32)]),
     "syk_launch_count": (_i64, [_i]),
     "syk_profile_enable": (_i, [_i]),
     "syk_profile_read": (_i, [_P(_d), _P(_i64), _i]),
@@ -339,6 +341,17 @@ def syk_apply_H_kernel_kind(h, dtype):
 
 def syk_set_apply_H_kernel(h, kind):
     _check(_lib.syk_set_apply_H_kernel(_h(h), int(kind)), "syk_set_apply_H_kernel")
+
+
+def syk_apply_H_layout(h, dtype):
+    nl, npass, tm, wm = _i(), _i(), _u32(), _u32()
+    _check(_lib.syk_apply_H_layout(_h(h), int(dtype), ctypes.byref(nl), ctypes.byref(npass), ctypes.byref(tm),
+                                   ctypes.byref(wm)), "syk_apply_H_layout")
+    return {"n_loads": nl.value, "n_passes": npass.value, "tile_mask": tm.value, "window_mask": wm.value}
+
+
+def syk_set_lockstep(epoch_len, lag):
+    _check(_lib.syk_set_lockstep(int(epoch_len), int(lag)), "syk_set_lockstep")
 
 
 def syk_launch_count(reset=False):

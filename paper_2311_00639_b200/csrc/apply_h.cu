@@ -369,7 +369,8 @@ int apply_h_kernel_kind(const syk_ham* h, int dtype) {
     const int avail = tma_stages(h, dtype) >= 3 ? 1 : 0;
     if (h->forced_kernel == 0) return 0;
     if (h->forced_kernel == 1) return avail;
-    if (regtile_tile_log2(h, dtype, h->forced_kernel == 2) > 0) return 2;
+    if (h->forced_kernel != 2 && scatter_tile_log2(h, dtype, h->forced_kernel == 3) > 0) return 3;
+    if (regtile_tile_log2(h, dtype, h->forced_kernel >= 2) > 0) return 2;
     return avail;
 }
 
@@ -378,8 +379,10 @@ int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, c
     SYK_TRY(ensure_device_tables(h));
     const int kind = apply_h_kernel_kind(h, dtype);
     profile_begin(stream);
-    const int rc = kind == 2 ? launch_apply_h_regtile(h, dtype, d_in, d_out, fa, stream) : dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
-                                     : launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
+    const int rc = kind == 3   ? launch_apply_h_scatter(h, dtype, d_in, d_out, fa, stream)
+                   : kind == 2 ? launch_apply_h_regtile(h, dtype, d_in, d_out, fa, stream)
+                   : dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
+                                       : launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
     profile_end(stream);
     return rc;
 }
@@ -419,8 +422,20 @@ int syk_apply_H_kernel_kind(const syk_ham* h, int dtype) {
     return syk::apply_h_kernel_kind(h, dtype);
 }
 
+int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
+                       uint32_t* window_mask) {
+    if (!h || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    return syk::scatter_layout_info(h, dtype, n_loads, n_passes, tile_mask, window_mask);
+}
+
+int syk_set_lockstep(int epoch_len, int lag) {
+    if (epoch_len < 0 || lag < 0 || lag > syk::kSyncRing - 2) return SYK_EINVAL;
+    syk::set_lockstep(epoch_len, lag);
+    return SYK_OK;
+}
+
 int syk_set_apply_H_kernel(syk_ham* h, int kind) {
-    if (!h || kind < -1 || kind > 2) return SYK_EINVAL;
+    if (!h || kind < -1 || kind > 3) return SYK_EINVAL;
     h->forced_kernel = kind;
     return SYK_OK;
 }

@@ -23,6 +23,7 @@
 //
 // Fused Lanczos epilogue (a-3 part 1) as in apply_h.cu: out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, per-CTA fp64
 // partial sums of Re<in|out>.  in[b] for that sum is read from the LAST load's slot (hi == 0: the tile itself).
+#include <atomic>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -51,6 +52,10 @@ struct RtParams {
     int j;
     int L;
     int nslot;
+    // lock-step of the persistent CTAs (see lockstep_gate): nullptr = free running
+    uint32_t* sync;
+    int epoch_len;   // loads per epoch
+    int lag;         // a CTA may start epoch e once every CTA has issued epoch e-1-lag
 };
 
 __host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
@@ -135,8 +140,17 @@ apply_h_regtile_kernel(const __grid_constant__ RtTable tab, const RtParams<T> p)
             int slot = 0;
             uint32_t phase = 0;
             const uint32_t stage0 = smem_u32(stages);
+            uint32_t g = 0, until_epoch = 0;   // loads issued; loads left in the current epoch
             for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 for (int l = 0; l < n_loads; ++l) {
+                    if (p.sync) {
+                        if (until_epoch == 0) {
+                            lockstep_gate(p.sync, g / (uint32_t)p.epoch_len, (uint32_t)p.lag);
+                            until_epoch = (uint32_t)p.epoch_len;
+                        }
+                        --until_epoch;
+                        ++g;
+                    }
                     mbar_wait(bar_empty + 8 * slot, phase ^ 1u);
                     mbar_arrive_expect_tx(bar_full + 8 * slot, TILE_BYTES);
                     const unsigned char* src =
@@ -150,6 +164,13 @@ apply_h_regtile_kernel(const __grid_constant__ RtTable tab, const RtParams<T> p)
                         phase ^= 1u;
                     }
                 }
+            }
+            if (p.sync) {
+                // report every remaining epoch of the longest-running CTA, so that nobody waits for this one
+                const uint32_t E = (uint32_t)p.epoch_len;
+                const uint32_t max_loads = ((n_tiles + gridDim.x - 1) / gridDim.x) * (uint32_t)n_loads;
+                const uint32_t n_epochs = (max_loads + E - 1) / E;
+                for (uint32_t f = g == 0 ? 0 : (g - 1) / E; f < n_epochs; ++f) atomicAdd(p.sync + (f % kSyncRing), 1u);
             }
         }
         __syncwarp();
@@ -300,6 +321,12 @@ const RtTable* get_rt_table(const syk_ham* h, int dtype) {
     return &h->rt[k]->tab;
 }
 
+// epoch length / lag of the lock-step (syk_set_lockstep; epoch_len 0 = free running).  Defaults from the sweeps
+// in profiles/r1e_lockstep_sweep.md (this kernel: N = 64 complex64 505 -> 345..361 ms, N = 56 complex128 unchanged).
+struct LockstepConfig { int epoch_len; int lag; };
+std::atomic<int> g_ls_epoch{8}, g_ls_lag{1};
+LockstepConfig lockstep_config() { return LockstepConfig{g_ls_epoch.load(), g_ls_lag.load()}; }
+
 template <typename T, int R>
 int launch_rt(const syk_ham* h, const RtTable& tab, const void* d_in, void* d_out, const FusedArgs& fa,
               cudaStream_t stream) {
@@ -318,6 +345,15 @@ int launch_rt(const syk_ham* h, const RtTable& tab, const void* d_in, void* d_ou
     if (sms <= 0) return SYK_ECUDA;
     const uint64_t n_tiles = 1ull << (h->L - tab.tile_log2);
     const int grid = (int)(n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms);
+    // lock-step only where it pays: the vector does not fit in L2 and there are several rounds of tiles
+    const LockstepConfig ls = lockstep_config();
+    p.sync = nullptr;
+    p.epoch_len = ls.epoch_len;
+    p.lag = ls.lag;
+    if (ls.epoch_len > 0 && n_tiles * kRtTileBytes > ((uint64_t)64 << 20) && n_tiles >= 4 * (uint64_t)grid) {
+        p.sync = h->dev.sync;
+        SYK_CUDA(cudaMemsetAsync(p.sync, 0, kSyncRing * sizeof(uint32_t), stream));
+    }
     if (fa.sc) {
         SYK_CUDA(cudaFuncSetAttribute(apply_h_regtile_kernel<T, R, true>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -349,6 +385,16 @@ int launch_apply_h_regtile(const syk_ham* h, int dtype, const void* d_in, void* 
     if (!tab) return SYK_EINVAL;
     if (dtype == SYK_C128) return launch_rt<double, kRt_R[1]>(h, *tab, d_in, d_out, fa, stream);
     return launch_rt<float, kRt_R[0]>(h, *tab, d_in, d_out, fa, stream);
+}
+
+void set_lockstep(int epoch_len, int lag) {
+    g_ls_epoch.store(epoch_len);
+    g_ls_lag.store(lag);
+}
+
+void get_lockstep(int* epoch_len, int* lag) {
+    *epoch_len = g_ls_epoch.load();
+    *lag = g_ls_lag.load();
 }
 
 void free_regtile_tables(const syk_ham* h) {

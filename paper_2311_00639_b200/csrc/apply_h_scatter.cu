@@ -1,0 +1,530 @@
+// a-2  apply_H, scatter-tile kernel: the gather form of Algorithm 1 with 128 KiB output tiles
+// whose index bits are CHOSEN per Hamiltonian.
+//
+//     out[b] = sum_t c_t (-1)^popcount(b & z_t) in[b ^ x_t]
+//
+// What bounds this product on B200 is not arithmetic but how often the vector is moved: once from DRAM per
+// distinct value of (x restricted to the bits above the L2 window), once from L2 into an SM per distinct value of
+// (x restricted to the bits outside a tile).  Both counts depend on WHICH qubits are the tile / window bits, and
+// the X-masks of a sparse SYK Hamiltonian are random 2- and 4-subsets of the qubits, so the host picks the bits
+// (choose_layout: hill climbing on  #loads + 2 #passes):
+//   * thread bits  : index bits 0..7 (256 consecutive amplitudes, one per consumer thread);
+//   * r bits       : NR further bit positions P[0..NR-1]; a thread keeps the R = 2^NR amplitudes
+//                    base | deposit(r, P) | tid  in registers (128 KiB of accumulators per SM).  P[0..2] = 8, 9, 10
+//                    (a "run" of 8 slices = 2048 consecutive amplitudes = one cp.async.bulk: the TMA unit costs
+//                    ~85 clk per copy, measured, so 2-4 KiB copies cannot feed an SM); the other NR-3 r bits sit
+//                    ANYWHERE in the index;
+//   * outer bits   : the rest, in an order O[0..]: the tile counter tau is deposited into them, O[0] fastest, so
+//                    the 148 tiles in flight differ in O[0..7] only -- those are the L2-window bits.
+// No data is permuted: a source tile is fetched run by run (cp.async.bulk, TMA unit, SASS UBLKCP; completion on
+// mbarriers) into a ring of shared-memory chunks.  Persistent CTAs, one per SM: two consumer warpgroups (232
+// registers per thread after setmaxnreg) and one producer warpgroup (40 registers, one working lane).
+//
+// Chunked ring: a 128 KiB tile does not fit twice in shared memory, so the ring holds 3 chunks of 64 KiB (half a
+// tile).  The source slice of output slice r under mask x is r ^ xr (xr = the r bits of x), so source chunk c feeds
+// output chunk oc = c ^ (xr >> LRC): the consumers take the chunks of a load in arrival order and branch
+// (uniformly) to the code that owns the accumulator registers of chunk oc.
+//
+// Per (amplitude, term): one LDS, two FMAs (the coefficient is exactly real or exactly imaginary: c = J s^4 times
+// 1, -1, i, -i); the sign is popcount((base | tid) & z) once per (term, chunk) and thread plus a Gray-code walk
+// over the slices of a chunk (one XOR each).  Per-term data comes from the __grid_constant__ table (constant
+// bank).  No atomics on data, one write per output: bitwise reproducible.
+//
+// Fused Lanczos epilogue (a-3 part 1) as in apply_h.cu: out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, per-CTA fp64
+// partial sums of Re<in|out> (in[b] re-read from global: an L2 hit, the tile has just been staged).
+//
+// Measured (profiles/r1e_*.md): both headline workloads sit at the L2 -> SM throughput ceiling (~6000-6600 B/clk
+// chip-wide): #loads x V / time = 12.1 TB/s (N = 56 complex128) and 10.1 TB/s (N = 64 complex64).
+#include <algorithm>
+#include <atomic>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "device_utils.cuh"
+
+namespace syk {
+
+namespace {
+
+constexpr int kConsumerWarps = 8;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+// Two consumer warpgroups + one producer warpgroup (only its first warp works).  The kernel is launched with
+// 65536 / 384 = 168 registers per thread; the consumers then take 232 and the producer warpgroup drops to 40
+// (setmaxnreg, per warpgroup): 2 x 232 + 40 <= 512 registers per lane on every SM sub-partition.
+constexpr int kThreads = kConsumerThreads + 128;
+constexpr int kConsumerRegs = 232, kProducerRegs = 40;
+constexpr int kThreadBits = 8;
+constexpr int kRun = 8;                            // consecutive slices per bulk copy (r bits 0..2 = index bits 8..10)
+constexpr int kMaxRing = 16;
+constexpr int kSmemLimit = 232448;                 // 227 KiB opt-in maximum per CTA on sm_100
+constexpr int kMiscBytes = 2 * kMaxRing * 8 + 40 * 8 + 128;
+constexpr int kWindowBits = 7;                     // ~log2(148 tiles in flight)
+constexpr int kFixedR = 3;                         // r bits 0..2 sit at index bits 8..10: a chunk is one contiguous run
+
+template <typename T>
+struct StParams {
+    using C = typename Cx<T>::type;
+    const C* in;
+    C* out;
+    const C* prev;
+    LanczosScalars* sc;
+    int j;
+    int nring;
+    uint32_t* sync;   // lock-step counters (device_utils.cuh lockstep_gate); nullptr = free running
+    int epoch_len;
+    int lag;
+};
+
+__device__ __forceinline__ void st_fused_scalars(LanczosScalars* sc, int j, double* red, double& s_in, double& s_prev) {
+    double n2 = reduce_partials(sc->partial_nrm, sc->n_partial_nrm, red);
+    double nj = sqrt(n2);
+    if (blockIdx.x == 0 && threadIdx.x == 0) sc->nrm[j] = nj;
+    s_in = nj > 0.0 ? 1.0 / nj : 0.0;
+    s_prev = 0.0;
+    if (j > 1) {
+        double np = sc->nrm[j - 1];
+        s_prev = np > 0.0 ? nj / np : 0.0;
+    }
+}
+
+__device__ __forceinline__ double st_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float st_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+
+// One term applied to the RC accumulators of output chunk OC.  `pb` = the thread's position inside the staged
+// source chunk; `w` = sign-carrying word of the coefficient times the sign of (thread, tile, chunk); the slices of
+// the chunk are walked in Gray-code order so that consecutive signs differ by one uniform XOR.
+template <typename T, int R, int RC, int OC, bool IMAG>
+__device__ __forceinline__ void accumulate_chunk(const unsigned char* __restrict__ pb, uint32_t xr_lo, uint32_t zr_lo,
+                                                 uint32_t a_lo, uint32_t w, T (&ar)[R], T (&ai)[R]) {
+    using C = typename Cx<T>::type;
+#pragma unroll
+    for (int i = 0; i < RC; ++i) {
+        const int rl = i ^ (i >> 1);
+        if (i > 0) w ^= (zr_lo * (0x80000000u / (uint32_t)(i & -i))) & 0x80000000u;   // z bit ctz(i) -> bit 31; a shift after unrolling
+        T a;
+        if constexpr (sizeof(T) == 8) a = __hiloint2double((int)w, (int)a_lo);
+        else a = __uint_as_float(w);
+        const C v = *reinterpret_cast<const C*>(pb + ((((uint32_t)rl ^ xr_lo) << kThreadBits) * (uint32_t)sizeof(C)));
+        constexpr int r0 = OC * RC;
+        if constexpr (IMAG) {   // (i a)(vx + i vy) = -a vy + i a vx
+            ar[r0 + rl] = st_fma(-a, v.y, ar[r0 + rl]);
+            ai[r0 + rl] = st_fma(a, v.x, ai[r0 + rl]);
+        } else {
+            ar[r0 + rl] = st_fma(a, v.x, ar[r0 + rl]);
+            ai[r0 + rl] = st_fma(a, v.y, ai[r0 + rl]);
+        }
+    }
+}
+
+template <typename T, int R, int RC, int OC, bool IMAG>
+__device__ __forceinline__ void dispatch_chunk(uint32_t oc, const unsigned char* pb, uint32_t xr_lo, uint32_t zr_lo,
+                                               uint32_t a_lo, uint32_t w, T (&ar)[R], T (&ai)[R]) {
+    if constexpr (OC + 1 == R / RC) {
+        accumulate_chunk<T, R, RC, OC, IMAG>(pb, xr_lo, zr_lo, a_lo, w, ar, ai);
+    } else {
+        if (oc == (uint32_t)OC) accumulate_chunk<T, R, RC, OC, IMAG>(pb, xr_lo, zr_lo, a_lo, w, ar, ai);
+        else dispatch_chunk<T, R, RC, OC + 1, IMAG>(oc, pb, xr_lo, zr_lo, a_lo, w, ar, ai);
+    }
+}
+
+template <typename T, int NR, int LRC, bool FUSED>
+__global__ void __launch_bounds__(kThreads, 1)
+apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p) {
+    using C = typename Cx<T>::type;
+    constexpr int R = 1 << NR;
+    constexpr int RC = 1 << LRC;                                  // slices per ring chunk
+    constexpr int NC = R / RC;                                    // chunks per tile
+    constexpr uint32_t SLICE_BYTES = kConsumerThreads * sizeof(C);
+    constexpr uint32_t RUN_BYTES = kRun * SLICE_BYTES;
+    constexpr uint32_t CHUNK_BYTES = RC * SLICE_BYTES;
+    static_assert(R % RC == 0 && RC % kRun == 0 && LRC >= kFixedR, "tile = whole chunks = whole runs");
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* q = smem + (size_t)p.nring * CHUNK_BYTES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(q);
+    q += 2 * kMaxRing * 8;
+    double* red = reinterpret_cast<double*>(q);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kMaxRing);
+    if (tid == 0) {
+        for (int s = 0; s < p.nring; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, kConsumerWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    double s_in = 1.0, s_prev = 0.0;
+    if (FUSED) st_fused_scalars(p.sc, p.j, red, s_in, s_prev);
+
+    const uint32_t n_tiles = 1u << tab.n_outer;
+    const int nring = p.nring, n_loads = tab.n_loads, n_outer = tab.n_outer;
+    double dot = 0.0;
+
+    if (warp >= kConsumerWarps) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kProducerRegs));
+        if (warp != kConsumerWarps || lane != 0) return;
+        // ---------------- producer: one lane streams the chunks (8 consecutive slices = one bulk copy) ----------
+        int pos = 0;
+        uint32_t phase = 0;
+        const uint32_t stage0 = smem_u32(smem);
+        uint32_t g = 0, until_epoch = 0;   // loads issued; loads left in the current epoch
+        for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            uint32_t base = 0;
+            for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
+            for (int l = 0; l < n_loads; ++l) {
+                if (p.sync) {
+                    if (until_epoch == 0) {
+                        lockstep_gate(p.sync, g / (uint32_t)p.epoch_len, (uint32_t)p.lag);
+                        until_epoch = (uint32_t)p.epoch_len;
+                    }
+                    --until_epoch;
+                    ++g;
+                }
+                const uint32_t src = base ^ tab.load_xo[l];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    mbar_wait(bar_empty + 8 * pos, phase ^ 1u);
+                    mbar_arrive_expect_tx(bar_full + 8 * pos, CHUNK_BYTES);
+#pragma unroll
+                    for (int u = 0; u < RC / kRun; ++u)
+                        bulk_load(stage0 + (uint32_t)pos * CHUNK_BYTES + (uint32_t)u * RUN_BYTES,
+                                  p.in + (uint64_t)(src | tab.dep_r[c * RC + u * kRun]), RUN_BYTES, bar_full + 8 * pos);
+                    if (++pos == nring) {
+                        pos = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+        }
+        if (p.sync) {
+            // report every remaining epoch of the longest-running CTA, so that nobody waits for this one
+            const uint32_t E = (uint32_t)p.epoch_len;
+            const uint32_t max_loads = ((n_tiles + gridDim.x - 1) / gridDim.x) * (uint32_t)n_loads;
+            const uint32_t n_epochs = (max_loads + E - 1) / E;
+            for (uint32_t f = g == 0 ? 0 : (g - 1) / E; f < n_epochs; ++f) atomicAdd(p.sync + (f % kSyncRing), 1u);
+        }
+    } else {
+        // ---------------- consumers ----------------
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kConsumerRegs));
+        int pos = 0;
+        uint32_t phase = 0;
+        for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            uint32_t base = 0;
+            for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
+            const uint32_t bt = base | (uint32_t)tid;
+            T ar[R], ai[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                ar[r] = 0;
+                ai[r] = 0;
+            }
+            for (int l = 0; l < n_loads; ++l) {
+                const int t0 = tab.load_t0[l], t1 = tab.load_t0[l + 1];
+                for (uint32_t c = 0; c < (uint32_t)NC; ++c) {
+                    mbar_wait(bar_full + 8 * pos, phase);
+                    const unsigned char* cp = smem + (size_t)pos * CHUNK_BYTES;
+                    for (int t = t0; t < t1; ++t) {
+                        const uint4 e = tab.term[t];
+                        const uint32_t xt = e.x & 255u, xr = (e.x >> 8) & 63u, zr = (e.x >> 16) & 63u;
+                        const uint32_t oc = c ^ (xr >> LRC);
+                        const unsigned char* pb = cp + (((uint32_t)tid ^ xt) * (uint32_t)sizeof(C));
+                        const uint32_t sgn = (uint32_t)(__popc(bt & e.y) + __popc((oc << LRC) & zr)) << 31;
+                        const uint32_t w = (sizeof(T) == 8 ? e.w : e.z) ^ sgn;
+                        constexpr uint32_t lo = (uint32_t)RC - 1u;
+                        if (e.x >> 31) dispatch_chunk<T, R, RC, 0, true>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
+                        else dispatch_chunk<T, R, RC, 0, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_empty + 8 * pos);
+                    if (++pos == nring) {
+                        pos = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+            // epilogue: slice r of the tile is 256 consecutive amplitudes
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const uint64_t b = (uint64_t)(bt | tab.dep_r[r]);
+                C o;
+                if (FUSED) {
+                    const C mine = __ldg(p.in + b);
+                    double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
+                    if (p.prev) {
+                        const C pv = p.prev[b];
+                        orr -= s_prev * (double)pv.x;
+                        oi -= s_prev * (double)pv.y;
+                    }
+                    o.x = (T)orr;
+                    o.y = (T)oi;
+                    dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+                } else {
+                    o.x = ar[r];
+                    o.y = ai[r];
+                }
+                p.out[b] = o;
+            }
+        }
+        if (FUSED) {
+            // fixed-order sum over the 256 consumer threads (named barrier 1: the producer warpgroup has left)
+            dot = warp_sum(dot);
+            if (lane == 0) red[warp] = dot;
+            asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+            if (warp == 0) {
+                double s = lane < kConsumerWarps ? red[lane] : 0.0;
+                s = warp_sum(s);
+                if (lane == 0) {
+                    p.sc->partial_dot[blockIdx.x] = s;
+                    if (blockIdx.x == 0) p.sc->n_partial_dot = gridDim.x;
+                }
+            }
+        }
+    }
+}
+
+// NR (log2 accumulators per thread) and LRC (log2 slices per ring chunk) per dtype index (SYK_C64 = 0, SYK_C128 = 1):
+// 128 KiB tiles in two 64 KiB chunks
+constexpr int kStNR[2] = {6, 5};
+constexpr int kStLRC[2] = {5, 4};
+
+uint32_t extract_bits(uint32_t v, const int* pos, int n) {
+    uint32_t r = 0;
+    for (int i = 0; i < n; ++i) r |= ((v >> pos[i]) & 1u) << i;
+    return r;
+}
+uint32_t deposit_bits(uint32_t v, const int* pos, int n) {
+    uint32_t r = 0;
+    for (int i = 0; i < n; ++i) r |= ((v >> i) & 1u) << pos[i];
+    return r;
+}
+
+struct LayoutCost {
+    int loads, passes;
+    int total() const { return loads + 2 * passes; }
+};
+
+// #loads = distinct x outside the tile bits; #passes = distinct x outside tile + window bits.  seq = the free
+// positions (index bits >= 11): seq[0..nr) are the free r bits, seq[nr..nr+kWindowBits) the window bits.
+LayoutCost layout_cost(const std::vector<uint32_t>& xs, const std::vector<int>& seq, int nr, std::vector<uint32_t>& tmp) {
+    uint32_t tile = (1u << (kThreadBits + kFixedR)) - 1u;
+    for (int i = 0; i < nr; ++i) tile |= 1u << seq[i];
+    uint32_t win = tile;
+    for (int i = nr; i < nr + kWindowBits && i < (int)seq.size(); ++i) win |= 1u << seq[i];
+    LayoutCost c;
+    tmp.resize(xs.size());
+    for (size_t i = 0; i < xs.size(); ++i) tmp[i] = xs[i] & ~tile;
+    std::sort(tmp.begin(), tmp.end());
+    c.loads = (int)(std::unique(tmp.begin(), tmp.end()) - tmp.begin());
+    for (size_t i = 0; i < xs.size(); ++i) tmp[i] = xs[i] & ~win;
+    std::sort(tmp.begin(), tmp.end());
+    c.passes = (int)(std::unique(tmp.begin(), tmp.end()) - tmp.begin());
+    return c;
+}
+
+// Deterministic first-improvement hill climbing over swaps that move a bit between the classes r / window / rest,
+// started from the identity layout (free r bits = 11.., window = the next 7).  nr = number of FREE r bits.
+void choose_layout(const std::vector<uint32_t>& xs, int L, int nr, std::vector<int>& seq) {
+    seq.clear();
+    for (int q = kThreadBits + kFixedR; q < L; ++q) seq.push_back(q);
+    const int n = (int)seq.size();
+    const int nw = std::min(kWindowBits, n - nr);
+    std::vector<uint32_t> tmp;
+    int cur = layout_cost(xs, seq, nr, tmp).total();
+    auto cls = [&](int i) { return i < nr ? 0 : (i < nr + nw ? 1 : 2); };
+    for (int sweep = 0; sweep < 16; ++sweep) {
+        bool improved = false;
+        for (int i = 0; i < nr + nw; ++i)
+            for (int j = i + 1; j < n; ++j) {
+                if (cls(i) == cls(j)) continue;
+                std::swap(seq[i], seq[j]);
+                const int c = layout_cost(xs, seq, nr, tmp).total();
+                if (c < cur) {
+                    cur = c;
+                    improved = true;
+                } else {
+                    std::swap(seq[i], seq[j]);
+                }
+            }
+        if (!improved) break;
+    }
+    // canonical order inside each class (the cost does not depend on it): ascending bit positions
+    std::sort(seq.begin(), seq.begin() + nr);
+    std::sort(seq.begin() + nr, seq.begin() + nr + nw);
+    std::sort(seq.begin() + nr + nw, seq.end());
+}
+
+bool build_st_table(const syk_ham* h, int dtype, StTable& tab) {
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    const int nr = kStNR[k];
+    const size_t nt = h->z.size();
+    if (nt == 0 || nt > (size_t)kStMaxTerms || h->L < kThreadBits + nr) return false;
+    std::vector<uint32_t> xs;
+    for (size_t g = 0; g < h->x.size(); ++g) xs.push_back((uint32_t)h->x[g]);
+    std::vector<int> seq;
+    choose_layout(xs, h->L, nr - kFixedR, seq);
+    const int n_outer = h->L - kThreadBits - nr;
+    std::vector<int> pvec;
+    for (int i = 0; i < kFixedR; ++i) pvec.push_back(kThreadBits + i);
+    for (int i = 0; i < nr - kFixedR; ++i) pvec.push_back(seq[i]);
+    const int* P = pvec.data();
+    const int* O = seq.data() + (nr - kFixedR);
+    uint32_t omask = 0;
+    for (int i = 0; i < n_outer; ++i) omask |= 1u << O[i];
+
+    struct Item { uint32_t key, xo; uint32_t order; uint4 e; };
+    std::vector<Item> items;
+    items.reserve(nt);
+    for (size_t g = 0; g < h->x.size(); ++g) {
+        const uint32_t x = (uint32_t)h->x[g];
+        for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1]; ++t) {
+            const std::complex<double> c = h->c[t];
+            const bool imag = c.imag() != 0.0;
+            if (imag && c.real() != 0.0) return false;   // never for SYK strings (c = J s^4 {1,-1,i,-i})
+            const double a = imag ? c.imag() : c.real();
+            const uint32_t z = (uint32_t)h->z[t];
+            Item it;
+            it.key = extract_bits(x, O, n_outer);
+            it.xo = x & omask;
+            it.order = (uint32_t)items.size();
+            it.e.x = (x & 255u) | (extract_bits(x, P, nr) << 8) | (extract_bits(z, P, nr) << 16) | (imag ? 0x80000000u : 0u);
+            it.e.y = z;
+            if (dtype == SYK_C128) {
+                uint64_t bits;
+                std::memcpy(&bits, &a, 8);
+                it.e.z = (uint32_t)bits;
+                it.e.w = (uint32_t)(bits >> 32);
+            } else {
+                const float af = (float)a;   // R-C64: rounded once
+                uint32_t bits;
+                std::memcpy(&bits, &af, 4);
+                it.e.z = bits;
+                it.e.w = 0;
+            }
+            items.push_back(it);
+        }
+    }
+    std::sort(items.begin(), items.end(), [](const Item& a, const Item& b) {
+        return a.key != b.key ? a.key < b.key : a.order < b.order;
+    });
+    int n_loads = 0;
+    for (size_t i = 0; i < items.size(); ++i) {
+        if (i == 0 || items[i].key != items[i - 1].key) {
+            if (n_loads >= kStMaxLoads) return false;
+            tab.load_xo[n_loads] = items[i].xo;
+            tab.load_t0[n_loads] = (uint16_t)i;
+            ++n_loads;
+        }
+        tab.term[i] = items[i].e;
+    }
+    tab.load_t0[n_loads] = (uint16_t)items.size();
+    tab.n_loads = n_loads;
+    tab.n_outer = n_outer;
+    tab.nr = nr;
+    for (int s = 0; s < 64; ++s) tab.dep_r[s] = s < (1 << nr) ? deposit_bits((uint32_t)s, P, nr) : 0u;
+    for (int i = 0; i < 32; ++i) tab.outer_pos[i] = i < n_outer ? (uint8_t)O[i] : 0;
+    uint32_t tile = 255u;
+    for (int i = 0; i < nr; ++i) tile |= 1u << P[i];
+    tab.tile_mask = tile;
+    return true;
+}
+
+const StTable* get_st_table(const syk_ham* h, int dtype) {
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    if (!h->st[k]) h->st[k] = new (std::nothrow) StCache();
+    if (!h->st[k]) return nullptr;
+    if (!h->st[k]->valid) {
+        if (!build_st_table(h, dtype, h->st[k]->tab)) return nullptr;
+        h->st[k]->valid = true;
+    }
+    return &h->st[k]->tab;
+}
+
+template <typename T, int NR, int LRC>
+int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_out, const FusedArgs& fa,
+              cudaStream_t stream) {
+    using C = typename Cx<T>::type;
+    constexpr size_t kChunkBytes = ((size_t)1 << LRC) * kConsumerThreads * sizeof(C);
+    StParams<T> p;
+    p.in = (const C*)d_in;
+    p.out = (C*)d_out;
+    p.prev = (const C*)fa.prev;
+    p.sc = fa.sc;
+    p.j = fa.j;
+    p.nring = (int)((kSmemLimit - kMiscBytes) / kChunkBytes);
+    if (p.nring > kMaxRing) p.nring = kMaxRing;
+    const size_t smem = (size_t)p.nring * kChunkBytes + kMiscBytes;
+    const int sms = num_sms();
+    if (sms <= 0) return SYK_ECUDA;
+    const uint64_t n_tiles = 1ull << tab.n_outer;
+    const int grid = (int)(n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms);
+    // lock-step only where it pays: the vector does not fit in L2 and there are several rounds of tiles
+    int epoch_len = 0, lag = 0;
+    get_lockstep(&epoch_len, &lag);
+    p.sync = nullptr;
+    p.epoch_len = epoch_len;
+    p.lag = lag;
+    if (epoch_len > 0 && ((uint64_t)sizeof(C) << h->L) > ((uint64_t)64 << 20) && n_tiles >= 4 * (uint64_t)grid) {
+        p.sync = h->dev.sync;
+        SYK_CUDA(cudaMemsetAsync(p.sync, 0, kSyncRing * sizeof(uint32_t), stream));
+    }
+    if (fa.sc) {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, true>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_scatter_kernel<T, NR, LRC, true><<<grid, kThreads, smem, stream>>>(tab, p);
+    } else {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_scatter_kernel<T, NR, LRC, false><<<grid, kThreads, smem, stream>>>(tab, p);
+    }
+    count_launch();
+    SYK_CUDA(cudaGetLastError());
+    return SYK_OK;
+}
+
+}  // namespace
+
+// 0 if the handle cannot use the kernel, else log2 of its tile size in amplitudes
+int scatter_tile_log2(const syk_ham* h, int dtype, bool forced) {
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    const int tl = kThreadBits + kStNR[k];
+    if (h->n_terms() == 0 || h->n_terms() > kStMaxTerms || h->L < tl) return 0;
+    // automatic choice: at least ~4 rounds of 128 KiB tiles on 148 SMs
+    if (!forced && h->L < tl + 10) return 0;
+    return get_st_table(h, dtype) ? tl : 0;
+}
+
+int launch_apply_h_scatter(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                           cudaStream_t stream) {
+    const StTable* tab = get_st_table(h, dtype);
+    if (!tab) return SYK_EINVAL;
+    if (dtype == SYK_C128) return launch_st<double, kStNR[1], kStLRC[1]>(h, *tab, d_in, d_out, fa, stream);
+    return launch_st<float, kStNR[0], kStLRC[0]>(h, *tab, d_in, d_out, fa, stream);
+}
+
+int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask, uint32_t* window_mask) {
+    const StTable* tab = get_st_table(h, dtype);
+    if (!tab) return SYK_EINVAL;
+    uint32_t win = tab->tile_mask;
+    for (int i = 0; i < kWindowBits && i < tab->n_outer; ++i) win |= 1u << tab->outer_pos[i];
+    std::vector<uint32_t> v;
+    for (size_t g = 0; g < h->x.size(); ++g) v.push_back((uint32_t)h->x[g] & ~win);
+    std::sort(v.begin(), v.end());
+    if (n_loads) *n_loads = tab->n_loads;
+    if (n_passes) *n_passes = (int)(std::unique(v.begin(), v.end()) - v.begin());
+    if (tile_mask) *tile_mask = tab->tile_mask;
+    if (window_mask) *window_mask = win;
+    return SYK_OK;
+}
+
+void free_scatter_tables(const syk_ham* h) {
+    for (int k = 0; k < 2; ++k) {
+        delete h->st[k];
+        h->st[k] = nullptr;
+    }
+}
+
+}  // namespace syk

@@ -14,6 +14,7 @@ namespace syk {
 // ---------------------------------------------------------------------------------------------------------
 // Host tables of one Hamiltonian in canonical order (a-1) and their device copy.
 // ---------------------------------------------------------------------------------------------------------
+constexpr int kSyncRing = 32;      // epoch counters of the register-tile kernel's lock-step (apply_h_regtile.cu)
 struct DeviceTables {
     uint32_t* gx = nullptr;        // [n_groups]    X-mask of each group
     uint32_t* goff = nullptr;      // [n_groups+1]  first term of each group
@@ -25,6 +26,7 @@ struct DeviceTables {
     uint32_t* load_hi[2] = {nullptr, nullptr};     // [n_loads]    x >> tile_log2
     uint32_t* load_g0[2] = {nullptr, nullptr};     // [n_loads+1]  first group of each load
     int n_loads[2] = {0, 0};
+    uint32_t* sync = nullptr;      // [kSyncRing] epoch counters of the register-tile kernel's lock-step (zeroed per launch)
     int device = -1;
     void* blob = nullptr;          // single allocation holding all of the above
 };
@@ -49,6 +51,24 @@ struct RtCache {
     RtTable tab;
     int valid_for = -1;                    // dtype * 64 + tile_log2 the table was built for
 };
+// Term/load table of the scatter-tile kernel (apply_h_scatter.cu), also a __grid_constant__ parameter.
+constexpr int kStMaxTerms = 1024;
+constexpr int kStMaxLoads = 1024;
+struct StTable {
+    // term t: .x = low 8 bits of x | (r bits of x) << 8 | (r bits of z) << 16 | (coefficient is imaginary) << 31 ;
+    //         .y = Z-mask ; (.z, .w) = bits of the signed magnitude a (double), or .z = bits of (float) a
+    uint4 term[kStMaxTerms];
+    uint32_t load_xo[kStMaxLoads];         // x restricted to the outer bit positions, per load (sorted by tile counter)
+    uint16_t load_t0[kStMaxLoads + 2];     // first term of each load
+    uint32_t dep_r[64];                    // r -> its bits deposited at the tile's r-bit positions
+    uint8_t outer_pos[32];                 // outer bit positions, [0] = fastest bit of the tile counter
+    uint32_t tile_mask;                    // thread bits | r bits
+    int n_loads, n_outer, nr;
+};
+struct StCache {
+    StTable tab;
+    bool valid = false;
+};
 }  // namespace syk
 
 struct syk_ham {
@@ -64,6 +84,7 @@ struct syk_ham {
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable syk::DeviceTables dev;             // created on first device use
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
+    mutable syk::StCache* st[2] = {nullptr, nullptr};   // scatter-tile kernel tables per dtype (host, lazily built)
     int64_t n_terms() const { return (int64_t)z.size(); }
     int64_t n_groups() const { return (int64_t)x.size(); }
 };
@@ -135,6 +156,16 @@ int regtile_tile_log2(const syk_ham* h, int dtype, bool forced);
 int launch_apply_h_regtile(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
                            cudaStream_t stream);
 void free_regtile_tables(const syk_ham* h);
+void set_lockstep(int epoch_len, int lag);
+void get_lockstep(int* epoch_len, int* lag);
+
+// scatter-tile kernel (apply_h_scatter.cu)
+int scatter_tile_log2(const syk_ham* h, int dtype, bool forced);
+int launch_apply_h_scatter(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                           cudaStream_t stream);
+int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
+                        uint32_t* window_mask);
+void free_scatter_tables(const syk_ham* h);
 
 // apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

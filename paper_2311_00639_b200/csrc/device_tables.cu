@@ -112,7 +112,8 @@ int ensure_device_tables(const syk_ham* h) {
         off_g0[k] = cur;
         cur = align(cur + g0[k].size() * 4);
     }
-    const size_t total = cur + 256;
+    const size_t off_sync = cur;
+    const size_t total = cur + align(kSyncRing * 4) + 256;
 
     std::vector<unsigned char> host(total, 0);
     uint32_t* p_gx = (uint32_t*)(host.data() + off_gx);
@@ -148,6 +149,7 @@ int ensure_device_tables(const syk_ham* h) {
     d.tz = (uint32_t*)(b + off_tz);
     d.tc128 = (double2*)(b + off_c128);
     d.tc64 = (float2*)(b + off_c64);
+    d.sync = (uint32_t*)(b + off_sync);
     for (int k = 0; k < 2; ++k) {
         d.load_hi[k] = (uint32_t*)(b + off_hi[k]);
         d.load_g0[k] = (uint32_t*)(b + off_g0[k]);

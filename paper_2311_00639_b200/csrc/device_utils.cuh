@@ -51,6 +51,25 @@ __device__ __forceinline__ double reduce_partials(const double* p, int n, double
     return block_sum(s, red);
 }
 
+// Lock-step of persistent CTAs (register-tile and scatter-tile apply_H kernels).  The L2 reuse of those kernels is
+// BETWEEN CTAs: source tile (T ^ d) ^ hi of a neighbouring output tile T ^ d is the source tile T ^ (hi ^ d) of tile
+// T, and loads are sorted by hi, so a line fetched from DRAM for one CTA is wanted by another CTA one or two loads
+// later -- provided both CTAs are at the same place of the load list.  Free-running CTAs drift apart by more loads
+// than L2 holds (ncu, N = 64: 5 % hit rate), so the producers pace each other: loads are counted in epochs of
+// `epoch_len`; a producer that starts epoch e first reports epoch e-1 as issued (one atomicAdd on a ring of
+// kSyncRing counters) and then waits until all gridDim.x CTAs have reported epoch e-1-lag.  Timing only: no data
+// depends on it, results stay bitwise equal.  All CTAs are co-resident (grid <= number of SMs, one CTA per SM), so
+// the wait cannot deadlock.
+__device__ __forceinline__ void lockstep_gate(uint32_t* sync, uint32_t e, uint32_t lag) {
+    if (e == 0) return;
+    atomicAdd(sync + ((e - 1) % kSyncRing), 1u);
+    if (e < 1 + lag) return;
+    const uint32_t f = e - 1 - lag;
+    const uint32_t target = gridDim.x * (f / kSyncRing + 1);
+    const volatile uint32_t* c = sync + (f % kSyncRing);
+    while (*c < target) __nanosleep(64);
+}
+
 // ---- mbarrier and bulk async copy (TMA unit, non-tensor form: SASS UBLKCP) -------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

@@ -163,6 +163,7 @@ void syk_free_hamiltonian(syk_ham* h) {
     if (!h) return;
     syk::free_device_tables(h);
     syk::free_regtile_tables(h);
+    syk::free_scatter_tables(h);
     delete h;
 }
 

@@ -45,20 +45,20 @@ def _fullsize_case(B, N, k, tdt, tol, n_samples):
     h = B.syk_build_hamiltonian(N, p, 0, 0)
     assert h.info()["n_terms"] == len(J)
     code = B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64
-    assert B.syk_apply_H_kernel_kind(h, code) == 2                        # the kernel bench.py times
+    assert B.syk_apply_H_kernel_kind(h, code) == 3                        # the kernel bench.py times
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
     d_in = torch.empty(D, dtype=tdt, device="cuda")
     d_out = torch.empty(D, dtype=tdt, device="cuda")
     B.syk_random_state(N, 0, 0, d_in, scratch)
     # (i) sampled outputs, including the first/last amplitude and the first/last tiles of the vector (16 KiB and
-    #     64 KiB tiles), for both TMA kernels; the default (register-tile) kernel runs last and feeds (ii)
+    #     64 / 128 KiB tiles), for all three TMA kernels; the default (scatter-tile) kernel runs last and feeds (ii)
     idx = inputs.sample_indices(D, n_samples, seed=17)
     edge = np.array([1, 1023, 1024, 4095, 4096, 8191, 8192, D // 2 - 1, D // 2, D - 8192, D - 4097, D - 1024, D - 2],
                     dtype=np.uint64)
     idx = np.unique(np.concatenate([idx, edge]))
     ref = _oracle_samples(N, q, J, idx, d_in)
     scale = np.sqrt(np.mean(np.abs(ref) ** 2))
-    for kind in (1, 2):
+    for kind in (1, 2, 3):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, code) == kind
         d_out.zero_()
@@ -137,3 +137,34 @@ def test_lanczos_step_N56_hermiticity(B):
     assert abs(beta[0] - 1.0) <= 1e-13
     assert abs(alpha[0] - a1) <= 1e-13
     assert abs(beta[1] ** 2 - (h2 - a1 * a1)) <= 1e-12
+
+
+def test_lockstep_pacing_does_not_change_results(B):
+    """syk_set_lockstep only paces the producers of the register-tile kernel: outputs are bitwise equal for free
+    running CTAs, the default pacing and the tightest pacing (N=48: 268 MB vector > L2; both paced kernels)."""
+    import torch
+    N = 48
+    D = 1 << 24
+    h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 0, 3)
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    d_in = torch.empty(D, dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, 0, 3, d_in, scratch)
+    for kind in (2, 3):
+        B.syk_set_apply_H_kernel(h, kind)
+        assert B.syk_apply_H_kernel_kind(h, B.SYK_C128) == kind
+        outs = []
+        try:
+            for epoch_len, lag in ((0, 0), (8, 1), (1, 0), (3, 5)):
+                B.syk_set_lockstep(epoch_len, lag)
+                o = torch.zeros(D, dtype=torch.complex128, device="cuda")
+                B.syk_apply_H(h, d_in, o)
+                torch.cuda.synchronize()
+                outs.append(o)
+        finally:
+            B.syk_set_lockstep(8, 1)
+        for o in outs[1:]:
+            assert torch.equal(torch.view_as_real(o), torch.view_as_real(outs[0]))
+    with pytest.raises(B.SykError):
+        B.syk_set_lockstep(-1, 0)
+    with pytest.raises(B.SykError):
+        B.syk_set_lockstep(4, 31)

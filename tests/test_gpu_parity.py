@@ -75,7 +75,7 @@ APPLY_CASES = [
 @pytest.mark.parametrize("N,k,gn", APPLY_CASES)
 def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
     """out = H.in against the oracle's sequential-gamma product (O5), every kernel the handle can use
-    (0 generic, 1 16 KiB-tile TMA, 2 register-tile TMA)."""
+    (0 generic, 1 16 KiB-tile TMA, 2 register-tile TMA, 3 scatter-tile TMA)."""
     q, J = couplings(N, k, seed=1)
     D = 1 << (N // 2)
     v = inputs.gaussian_state(D, seed=100 + N, dtype=npdtype(dt))
@@ -83,11 +83,11 @@ def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
     h = B.syk_build_from_terms(N, q, J, gn)
     d_in = to_dev(torch, v)
     kinds = {0}
-    for want in (1, 2):
+    for want in (1, 2, 3):
         B.syk_set_apply_H_kernel(h, want)
         kinds.add(B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)))
     if N >= 28:
-        assert kinds == {0, 1, 2}
+        assert kinds == {0, 1, 2, 3}
     for kind in sorted(kinds):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
@@ -117,7 +117,7 @@ def test_apply_H_structured_masks(B, torch, qubits, dt):
     ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
     h = B.syk_build_from_terms(N, q, J)
     d_in = to_dev(torch, v)
-    for kind in (0, 1, 2):
+    for kind in (0, 1, 2, 3):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
         d_out = torch.zeros(D, dtype=tdtype(torch, dt), device="cuda")
@@ -294,6 +294,42 @@ def test_lanczos_identities(B, torch):
     # extremal Ritz values converge first: after 24 of 256 steps the lowest one is within 1 % of the band width
     assert abs(ritz.min() - w.min()) < 1e-2 * (w.max() - w.min())
     assert st["n_matvec"] == m
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_fused_lanczos_every_kernel_kind(B, torch, dt):
+    """The fused epilogue (out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, <u_j|out> partial sums) of every apply_H
+    kernel: 6 Lanczos steps at N=28 (several tiles) against the textbook three-term recurrence run with the oracle's
+    sequential-gamma matvec in fp64."""
+    N, m = 28, 6
+    q, J = couplings(N, 4, seed=2)
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 21, npdtype(dt))
+    v = psi.astype(np.complex128)
+    b0 = np.linalg.norm(v)
+    v = v / b0
+    v_prev = np.zeros_like(v)
+    beta_prev = 0.0
+    a_ref, b_ref = [], [b0]
+    for _ in range(m):
+        w = ohm.matvec_sequential(N, q, J, v) - beta_prev * v_prev
+        a = np.vdot(v, w).real
+        w = w - a * v
+        bn = np.linalg.norm(w)
+        a_ref.append(a)
+        b_ref.append(bn)
+        v_prev, v, beta_prev = v, w / bn, bn
+    h = B.syk_build_from_terms(N, q, J)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, code, {"krylov_dim": m}))
+    d_psi = to_dev(torch, psi)
+    tol = 1e-11 if dt == "c128" else 2e-5
+    for kind in (0, 1, 2, 3):
+        B.syk_set_apply_H_kernel(h, kind)
+        assert B.syk_apply_H_kernel_kind(h, code) == kind
+        alpha, beta, st = B.syk_lanczos_run(h, d_psi, m, wk)
+        assert np.max(np.abs(np.asarray(alpha) - np.asarray(a_ref))) <= tol, (kind, dt)
+        assert np.max(np.abs(np.asarray(beta) - np.asarray(b_ref))) <= tol, (kind, dt)
 
 
 EVOLVE_CASES = [
