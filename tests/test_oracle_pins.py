@@ -10,7 +10,7 @@ import os
 import numpy as np
 import pytest
 
-from oracle import alg1, evolve, hamiltonian, majorana, otoc, rng
+from oracle import alg1, evolve, green, hamiltonian, majorana, otoc, rng
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -343,3 +343,46 @@ def test_P12_qualitative_decay():
                 axis=0)
     ratio = (F / F[0]).real
     assert ratio[0] == 1.0 and 0.5 < ratio[1] < 1.0 and ratio[2] < 0.85
+
+
+# ---------------------------------------------------------------- P13 Green function closed forms
+@pytest.mark.parametrize("gamma_norm", [0, 1])
+def test_P13_green_closed_forms(gamma_norm):
+    """G(t) = <psi|e^{(it-b/2)H} g e^{-iHt} g e^{-bH/2}|psi>: (i) G(0) = s^2 <psi|e^{-bH}|psi> from the spectral
+    sum; (ii) H = 0: G = s^2 for all t; (iii) one-term H = J P with g anticommuting with P: g e^{-iHt} g =
+    s^2 e^{+iHt}, so G(t) = s^2 <psi|e^{(2it - b)H}|psi> = s^2 [cosh(zJs^4) + sinh(zJs^4) <P>/s^4], z = 2it - b;
+    with g commuting with P the t-dependence cancels: G(t) = G(0); (iv) the same-psi value averaged over many psi
+    approaches the exact trace, which is what PAPER.md:212 estimates."""
+    s = majorana.gamma_scale(gamma_norm)
+    s2, s4 = s * s, s ** 4
+    N = 8
+    q, J, _ = rng.sample_couplings(N, 1.0, seed=7, realization=0)
+    prop = evolve.ExactPropagator(N, q, J, gamma_norm)
+    H = hamiltonian.dense_hamiltonian(N, q, J, gamma_norm)
+    w, U = np.linalg.eigh(H)
+    psi = _random_state(16, 3)
+    beta = 1.7
+    G0 = green.green_same_psi(prop, N, N - 1, beta, [0.0], psi, gamma_norm)[0]
+    assert abs(G0 - s2 * np.sum(np.abs(U.conj().T @ psi) ** 2 * np.exp(-beta * w))) < 1e-13
+    # (ii) empty Hamiltonian
+    empty = evolve.ExactPropagator(N, np.zeros((0, 4), dtype=np.int32), np.zeros(0), gamma_norm)
+    assert np.allclose(green.green_same_psi(empty, N, 2, beta, [0.0, 1.0, 3.0], psi, gamma_norm), s2, atol=1e-14)
+    # (iii) single term (0,1,2,3) = -s^4 Z0 Z1: gamma_0 (X on qubit 0) anticommutes with it, gamma_6 commutes
+    Jq = 0.83
+    one = evolve.ExactPropagator(N, np.array([[0, 1, 2, 3]], dtype=np.int32), np.array([Jq]), gamma_norm)
+    P = hamiltonian.dense_hamiltonian(N, np.array([[0, 1, 2, 3]], dtype=np.int32), np.array([1.0]), gamma_norm)
+    expP = np.vdot(psi, P @ psi).real / s4
+    t_grid = np.array([0.0, 0.4, 1.3])
+    z = 2j * t_grid - beta
+    want = s2 * (np.cosh(z * Jq * s4) + np.sinh(z * Jq * s4) * expP)
+    assert np.allclose(green.green_same_psi(one, N, 0, beta, t_grid, psi, gamma_norm), want, atol=1e-13)
+    Gc = green.green_same_psi(one, N, 6, beta, t_grid, psi, gamma_norm)
+    assert np.allclose(Gc, Gc[0], atol=1e-13)
+    # (iv) trace estimator
+    g = majorana.jw_gammas(N, gamma_norm)
+    tg = [0.0, 0.7, 1.9]
+    Gtr = green.green_exact_trace(H, g[N - 1], 1.0, tg)
+    est = np.mean([green.green_same_psi(prop, N, N - 1, 1.0, tg, _random_state(16, 500 + k), gamma_norm)
+                   for k in range(300)], axis=0)
+    assert np.allclose(est, Gtr, atol=0.12 * abs(Gtr[0]))
+    assert abs(Gtr[0].imag) < 1e-13 and Gtr[0].real > 0
