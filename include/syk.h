@@ -158,6 +158,14 @@ int syk_otoc(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const d
              void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
              syk_stats* stats, void* stream);
 
+/* Retarded Green function:  G(t) = <psi| e^{(it-b/2)H} g_n e^{-iHt} g_n e^{-bH/2} |psi>  for t in
+ * t_grid (non-decreasing, >= 0); G_out[n_t][2] (host) receives the un-normalised complex values, G_R(t) =
+ * Re G(t)/G(0) is the caller's division.  Same work space, ownership and error rules as syk_otoc (d_psi is
+ * destroyed; syk_otoc_workspace_bytes). */
+int syk_green(const syk_ham* h, int dtype, int n, double beta, const double* t_grid, int n_t, void* d_psi,
+              double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+              void* stream);
+
 /* Batched over disorder realizations: realization r uses hams[r], state d_psi + r*batch_stride elements, and
  * writes F_out[r][n_t][2].  One work space is shared (realizations run back to back on `stream`). */
 int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,

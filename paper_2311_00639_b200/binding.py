@@ -70,6 +70,7 @@ _SIGNATURES = {
     "syk_krylov_evolve_host": (_i, [_vp, _i, _vp, _d, _d, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
     "syk_otoc_workspace_bytes": (_i, [_vp, _i, _P(syk_krylov_opts), _P(_sz)]),
     "syk_otoc": (_i, [_vp, _i, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
+    "syk_green": (_i, [_vp, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
     "syk_otoc_batched": (_i, [_P(_vp), _i, _i, _i, _i, _d, _vp, _i, _vp, _i64, _vp, _P(syk_krylov_opts), _vp, _sz,
                               _P(syk_stats), _vp]),
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
@@ -320,6 +321,17 @@ def syk_otoc(h, i_W, j_V, beta, t_grid, d_psi, d_work, opts=None, stream=None):
                          _dptr(d_psi), F.ctypes.data, _opts(opts), _dptr(d_work),
                          d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)), "syk_otoc")
     return F[:, 0] + 1j * F[:, 1], st.as_dict()
+
+
+def syk_green(h, n, beta, t_grid, d_psi, d_work, opts=None, stream=None):
+    """Returns (G[n_t] complex128 un-normalised, stats).  d_psi is destroyed."""
+    t = np.ascontiguousarray(t_grid, dtype=np.float64)
+    G = np.zeros((len(t), 2), dtype=np.float64)
+    st = syk_stats()
+    _check(_lib.syk_green(_h(h), dtype_code(d_psi), int(n), float(beta), t.ctypes.data, len(t), _dptr(d_psi),
+                          G.ctypes.data, _opts(opts), _dptr(d_work), d_work.numel() * d_work.element_size(),
+                          ctypes.byref(st), _stream(stream)), "syk_green")
+    return G[:, 0] + 1j * G[:, 1], st.as_dict()
 
 
 def syk_otoc_batched(hams, i_W, j_V, beta, t_grid, d_psi, batch_stride, d_work, opts=None, stream=None):

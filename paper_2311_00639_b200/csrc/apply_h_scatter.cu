@@ -31,7 +31,8 @@
 // bank).  No atomics on data, one write per output: bitwise reproducible.
 //
 // Fused Lanczos epilogue (a-3 part 1) as in apply_h.cu: out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, per-CTA fp64
-// partial sums of Re<in|out> (in[b] re-read from global: an L2 hit, the tile has just been staged).
+// partial sums of Re<in|out>.  The tile of `in` and of `prev` are staged through the same ring after the last
+// source tile (their DRAM latency would otherwise be exposed once per tile: measured 50 ms of 385 ms at N = 64).
 //
 // Measured (profiles/r1e_*.md): both headline workloads sit at the L2 -> SM throughput ceiling (~6000-6600 B/clk
 // chip-wide): #loads x V / time = 12.1 TB/s (N = 56 complex128) and 10.1 TB/s (N = 64 complex64).
@@ -199,6 +200,27 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                     }
                 }
             }
+            if (FUSED) {
+                // operands of the fused epilogue, staged like source tiles so that their latency is hidden:
+                // chunk c of in's own tile, then chunk c of prev's
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    for (int which = 0; which < (p.prev ? 2 : 1); ++which) {
+                        const C* from = which ? p.prev : p.in;
+                        mbar_wait(bar_empty + 8 * pos, phase ^ 1u);
+                        mbar_arrive_expect_tx(bar_full + 8 * pos, CHUNK_BYTES);
+#pragma unroll
+                        for (int u = 0; u < RC / kRun; ++u)
+                            bulk_load(stage0 + (uint32_t)pos * CHUNK_BYTES + (uint32_t)u * RUN_BYTES,
+                                      from + (uint64_t)(base | tab.dep_r[c * RC + u * kRun]), RUN_BYTES,
+                                      bar_full + 8 * pos);
+                        if (++pos == nring) {
+                            pos = 0;
+                            phase ^= 1u;
+                        }
+                    }
+                }
+            }
         }
         if (p.sync) {
             // report every remaining epoch of the longest-running CTA, so that nobody waits for this one
@@ -247,26 +269,58 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 }
             }
             // epilogue: slice r of the tile is 256 consecutive amplitudes
+            if constexpr (FUSED) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const uint64_t b = (uint64_t)(bt | tab.dep_r[r]);
-                C o;
-                if (FUSED) {
-                    const C mine = __ldg(p.in + b);
-                    double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
-                    if (p.prev) {
-                        const C pv = p.prev[b];
-                        orr -= s_prev * (double)pv.x;
-                        oi -= s_prev * (double)pv.y;
+                for (int c = 0; c < NC; ++c) {
+                    mbar_wait(bar_full + 8 * pos, phase);
+                    const C* mine_s = reinterpret_cast<const C*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
+                    const int pos_in = pos;
+                    if (++pos == nring) {
+                        pos = 0;
+                        phase ^= 1u;
                     }
-                    o.x = (T)orr;
-                    o.y = (T)oi;
-                    dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
-                } else {
+                    const C* prev_s = nullptr;
+                    int pos_prev = 0;
+                    if (p.prev) {
+                        mbar_wait(bar_full + 8 * pos, phase);
+                        prev_s = reinterpret_cast<const C*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
+                        pos_prev = pos;
+                        if (++pos == nring) {
+                            pos = 0;
+                            phase ^= 1u;
+                        }
+                    }
+#pragma unroll
+                    for (int rl = 0; rl < RC; ++rl) {
+                        const int r = c * RC + rl;
+                        const uint64_t b = (uint64_t)(bt | tab.dep_r[r]);
+                        const C mine = mine_s[rl * kConsumerThreads];
+                        double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
+                        if (prev_s) {
+                            const C pv = prev_s[rl * kConsumerThreads];
+                            orr -= s_prev * (double)pv.x;
+                            oi -= s_prev * (double)pv.y;
+                        }
+                        C o;
+                        o.x = (T)orr;
+                        o.y = (T)oi;
+                        dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+                        p.out[b] = o;
+                    }
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(bar_empty + 8 * pos_in);
+                        if (prev_s) mbar_arrive(bar_empty + 8 * pos_prev);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    C o;
                     o.x = ar[r];
                     o.y = ai[r];
+                    p.out[(uint64_t)(bt | tab.dep_r[r])] = o;
                 }
-                p.out[b] = o;
             }
         }
         if (FUSED) {

@@ -59,6 +59,50 @@ static int otoc_one(const syk_ham* h, int dtype, int i_W, int j_V, double beta, 
     return rc_soft;
 }
 
+// Retarded Green function:
+//   G(t) = <psi| e^{(it-b/2)H} g_n e^{-iHt} g_n e^{-bH/2} |psi> = < E(t) l0 | g_n E(t) g_n l0 >,  l0 = E(-ib/2) psi,
+// so both sides advance incrementally along the t grid: two evolutions by dt per grid point, one gamma insertion,
+// one inner product.  Resident: l (in psi's buffer), phi, r + Krylov work.
+static int green_one(const syk_ham* h, int dtype, int n, double beta, const double* t_grid, int n_t, void* d_psi,
+                     double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                     cudaStream_t st) {
+    const uint64_t D = 1ull << h->L;
+    const size_t vbytes = (size_t)D * elem_bytes(dtype);
+    size_t kbytes = 0;
+    SYK_TRY(syk_krylov_workspace_bytes(h, dtype, opts, &kbytes));
+    if (work_bytes < 2 * vbytes + kbytes) return SYK_ENOMEM;
+    char* l = (char*)d_psi;
+    char* phi = (char*)d_work;
+    char* r = phi + vbytes;
+    char* kwork = r + vbytes;
+    LanczosScalars* sc = (LanczosScalars*)kwork;
+    const int N = h->N, gn = h->gamma_norm;
+    int rc_soft = SYK_OK;
+    auto evolve = [&](void* v, double tre, double tim) -> int {
+        int rc = krylov_evolve_impl(h, dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+        if (rc == SYK_ENOCONV) {
+            rc_soft = rc;
+            return SYK_OK;
+        }
+        return rc;
+    };
+    SYK_TRY(evolve(l, 0.0, -beta / 2.0));
+    SYK_TRY(launch_gamma(N, n, gn, dtype, l, phi, st));
+    double t_prev = 0.0;
+    for (int k = 0; k < n_t; ++k) {
+        const double dt = t_grid[k] - t_prev;
+        if (dt > 0.0) {
+            SYK_TRY(evolve(l, dt, 0.0));
+            SYK_TRY(evolve(phi, dt, 0.0));
+        }
+        t_prev = t_grid[k];
+        SYK_TRY(launch_gamma(N, n, gn, dtype, phi, r, st));
+        SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
+        SYK_TRY(fetch_cdot(sc, G_out + 2 * k, st));
+    }
+    return rc_soft;
+}
+
 static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
                          const void* d_psi, const double* F_out, const void* d_work) {
     if (!h || (dtype != SYK_C64 && dtype != SYK_C128) || !d_psi || !d_work || n_t < 0 || (n_t > 0 && (!t_grid || !F_out)))
@@ -91,6 +135,17 @@ int syk_otoc(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const d
     if (stats) *stats = syk_stats{};
     return syk::otoc_one(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, opts, d_work, work_bytes, stats,
                          (cudaStream_t)stream);
+}
+
+int syk_green(const syk_ham* h, int dtype, int n, double beta, const double* t_grid, int n_t, void* d_psi,
+              double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+              void* stream) {
+    // same argument rules as syk_otoc with a single operator index
+    if (!h || n < 0 || n >= h->N) return SYK_EINVAL;
+    if (!syk::otoc_args_ok(h, dtype, n, n == 0 ? 1 : 0, beta, t_grid, n_t, d_psi, G_out, d_work)) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    return syk::green_one(h, dtype, n, beta, t_grid, n_t, d_psi, G_out, opts, d_work, work_bytes, stats,
+                          (cudaStream_t)stream);
 }
 
 int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,

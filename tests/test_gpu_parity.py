@@ -9,6 +9,7 @@ import numpy as np
 import pytest
 
 from oracle import evolve as oev
+from oracle import green as ogreen
 from oracle import hamiltonian as ohm
 from oracle import majorana
 from oracle import otoc as ootoc
@@ -549,3 +550,48 @@ def test_otoc_argument_errors(B, torch):
     for args in ((3, 3, 1.0, [0.0]), (16, 0, 1.0, [0.0]), (0, 1, -1.0, [0.0]), (0, 1, 1.0, [1.0, 0.5])):
         with pytest.raises(B.SykError):
             B.syk_otoc(h, args[0], args[1], args[2], args[3], psi, wk, o)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-2 Green function
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_green_vs_oracle(B, torch, dt):
+    """G(t) = <psi|e^{(it-b/2)H} g e^{-iHt} g e^{-bH/2}|psi> against the exact-diagonalisation oracle, N=16 dense
+    (configs[0] Hamiltonian) and N=20 sparse; one-pass and two-pass."""
+    for N, k, n, beta, o in ((16, None, 15, 5.0, {"krylov_dim": 20}), (20, 4, 3, 2.0, {"krylov_dim": 16, "two_pass": 1})):
+        q, J = couplings(N, k, seed=0)
+        D = 1 << (N // 2)
+        psi = inputs.gaussian_state(D, 31, npdtype(dt))
+        prop = oev.ExactPropagator(N, q, J)
+        t_grid = np.array([0.0, 0.5, 1.0, 2.5, 2.5, 6.0])
+        ref = ogreen.green_same_psi(prop, N, n, beta, t_grid, psi.astype(np.complex128))
+        h = B.syk_build_from_terms(N, q, J)
+        code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+        wk = work(torch, B.syk_otoc_workspace_bytes(h, code, o))
+        G, st = B.syk_green(h, n, beta, t_grid, to_dev(torch, psi), wk, o)
+        assert np.max(np.abs(G - ref)) / abs(ref[0]) <= TOL[dt], (N, dt)
+        assert st["n_matvec"] > 0
+
+
+def test_green_closed_form_and_errors(B, torch):
+    """G(0) = s^2 <psi|e^{-bH}|psi>; beta = 0, t = 0 gives exactly s^2 for a normalised psi; argument errors."""
+    N = 20
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 5)
+    for gn, s2 in ((0, 1.0), (1, 0.5)):
+        h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 1, 0, gn)
+        o = {"krylov_dim": 12}
+        wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+        G, _ = B.syk_green(h, 7, 0.0, [0.0], to_dev(torch, psi), wk, o)
+        assert abs(G[0] - s2) <= 1e-13
+        d = to_dev(torch, psi)
+        B.syk_krylov_evolve(h, d, 0.0, -0.75, wk, o)                        # e^{-bH/2} psi, b = 1.5
+        n2 = float(torch.linalg.vector_norm(d).item()) ** 2
+        G, _ = B.syk_green(h, 7, 1.5, [0.0], to_dev(torch, psi), wk, o)
+        assert abs(G[0] - s2 * n2) <= 1e-12 * n2
+    for bad in (dict(n=-1), dict(n=N), dict(beta=-1.0), dict(t=[1.0, 0.5])):
+        with pytest.raises(B.SykError):
+            B.syk_green(h, bad.get("n", 3), bad.get("beta", 1.0), bad.get("t", [0.0]), to_dev(torch, psi), wk, o)
+    with pytest.raises(B.SykError):
+        B.syk_green(h, 3, 1.0, [0.0], to_dev(torch, psi), work(torch, 1024), o)
