@@ -43,6 +43,12 @@ WORKLOADS = {
     # smaller shapes of the same path (parity-test sizes; handy for quick runs and ncu)
     "N48_k4_c128": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                     "i_W": 47, "j_V": 46},
+    # BASELINE.json configs[1] / configs[2] shapes: disorder realizations batched on one GPU (run back to back on one
+    # stream; each step advances every realization by one time segment)
+    "N32_k4_c128_x100": {"N": 32, "k": 4, "dtype": "c128", "krylov_dim": 12, "two_pass": 0, "dt": 0.1, "beta": 5.0,
+                         "i_W": 31, "j_V": 30, "batch": 100},
+    "N48_k4_c128_x20": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 30, "two_pass": 0, "dt": 0.5, "beta": 5.0,
+                        "i_W": 47, "j_V": 46, "batch": 20},
     "N40_k4_c128": {"N": 40, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                     "i_W": 39, "j_V": 38},
 }
@@ -70,7 +76,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "500",
                  "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
@@ -224,7 +230,8 @@ def run_ours(args, wl, name):
     p = inputs.bernoulli_p(N, k)
     opts = {"krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"]}
     tau = (wl["dt"], 0.0)                            # one real-time segment of the t grid
-    realization = rank                               # independent realizations per rank (weak scaling)
+    batch = int(wl.get("batch", 1))
+    realization = rank * batch                       # independent realizations per rank (weak scaling)
 
     h0 = B.syk_build_hamiltonian(N, p, 0, realization)
     info = h0.info()
@@ -232,23 +239,26 @@ def run_ours(args, wl, name):
     kbytes = B.syk_krylov_workspace_bytes(h0, code, opts)
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
     wk = torch.empty(kbytes + V, dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
-    l = torch.empty(D, dtype=tdt, device="cuda")
-    r = torch.empty(D, dtype=tdt, device="cuda")
-    B.syk_random_state(N, 0, realization, r, scratch)
-    B.syk_apply_gamma(N, wl["j_V"], r, l)            # a second, different state for the bra side
+    l = torch.empty((batch, D), dtype=tdt, device="cuda")
+    r = torch.empty((batch, D), dtype=tdt, device="cuda")
+    for i in range(batch):
+        B.syk_random_state(N, 0, realization + i, r[i], scratch)
+        B.syk_apply_gamma(N, wl["j_V"], r[i], l[i])  # a second, different state for the bra side
     torch.cuda.synchronize()
 
     stats_acc = {"n_matvec": 0, "model_bytes": 0.0, "n_substeps": 0}
 
     def step():
-        h = B.syk_build_hamiltonian(N, p, 0, realization)                         # a-1
-        B.syk_apply_gamma(N, wl["i_W"], r, r)                                     # a-5 insertion (in place)
-        st = B.syk_krylov_evolve(h, r, tau[0], tau[1], wk, opts)                  # a-2, a-3, a-4
-        F = B.syk_dot(N, l, r, scratch)                                           # a-5 inner product
-        stats_acc["n_matvec"] += st["n_matvec"]
-        stats_acc["n_substeps"] += st["n_substeps"]
-        stats_acc["model_bytes"] += st["model_bytes"] + 4.0 * V                   # gamma: 2V, dot: 2V
-        h.close()
+        F = 0.0
+        for i in range(batch):
+            h = B.syk_build_hamiltonian(N, p, 0, realization + i)                     # a-1
+            B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                               # a-5 insertion (in place)
+            st = B.syk_krylov_evolve(h, r[i], tau[0], tau[1], wk, opts)               # a-2, a-3, a-4
+            F = B.syk_dot(N, l[i], r[i], scratch)                                     # a-5 inner product
+            stats_acc["n_matvec"] += st["n_matvec"]
+            stats_acc["n_substeps"] += st["n_substeps"]
+            stats_acc["model_bytes"] += st["model_bytes"] + 4.0 * V                   # gamma: 2V, dot: 2V
+            h.close()
         return F
 
     def barrier():
@@ -261,11 +271,11 @@ def run_ours(args, wl, name):
     for key in stats_acc:
         stats_acc[key] = 0
     B.syk_launch_count(reset=True)
-    B.syk_profile_enable(True)
+    B.syk_profile_enable(not args.no_kernel_timing)
     B.syk_profile_read(reset=True)
     sampler = ClockSampler(local)
     barrier()
-    if rank == 0:
+    if rank == 0 and not args.no_clocks:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -299,10 +309,12 @@ def run_ours(args, wl, name):
         host = torch.empty(D, dtype=tdt, pin_memory=True)
         fill_host_state(host.numpy(), 7 + rank)
         def e2e_step():
-            h = B.syk_build_hamiltonian(N, p, 0, realization)
-            st = B.syk_krylov_evolve_host(h, host, tau[0], tau[1], wk, opts)
-            h.close()
-            return st
+            tot = {"model_bytes": 0.0}
+            for i in range(batch):
+                h = B.syk_build_hamiltonian(N, p, 0, realization + i)
+                tot["model_bytes"] += B.syk_krylov_evolve_host(h, host, tau[0], tau[1], wk, opts)["model_bytes"]
+                h.close()
+            return tot
         e2e_step()
         barrier()
         n_e2e = max(1, min(args.steps, 3))
@@ -318,8 +330,8 @@ def run_ours(args, wl, name):
             b = torch.tensor([e2e_bytes], dtype=torch.float64, device="cuda")
             dist.all_reduce(b, op=dist.ReduceOp.SUM)
             t_e2e, e2e_bytes = float(t[0]), float(b[0])
-        e2e = {"value": e2e_bytes / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": V, "d2h_bytes_per_step": V,
-               "steps": n_e2e, "call": "syk_krylov_evolve_host (pinned host vector in and out each step)"}
+        e2e = {"value": e2e_bytes / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": V * batch,
+               "d2h_bytes_per_step": V * batch, "steps": n_e2e, "call": "syk_krylov_evolve_host (pinned host vector in and out each step)"}
         del host
     except Exception as ex:   # noqa: BLE001 -- report, do not hide
         e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
@@ -369,8 +381,10 @@ def run_ours(args, wl, name):
             "vs_baseline": None, "dtype": "f64" if wl["dtype"] == "c128" else "f32", "data": "synthetic",
             "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2, "n_terms": n_t, "n_xmasks": n_x,
                        "vector_bytes": V, "krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"],
-                       "tau": list(tau), "realizations_per_gpu": 1,
-                       "l2_policy": "inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9),
+                       "tau": list(tau), "realizations_per_gpu": batch,
+                       "l2_policy": ("inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9)) if V > 3e8 else
+                                    ("working set of one step %.2f GB > L2 (%d realizations x %d vectors of %.1f MB)"
+                                     % (batch * (wl["krylov_dim"] + 2) * V / 1e9, batch, wl["krylov_dim"] + 2, V / 1e6)),
                        "step": "build_hamiltonian + gamma insertion + krylov_evolve (m fused Lanczos steps, "
                                "host exp, combine) + inner product"},
             "lanczos_steps_per_s": total_matvec / (ms * 1e-3), "matvecs_per_step": total_matvec / args.steps / world,
@@ -390,6 +404,8 @@ def main():
     ap.add_argument("--workload", default="N56_k4_c128", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
+    ap.add_argument("--no-clocks", action="store_true", help="do not poll nvidia-smi (diagnosis only)")
+    ap.add_argument("--no-kernel-timing", action="store_true", help="no CUDA events around apply_H (diagnosis only)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("note: fewer than 3 warm-up steps; not a valid bench number", file=sys.stderr)
