@@ -14,11 +14,12 @@ Modules
   hamiltonian  dense H, monomial-row evaluation, derived integer tables, H.v     (O3-O5)
   evolve       exact exp(-i tau H) by full diagonalisation; Chebyshev series     (O6, O8)
   otoc         same-psi and exact-trace regularised OTOC                        (O7)
+  green        same-psi and exact-trace retarded Green function
   alg1         literal transcription of the paper's Algorithm 1 (Python + C)    (P6)
 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): Clifford algebra, Hermiticity/trace/parity,
 Tr H^2 closed form, hand-worked Pauli products (tests/golden/), two representations with one
 spectrum, literal Algorithm 1 vs dense, exactly solvable exponentials, group properties,
-OTOC closed forms.  Parity unpinned: none of the functions here; what stays unpinned is
+OTOC and Green-function closed forms.  Parity unpinned: none of the functions here; what stays unpinned is
 agreement with the paper's Fig. 1 curves and its iteration counts (no data in PAPER.md).
 """
