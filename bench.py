@@ -49,6 +49,9 @@ WORKLOADS = {
                          "i_W": 31, "j_V": 30, "batch": 100},
     "N48_k4_c128_x20": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 30, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                         "i_W": 47, "j_V": 46, "batch": 20},
+    # BASELINE.json configs[2], dense p = 1 member: ALU-bound (194 580 terms on 10 903 X-masks, ~0.75 s per matvec)
+    "N48_dense_c128": {"N": 48, "k": None, "dtype": "c128", "krylov_dim": 12, "two_pass": 0, "dt": 0.05, "beta": 5.0,
+                       "i_W": 47, "j_V": 46},
     "N40_k4_c128": {"N": 40, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                     "i_W": 39, "j_V": 38},
 }
@@ -346,7 +349,7 @@ def run_ours(args, wl, name):
     avg_ms = apply_ms / apply_n if apply_n else float("nan")
     achieved = per_launch_bytes / (avg_ms * 1e-3) / 1e9 if apply_n else None
     kernel_names = {0: "apply_h_generic_kernel", 1: "apply_h_tma_kernel", 2: "apply_h_regtile_kernel",
-                    3: "apply_h_scatter_kernel"}
+                    3: "apply_h_scatter_kernel", 4: "apply_h_dense_kernel"}
     kind = B.syk_apply_H_kernel_kind(h0, code)
     layout = B.syk_apply_H_layout(h0, code) if kind == 3 else None
     roofline = {"bound": "hbm", "kernel": kernel_names[kind], "layout": layout, "achieved": achieved, "peak": peak,
@@ -355,6 +358,15 @@ def run_ours(args, wl, name):
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms, "launches_timed": apply_n,
                 "share_of_step": apply_ms / ms if ms else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None}
+    if kind in (0, 4) and n_t > 8 * n_x:
+        # dense table: plain-ALU bound: amplitude-terms per second against the issue-slot peak
+        # 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz / 3 slots per amplitude-term (LOP3 + POPC + signed add)
+        alu_peak = 148 * 4 * 32 * 1.965e9 / 3.0 / 1e9
+        ach = n_t * D / (avg_ms * 1e-3) / 1e9 if apply_n else None
+        roofline.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "G amplitude-terms/s",
+                         "frac": ach / alu_peak if ach else None,
+                         "peak_source": "derived: 148 SM x 4 x 32 lanes x 1.965 GHz / 3 issue slots (DESIGN.md section 6)",
+                         "model_GBs_for_reference": achieved})
     # DRAM bytes per launch of that kernel from the last committed `ncu --set full` capture (profiles/traffic.csv)
     traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_file):

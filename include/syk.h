@@ -177,9 +177,11 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
 /* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined 16 KiB-tile gather,
  * 2 = TMA-pipelined register-tile gather (64 KiB tiles; sparse H with <= 1024 terms and D >= 2^22 / 2^23),
  * 3 = TMA-pipelined scatter-tile gather (128 KiB tiles on index bits chosen per Hamiltonian; sparse H with
- *     1..1024 terms and D >= 2^23 / 2^24). */
+ *     1..1024 terms and D >= 2^23 / 2^24),
+ * 4 = dense-table kernel (many terms per X-mask: terms binned by the Walsh index of their Z-mask and transformed once per
+ *     X-mask; chosen for > 1024 terms with >= 4 terms per X-mask and D >= 2^20; holds its own device table). */
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
-/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 as above
+/* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 / 4 as above
  * (a kind the handle cannot use falls back to the next lower one). */
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
 /* Tile layout the scatter-tile kernel (kind 3) chose for this Hamiltonian: n_loads = source tiles fetched per

@@ -369,6 +369,8 @@ int apply_h_kernel_kind(const syk_ham* h, int dtype) {
     const int avail = tma_stages(h, dtype) >= 3 ? 1 : 0;
     if (h->forced_kernel == 0) return 0;
     if (h->forced_kernel == 1) return avail;
+    if (h->forced_kernel == 4) return dense_kernel_ok(h, true) ? 4 : 0;
+    if (h->forced_kernel < 0 && dense_kernel_ok(h, false)) return 4;
     if (h->forced_kernel != 2 && scatter_tile_log2(h, dtype, h->forced_kernel == 3) > 0) return 3;
     if (regtile_tile_log2(h, dtype, h->forced_kernel >= 2) > 0) return 2;
     return avail;
@@ -379,7 +381,8 @@ int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, c
     SYK_TRY(ensure_device_tables(h));
     const int kind = apply_h_kernel_kind(h, dtype);
     profile_begin(stream);
-    const int rc = kind == 3   ? launch_apply_h_scatter(h, dtype, d_in, d_out, fa, stream)
+    const int rc = kind == 4   ? launch_apply_h_dense(h, dtype, d_in, d_out, fa, stream)
+                   : kind == 3 ? launch_apply_h_scatter(h, dtype, d_in, d_out, fa, stream)
                    : kind == 2 ? launch_apply_h_regtile(h, dtype, d_in, d_out, fa, stream)
                    : dtype == SYK_C128 ? launch_typed<double, 4>(h, d_in, d_out, fa, kind, stream)
                                        : launch_typed<float, 8>(h, d_in, d_out, fa, kind, stream);
@@ -435,7 +438,7 @@ int syk_set_lockstep(int epoch_len, int lag) {
 }
 
 int syk_set_apply_H_kernel(syk_ham* h, int kind) {
-    if (!h || kind < -1 || kind > 3) return SYK_EINVAL;
+    if (!h || kind < -1 || kind > 4) return SYK_EINVAL;
     h->forced_kernel = kind;
     return SYK_OK;
 }

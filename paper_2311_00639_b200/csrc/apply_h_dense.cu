@@ -1,0 +1,476 @@
+// a-2  apply_H, dense-table kernel: the gather form of Algorithm 1 for Hamiltonians with MANY terms
+// per X-mask (dense p = 1: T = 194 580 terms on D_x = 10 903 masks at N = 48, 17.8 terms per mask).
+//
+//     out[b] = sum_g in[b ^ x_g] * S_g(b),      S_g(b) = sum_{t in g} c_t (-1)^popcount(b & z_t)
+//
+// Here the vector traffic is negligible (a few hundred source tiles per output tile, all L2 hits) and the work is
+// the T sign-accumulates per amplitude: plain ALU.  Three things keep that cheap:
+//   * the thread owns R = 16 amplitudes  base | tid | r << 8  (r = index bits 8..11), so everything that depends on
+//     the term only (table read, popcount of the tile/thread part of the sign) is paid once per 16 amplitudes;
+//   * the r-dependence of the sign is a WALSH FUNCTION of r:  (-1)^popcount(r & zr),  zr = bits 8..11 of z.  So the
+//     terms of a group are first binned by zr -- one add per TERM into one of 16 registers (terms come sorted by
+//     bin, so the register is a compile-time index of an unrolled walk over the bins that occur) -- and
+//     S_g(r) for the 16 r is the Walsh-Hadamard transform of the bins: 64 adds per group instead of 16 per term;
+//   * c_t is exactly real or exactly imaginary (J s^4 times 1, -1, i, -i): two real bin arrays, no complex adds.
+// Then one complex multiply-add per (group, amplitude) with the source read from the staged tile.
+//
+// Source tiles (2^12 amplitudes: 64 / 32 KiB) come through the same cp.async.bulk ring as in the other tile kernels
+// (one producer lane, mbarriers); the table (a few MB, streamed once per output tile) is staged chunk by chunk in
+// shared memory by the consumers themselves, double buffered, so the inner loops read it with broadcast LDS (read
+// from global with warp-uniform addresses, each term cost an exposed L2 latency: 1120 ms per N = 48 matvec).
+// No atomics on data, one write per output: bitwise reproducible.  Fused Lanczos epilogue as in apply_h.cu.
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "device_utils.cuh"
+
+namespace syk {
+
+namespace {
+
+constexpr int kConsumerWarps = 8;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+constexpr int kThreads = kConsumerThreads + 32;
+constexpr int kR = 16;                             // amplitudes per thread
+constexpr int kTileLog2D = 12;                     // 256 threads x 16
+constexpr int kTile = 1 << kTileLog2D;
+constexpr int kMaxSlots = 6;
+constexpr int kSmemLimit = 232448;
+constexpr int kMiscBytes = 2 * kMaxSlots * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, reduction scratch, table buffers
+constexpr int kTableBufBytes = 2 * 512 * 16;
+
+// The table is ONE stream of 16-byte entries, cut into chunks of <= kChunkEntries entries that hold whole groups:
+//   group header : .x = tile-local X-mask, .y = number of terms that follow, .z = 1 real / 2 imaginary / 3 both,
+//                  .w = which of the 32 bins occur
+//   term         : .x = Z-mask, .y = bin = zr (bits 8..11 of z) + 16 if the coefficient is imaginary; terms of a
+//                  group are sorted by bin and bit 8 of .y marks the last term of a bin,
+//                  (.z, .w) = bits of the signed magnitude a (double) or .z = bits of (float) a
+// The consumers copy chunk k+1 into shared memory while they work on chunk k (double buffer), so every table read
+// in the inner loops is a broadcast LDS instead of a dependent global load.
+constexpr int kChunkEntries = 512;
+struct DenseLoad { uint32_t hi, c0, c1, pad; };    // source tile = tile ^ hi; chunks [c0, c1)
+struct DenseChunk { uint32_t e0, ne, pad0, pad1; };// entries [e0, e0 + ne)
+
+template <typename T>
+struct DnParams {
+    using C = typename Cx<T>::type;
+    const C* in;
+    C* out;
+    const C* prev;
+    LanczosScalars* sc;
+    int j;
+    int L;
+    int nslot;
+    const DenseLoad* loads;
+    const DenseChunk* chunks;
+    const uint4* entries;
+    int n_loads;
+    int n_chunks;
+};
+
+__device__ __forceinline__ void dn_fused_scalars(LanczosScalars* sc, int j, double* red, double& s_in, double& s_prev) {
+    double n2 = reduce_partials(sc->partial_nrm, sc->n_partial_nrm, red);
+    double nj = sqrt(n2);
+    if (blockIdx.x == 0 && threadIdx.x == 0) sc->nrm[j] = nj;
+    s_in = nj > 0.0 ? 1.0 / nj : 0.0;
+    s_prev = 0.0;
+    if (j > 1) {
+        double np = sc->nrm[j - 1];
+        s_prev = np > 0.0 ? nj / np : 0.0;
+    }
+}
+
+// in-place Walsh-Hadamard transform: s[r] = sum_z c[z] (-1)^popcount(r & z)
+template <typename T>
+__device__ __forceinline__ void wht16(T (&c)[kR]) {
+#pragma unroll
+    for (int h = 1; h < kR; h <<= 1) {
+#pragma unroll
+        for (int i = 0; i < kR; ++i) {
+            if ((i & h) == 0) {
+                const T a = c[i], b = c[i | h];
+                c[i] = a + b;
+                c[i | h] = a - b;
+            }
+        }
+    }
+}
+
+// bins B, B+1, ... of one group: for every bin that occurs, add its run of terms (closed by bit 8 of .y) to the register
+// that owns it.  `e` always holds entry `t`, loaded one step ahead.
+template <typename T, int B>
+__device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_t& t, uint4& e, uint32_t occ, uint32_t bt,
+                                          T (&cr)[kR], T (&ci)[kR]) {
+    if constexpr (B < 2 * kR) {
+        if (occ & (1u << B)) {
+            uint32_t last;
+            do {
+                const uint4 cur = e;
+                ++t;
+                e = ent[t < (uint32_t)kChunkEntries ? t : (uint32_t)kChunkEntries - 1u];
+                const uint32_t sgn = (uint32_t)__popc(bt & cur.x) << 31;
+                T a;
+                if constexpr (sizeof(T) == 8) a = __hiloint2double((int)(cur.w ^ sgn), (int)cur.z);
+                else a = __uint_as_float(cur.z ^ sgn);
+                if constexpr (B < kR) cr[B] += a;
+                else ci[B - kR] += a;
+                last = cur.y & 256u;
+            } while (!last);
+        }
+        walk_bins<T, B + 1>(ent, t, e, occ, bt, cr, ci);
+    }
+}
+
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnParams<T> p) {
+    using C = typename Cx<T>::type;
+    constexpr uint32_t TILE_BYTES = kTile * sizeof(C);
+    constexpr uint32_t kChunk = 16384;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    C* stages = reinterpret_cast<C*>(smem);
+    unsigned char* q = smem + (size_t)p.nslot * TILE_BYTES;
+    uint4* tbuf = reinterpret_cast<uint4*>(q);      // 2 x kChunkEntries table entries
+    q += 2 * kChunkEntries * sizeof(uint4);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(q);
+    q += 2 * kMaxSlots * 8;
+    double* red = reinterpret_cast<double*>(q);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kMaxSlots);
+    if (tid == 0) {
+        for (int s = 0; s < p.nslot; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, kConsumerWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    double s_in = 1.0, s_prev = 0.0;
+    if (FUSED) dn_fused_scalars(p.sc, p.j, red, s_in, s_prev);
+
+    const uint32_t n_tiles = 1u << (p.L - kTileLog2D);
+    const int nslot = p.nslot, n_loads = p.n_loads;
+    double dot = 0.0;
+
+    if (warp == kConsumerWarps) {
+        // ---------------- producer: one lane streams source tiles into the ring ----------------
+        if (lane == 0) {
+            int slot = 0;
+            uint32_t phase = 0;
+            const uint32_t stage0 = smem_u32(stages);
+            for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                for (int l = 0; l < n_loads; ++l) {
+                    const uint32_t hi = __ldg(&p.loads[l].hi);
+                    mbar_wait(bar_empty + 8 * slot, phase ^ 1u);
+                    mbar_arrive_expect_tx(bar_full + 8 * slot, TILE_BYTES);
+                    const unsigned char* src =
+                        reinterpret_cast<const unsigned char*>(p.in + ((uint64_t)(tile ^ hi) << kTileLog2D));
+                    const uint32_t dst = stage0 + (uint32_t)slot * TILE_BYTES;
+#pragma unroll
+                    for (uint32_t c = 0; c < TILE_BYTES; c += kChunk) bulk_load(dst + c, src + c, kChunk, bar_full + 8 * slot);
+                    if (++slot == nslot) {
+                        slot = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    } else {
+        // ---------------- consumers ----------------
+        int slot = 0;
+        uint32_t phase = 0;
+        // table stream: this thread's two entries of the chunk being prefetched
+        uint32_t ck = 0;                       // chunk whose copy sits in tbuf[ck & 1] after the next barrier
+        uint4 pre0, pre1;
+        auto fetch = [&](uint32_t c) {         // global -> registers (chunk c, wrapping around the table)
+            const DenseChunk ch = *reinterpret_cast<const DenseChunk*>(&p.chunks[c]);
+            const uint32_t i0 = (uint32_t)tid, i1 = (uint32_t)tid + kConsumerThreads;
+            pre0 = i0 < ch.ne ? __ldg(p.entries + ch.e0 + i0) : make_uint4(0, 0, 0, 0);
+            pre1 = i1 < ch.ne ? __ldg(p.entries + ch.e0 + i1) : make_uint4(0, 0, 0, 0);
+        };
+        auto stash = [&](uint32_t c) {         // registers -> shared buffer (c & 1)
+            uint4* dst = tbuf + (c & 1u) * kChunkEntries;
+            dst[tid] = pre0;
+            dst[tid + kConsumerThreads] = pre1;
+        };
+        fetch(0);
+        stash(0);
+        for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const uint32_t base = tile << kTileLog2D;
+            const uint32_t bt = base | (uint32_t)tid;
+            T ar[kR], ai[kR];
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                ar[r] = 0;
+                ai[r] = 0;
+            }
+            for (int l = 0; l < n_loads; ++l) {
+                const uint32_t c0 = __ldg(&p.loads[l].c0), c1 = __ldg(&p.loads[l].c1);
+                mbar_wait(bar_full + 8 * slot, phase);
+                const C* sp = stages + (size_t)slot * kTile;
+                for (uint32_t c = c0; c < c1; ++c, ++ck) {
+                    // chunk c is in tbuf[ck & 1] once every consumer has stashed it; the other buffer is free again
+                    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+                    const uint32_t cn = c + 1 == (uint32_t)p.n_chunks ? 0u : c + 1;
+                    fetch(cn);
+                    const uint32_t ne = __ldg(&p.chunks[c].ne);
+                    const uint4* ent = tbuf + (ck & 1u) * kChunkEntries;
+                    uint32_t i = 0;
+                    while (i < ne) {
+                        const uint4 gh = ent[i];               // group header
+                        const uint32_t i_end = i + 1 + gh.y;
+                        T cr[kR], ci[kR];
+#pragma unroll
+                        for (int r = 0; r < kR; ++r) {
+                            cr[r] = 0;
+                            ci[r] = 0;
+                        }
+                        // terms are sorted by bin; .w of the header says which bins occur, bit 8 of a term's .y closes
+                        // its bin.  The stream is read one entry ahead whatever the bin structure is.
+                        uint32_t t = i + 1;
+                        uint4 e = ent[t];
+                        walk_bins<T, 0>(ent, t, e, gh.w, bt, cr, ci);
+                        i = i_end;
+                        const C* pb = sp + ((uint32_t)tid ^ (gh.x & 255u));
+                        const uint32_t xr = gh.x >> 8;
+                        if (gh.z == 1u) {          // real coefficients only
+                            wht16(cr);
+#pragma unroll
+                            for (int r = 0; r < kR; ++r) {
+                                const C v = pb[((uint32_t)r ^ xr) << 8];
+                                ar[r] += cr[r] * v.x;
+                                ai[r] += cr[r] * v.y;
+                            }
+                        } else if (gh.z == 2u) {   // imaginary coefficients only
+                            wht16(ci);
+#pragma unroll
+                            for (int r = 0; r < kR; ++r) {
+                                const C v = pb[((uint32_t)r ^ xr) << 8];
+                                ar[r] -= ci[r] * v.y;
+                                ai[r] += ci[r] * v.x;
+                            }
+                        } else {
+                            wht16(cr);
+                            wht16(ci);
+#pragma unroll
+                            for (int r = 0; r < kR; ++r) {
+                                const C v = pb[((uint32_t)r ^ xr) << 8];
+                                ar[r] += cr[r] * v.x - ci[r] * v.y;
+                                ai[r] += cr[r] * v.y + ci[r] * v.x;
+                            }
+                        }
+                    }
+                    stash(ck + 1);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
+                if (++slot == nslot) {
+                    slot = 0;
+                    phase ^= 1u;
+                }
+            }
+            // epilogue (a tile takes milliseconds of arithmetic here: the latency of these global reads is nothing)
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const uint64_t b = (uint64_t)base + (uint32_t)tid + r * kConsumerThreads;
+                C o;
+                if (FUSED) {
+                    const C mine = __ldg(p.in + b);
+                    double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
+                    if (p.prev) {
+                        const C pv = p.prev[b];
+                        orr -= s_prev * (double)pv.x;
+                        oi -= s_prev * (double)pv.y;
+                    }
+                    o.x = (T)orr;
+                    o.y = (T)oi;
+                    dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+                } else {
+                    o.x = ar[r];
+                    o.y = ai[r];
+                }
+                p.out[b] = o;
+            }
+        }
+    }
+    if (FUSED) {
+        double s = block_sum(dot, red);
+        if (tid == 0) {
+            p.sc->partial_dot[blockIdx.x] = s;
+            if (blockIdx.x == 0) p.sc->n_partial_dot = gridDim.x;
+        }
+    }
+}
+
+// Host: the entry stream (group header + its terms, canonical order), cut into chunks of whole groups that do not
+// cross a load (run of equal x >> 12, ascending); uploaded once per handle and dtype.
+int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
+    const size_t ng = h->x.size();
+    std::vector<DenseLoad> loads;
+    std::vector<DenseChunk> chunks;
+    std::vector<uint4> entries;
+    entries.reserve(h->z.size() + ng);
+    for (size_t g = 0; g < ng; ++g) {
+        const uint32_t x = (uint32_t)h->x[g];
+        const uint32_t hi = x >> kTileLog2D;
+        const uint32_t nt = h->group_off[g + 1] - h->group_off[g];
+        if (nt + 1 > (uint32_t)kChunkEntries) return SYK_EINVAL;   // a group must fit one chunk (dense N <= 64: 497)
+        const bool new_load = loads.empty() || loads.back().hi != hi;
+        if (new_load) {
+            if (!loads.empty()) loads.back().c1 = (uint32_t)chunks.size();
+            loads.push_back(DenseLoad{hi, (uint32_t)chunks.size(), 0u, 0u});
+        }
+        if (new_load || chunks.back().ne + nt + 1 > (uint32_t)kChunkEntries)
+            chunks.push_back(DenseChunk{(uint32_t)entries.size(), 0u, 0u, 0u});
+        uint32_t flags = 0, occ = 0;
+        const size_t header_at = entries.size();
+        entries.push_back(make_uint4(x & (uint32_t)(kTile - 1), nt, 0u, 0u));
+        std::vector<uint4> run;
+        run.reserve(nt);
+        for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1]; ++t) {
+            const std::complex<double> c = h->c[t];
+            const bool imag = c.imag() != 0.0;
+            if (imag && c.real() != 0.0) return SYK_EINVAL;   // never for SYK strings
+            const double a = imag ? c.imag() : c.real();
+            const uint32_t z = (uint32_t)h->z[t];
+            uint4 e;
+            e.x = z;
+            e.y = ((z >> 8) & 15u) | (imag ? 16u : 0u);
+            if (dtype == SYK_C128) {
+                uint64_t bits;
+                std::memcpy(&bits, &a, 8);
+                e.z = (uint32_t)bits;
+                e.w = (uint32_t)(bits >> 32);
+            } else {
+                const float af = (float)a;   // R-C64: rounded once
+                uint32_t bits;
+                std::memcpy(&bits, &af, 4);
+                e.z = bits;
+                e.w = 0;
+            }
+            run.push_back(e);
+            flags |= imag ? 2u : 1u;
+            occ |= 1u << (e.y & 31u);
+        }
+        std::stable_sort(run.begin(), run.end(), [](const uint4& p, const uint4& q) { return (p.y & 31u) < (q.y & 31u); });
+        for (size_t i = 0; i < run.size(); ++i) {
+            if (i + 1 == run.size() || (run[i + 1].y & 31u) != (run[i].y & 31u)) run[i].y |= 256u;   // closes its bin
+            entries.push_back(run[i]);
+        }
+        entries[header_at].w = occ;
+        entries[header_at].z = flags;
+        chunks.back().ne += nt + 1;
+    }
+    if (!loads.empty()) loads.back().c1 = (uint32_t)chunks.size();
+    auto align = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t off_c = align(loads.size() * sizeof(DenseLoad));
+    const size_t off_e = off_c + align(chunks.size() * sizeof(DenseChunk));
+    const size_t total = off_e + align(entries.size() * sizeof(uint4)) + 256;
+    std::vector<unsigned char> host(total, 0);
+    std::memcpy(host.data(), loads.data(), loads.size() * sizeof(DenseLoad));
+    std::memcpy(host.data() + off_c, chunks.data(), chunks.size() * sizeof(DenseChunk));
+    std::memcpy(host.data() + off_e, entries.data(), entries.size() * sizeof(uint4));
+    int dev = 0;
+    SYK_CUDA(cudaGetDevice(&dev));
+    void* blob = nullptr;
+    SYK_CUDA(cudaMalloc(&blob, total));
+    cudaError_t e = cudaMemcpy(blob, host.data(), total, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(blob);
+        set_cuda_error(e, "cudaMemcpy(dense term tables)");
+        return SYK_ECUDA;
+    }
+    dc.blob = blob;
+    dc.device = dev;
+    dc.off_groups = off_c;
+    dc.off_terms = off_e;
+    dc.n_loads = (int)loads.size();
+    dc.n_chunks = (int)chunks.size();
+    return SYK_OK;
+}
+
+int get_dense_tables(const syk_ham* h, int dtype, const DenseCache** out) {
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    int dev = 0;
+    SYK_CUDA(cudaGetDevice(&dev));
+    if (!h->dn[k]) h->dn[k] = new (std::nothrow) DenseCache();
+    if (!h->dn[k]) return SYK_ENOMEM;
+    DenseCache& dc = *h->dn[k];
+    if (dc.blob && dc.device != dev) {
+        cudaFree(dc.blob);
+        dc = DenseCache();
+    }
+    if (!dc.blob) SYK_TRY(build_dense_tables(h, dtype, dc));
+    *out = &dc;
+    return SYK_OK;
+}
+
+template <typename T>
+int launch_dn(const syk_ham* h, const DenseCache& dc, const void* d_in, void* d_out, const FusedArgs& fa,
+              cudaStream_t stream) {
+    using C = typename Cx<T>::type;
+    constexpr size_t kTileBytes = (size_t)kTile * sizeof(C);
+    DnParams<T> p;
+    p.in = (const C*)d_in;
+    p.out = (C*)d_out;
+    p.prev = (const C*)fa.prev;
+    p.sc = fa.sc;
+    p.j = fa.j;
+    p.L = h->L;
+    p.nslot = (int)((kSmemLimit - kMiscBytes) / kTileBytes);
+    if (p.nslot > kMaxSlots) p.nslot = kMaxSlots;
+    p.loads = (const DenseLoad*)dc.blob;
+    p.chunks = (const DenseChunk*)((const unsigned char*)dc.blob + dc.off_groups);
+    p.entries = (const uint4*)((const unsigned char*)dc.blob + dc.off_terms);
+    p.n_loads = dc.n_loads;
+    p.n_chunks = dc.n_chunks;
+    const size_t smem = (size_t)p.nslot * kTileBytes + kMiscBytes;
+    const int sms = num_sms();
+    if (sms <= 0) return SYK_ECUDA;
+    const uint64_t n_tiles = 1ull << (h->L - kTileLog2D);
+    const int grid = (int)(n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms);
+    if (fa.sc) {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_dense_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_dense_kernel<T, true><<<grid, kThreads, smem, stream>>>(p);
+    } else {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_dense_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_dense_kernel<T, false><<<grid, kThreads, smem, stream>>>(p);
+    }
+    count_launch();
+    SYK_CUDA(cudaGetLastError());
+    return SYK_OK;
+}
+
+}  // namespace
+
+// Can the handle use the dense-table kernel?  Automatic choice: many terms per X-mask and at least one tile per SM.
+bool dense_kernel_ok(const syk_ham* h, bool forced) {
+    if (h->n_terms() == 0 || h->L < kTileLog2D) return false;
+    if (forced) return true;
+    return h->L >= kTileLog2D + 8 && h->n_terms() >= 4 * h->n_groups() && h->n_terms() > kRtMaxTerms;
+}
+
+int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                         cudaStream_t stream) {
+    const DenseCache* dc = nullptr;
+    SYK_TRY(get_dense_tables(h, dtype, &dc));
+    if (dtype == SYK_C128) return launch_dn<double>(h, *dc, d_in, d_out, fa, stream);
+    return launch_dn<float>(h, *dc, d_in, d_out, fa, stream);
+}
+
+void free_dense_tables(const syk_ham* h) {
+    for (int k = 0; k < 2; ++k) {
+        if (h->dn[k]) {
+            if (h->dn[k]->blob) cudaFree(h->dn[k]->blob);
+            delete h->dn[k];
+            h->dn[k] = nullptr;
+        }
+    }
+}
+
+}  // namespace syk

@@ -69,6 +69,13 @@ struct StCache {
     StTable tab;
     bool valid = false;
 };
+// Device tables of the dense-table kernel (apply_h_dense.cu): one allocation holding loads | groups | terms.
+struct DenseCache {
+    void* blob = nullptr;
+    int device = -1;
+    size_t off_groups = 0, off_terms = 0;   // byte offsets of the chunk list and of the entry stream
+    int n_loads = 0, n_chunks = 0;
+};
 }  // namespace syk
 
 struct syk_ham {
@@ -85,6 +92,7 @@ struct syk_ham {
     mutable syk::DeviceTables dev;             // created on first device use
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
     mutable syk::StCache* st[2] = {nullptr, nullptr};   // scatter-tile kernel tables per dtype (host, lazily built)
+    mutable syk::DenseCache* dn[2] = {nullptr, nullptr};   // dense-table kernel tables per dtype (device, lazily built)
     int64_t n_terms() const { return (int64_t)z.size(); }
     int64_t n_groups() const { return (int64_t)x.size(); }
 };
@@ -166,6 +174,12 @@ int launch_apply_h_scatter(const syk_ham* h, int dtype, const void* d_in, void* 
 int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
                         uint32_t* window_mask);
 void free_scatter_tables(const syk_ham* h);
+
+// dense-table kernel (apply_h_dense.cu)
+bool dense_kernel_ok(const syk_ham* h, bool forced);
+int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
+                         cudaStream_t stream);
+void free_dense_tables(const syk_ham* h);
 
 // apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

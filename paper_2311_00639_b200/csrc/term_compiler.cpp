@@ -164,6 +164,7 @@ void syk_free_hamiltonian(syk_ham* h) {
     syk::free_device_tables(h);
     syk::free_regtile_tables(h);
     syk::free_scatter_tables(h);
+    syk::free_dense_tables(h);
     delete h;
 }
 

@@ -69,6 +69,7 @@ APPLY_CASES = [
     # N, k (None = dense), gamma_norm
     (4, None, 0), (6, None, 1), (8, None, 0), (12, None, 0), (16, None, 0), (16, 4, 1),
     (20, 4, 0), (22, 8, 0), (24, 4, 0), (26, 2, 0), (28, 4, 1), (30, 8, 0), (32, 4, 0),
+    (24, None, 0), (28, None, 1),      # dense beyond the shared-memory table: generic and dense-table kernels
 ]
 
 
@@ -76,7 +77,7 @@ APPLY_CASES = [
 @pytest.mark.parametrize("N,k,gn", APPLY_CASES)
 def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
     """out = H.in against the oracle's sequential-gamma product (O5), every kernel the handle can use
-    (0 generic, 1 16 KiB-tile TMA, 2 register-tile TMA, 3 scatter-tile TMA)."""
+    (0 generic, 1 16 KiB-tile TMA, 2 register-tile TMA, 3 scatter-tile TMA, 4 dense-table)."""
     q, J = couplings(N, k, seed=1)
     D = 1 << (N // 2)
     v = inputs.gaussian_state(D, seed=100 + N, dtype=npdtype(dt))
@@ -84,11 +85,13 @@ def test_apply_H_vs_oracle(B, torch, N, k, gn, dt):
     h = B.syk_build_from_terms(N, q, J, gn)
     d_in = to_dev(torch, v)
     kinds = {0}
-    for want in (1, 2, 3):
+    for want in (1, 2, 3, 4):
         B.syk_set_apply_H_kernel(h, want)
         kinds.add(B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)))
-    if N >= 28:
-        assert kinds == {0, 1, 2, 3}
+    if N >= 28 and k is not None:
+        assert kinds == {0, 1, 2, 3, 4}
+    if N >= 24 and k is None:
+        assert kinds >= {0, 4}
     for kind in sorted(kinds):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
@@ -118,7 +121,7 @@ def test_apply_H_structured_masks(B, torch, qubits, dt):
     ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
     h = B.syk_build_from_terms(N, q, J)
     d_in = to_dev(torch, v)
-    for kind in (0, 1, 2, 3):
+    for kind in (0, 1, 2, 3, 4):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, B.dtype_code(d_in)) == kind
         d_out = torch.zeros(D, dtype=tdtype(torch, dt), device="cuda")
@@ -325,7 +328,7 @@ def test_fused_lanczos_every_kernel_kind(B, torch, dt):
     wk = work(torch, B.syk_krylov_workspace_bytes(h, code, {"krylov_dim": m}))
     d_psi = to_dev(torch, psi)
     tol = 1e-11 if dt == "c128" else 2e-5
-    for kind in (0, 1, 2, 3):
+    for kind in (0, 1, 2, 3, 4):
         B.syk_set_apply_H_kernel(h, kind)
         assert B.syk_apply_H_kernel_kind(h, code) == kind
         alpha, beta, st = B.syk_lanczos_run(h, d_psi, m, wk)
