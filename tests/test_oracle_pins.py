@@ -10,7 +10,7 @@ import os
 import numpy as np
 import pytest
 
-from oracle import alg1, evolve, green, hamiltonian, majorana, otoc, rng
+from oracle import alg1, evolve, green, hamiltonian, majorana, otoc, parity, rng
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -386,3 +386,56 @@ def test_P13_green_closed_forms(gamma_norm):
                    for k in range(300)], axis=0)
     assert np.allclose(est, Gtr, atol=0.12 * abs(Gtr[0]))
     assert abs(Gtr[0].imag) < 1e-13 and Gtr[0].real > 0
+
+
+# ---------------------------------------------------------------- P14 parity blocks
+@pytest.mark.parametrize("gamma_norm", [0, 1])
+def test_P14_parity_blocks(gamma_norm):
+    """(i) spectrum(H) = spectrum(H_UU) u spectrum(H_DD); (ii) the paper's statements about the last two gammas hold
+    for the Jordan-Wigner blocks too: the block of gamma_{N-1} is -i s (+1 | -1) times the identity with opposite signs
+    for the two directions (g^{UD} = -g^{DU} = -i 1), the block of gamma_{N-2} is the same diagonal sign
+    matrix in both directions; (iii) F(t) and G(t) of the full space are the sums of their two block
+    terms ("+ swap UD"), for the sector components of the same psi; (iv) (H v) restricted = H_ss
+    v_s, (gamma v) restricted = block times v restricted."""
+    N, L = 10, 5
+    s = majorana.gamma_scale(gamma_norm)
+    q, J, _ = rng.sample_couplings(N, 0.4, seed=11, realization=0)
+    H = hamiltonian.dense_hamiltonian(N, q, J, gamma_norm)
+    blocks = [parity.block_hamiltonian(N, q, J, sec, gamma_norm) for sec in (0, 1)]
+    w = np.sort(np.concatenate([np.linalg.eigvalsh(b) for b in blocks]))
+    assert np.allclose(w, np.linalg.eigvalsh(H), atol=1e-12)
+    # (ii)
+    gl0, gl1 = parity.block_gamma(N, N - 1, 0, gamma_norm), parity.block_gamma(N, N - 1, 1, gamma_norm)
+    eye = np.eye(1 << (L - 1))
+    assert np.allclose(gl0, -gl1, atol=0) and np.allclose(np.abs(gl0), s * eye, atol=1e-15)
+    assert np.allclose(gl0, gl0[0, 0] * eye, atol=0) and abs(gl0[0, 0].real) == 0.0 and abs(gl0[0, 0].imag) == s
+    gm0, gm1 = parity.block_gamma(N, N - 2, 0, gamma_norm), parity.block_gamma(N, N - 2, 1, gamma_norm)
+    assert np.array_equal(gm0, gm1) and np.allclose(np.abs(gm0), s * eye, atol=1e-15)
+    assert np.count_nonzero(gm0 - np.diag(np.diag(gm0))) == 0 and set(np.unique(np.diag(gm0).real / s)) == {-1.0, 1.0}
+    # (iv)
+    v = _random_state(1 << L, 4)
+    for sec in (0, 1):
+        vs = parity.restrict(v, L, sec)
+        full = parity.embed(vs, L, sec)
+        assert np.allclose(parity.restrict(H @ full, L, sec), blocks[sec] @ vs, atol=1e-14)
+        assert np.allclose(parity.restrict(H @ full, L, 1 - sec), 0, atol=0)
+        for n in (0, 3, N - 2, N - 1):
+            gv = hamiltonian.apply_gamma(N, n, full, gamma_norm)
+            assert np.allclose(parity.restrict(gv, L, 1 - sec), parity.block_gamma(N, n, 1 - sec, gamma_norm) @ vs, atol=1e-15)
+            assert np.allclose(parity.restrict(gv, L, sec), 0, atol=0)
+    # (iii)
+    prop = evolve.ExactPropagator(N, q, J, gamma_norm)
+    props = [parity.BlockPropagator(N, q, J, sec, gamma_norm) for sec in (0, 1)]
+    t_grid = [0.0, 0.8, 2.1]
+    F = otoc.otoc_same_psi(prop, N, N - 1, N - 2, 1.5, t_grid, v, gamma_norm)
+    Fb = sum(parity.otoc_block_same_psi(props, N, N - 1, N - 2, 1.5, t_grid, parity.restrict(v, L, sec), sec, gamma_norm)
+             for sec in (0, 1))
+    assert np.allclose(F, Fb, atol=1e-13)
+    F2 = otoc.otoc_same_psi(prop, N, 2, 5, 1.5, t_grid, v, gamma_norm)
+    F2b = sum(parity.otoc_block_same_psi(props, N, 2, 5, 1.5, t_grid, parity.restrict(v, L, sec), sec, gamma_norm)
+              for sec in (0, 1))
+    assert np.allclose(F2, F2b, atol=1e-13)
+    G = green.green_same_psi(prop, N, N - 1, 1.5, t_grid, v, gamma_norm)
+    Gb = sum(parity.green_block_same_psi(props, N, N - 1, 1.5, t_grid, parity.restrict(v, L, sec), sec, gamma_norm)
+             for sec in (0, 1))
+    assert np.allclose(G, Gb, atol=1e-13)
