@@ -166,6 +166,29 @@ int syk_green(const syk_ham* h, int dtype, int n, double beta, const double* t_g
               double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
               void* stream);
 
+/* ------------------------------------------------------------------------------------------------------------
+ * Parity blocks, PAPER.md:220-247 (reading R-BLOCK of DESIGN.md).  H commutes with the fermion
+ * parity Z^{(x)L}: H = H_UU (+) H_DD with sector 0 = even, 1 = odd popcount of the basis index.  A block acts on
+ * D/2 = 2^(L-1) amplitudes: reduced index b' = low L-1 bits of b, the dropped top bit is parity(b') xor sector.
+ *
+ * syk_build_parity_block: the block of a FULL handle (N >= 6) as a handle of its own on L-1 qubits -- every call that
+ * takes a handle (syk_apply_H, syk_lanczos_run, syk_krylov_evolve, work-space queries, ...) works on it with vectors
+ * of D/2 amplitudes; syk_ham_info reports N-2 and D/2; quartet_of_term / J_of_term still name the original quartets.
+ * syk_apply_gamma_block: gamma_n of the full space (0 <= n < N) as a map from sector 1-sector_out to sector_out on
+ * reduced vectors (in place allowed); gamma_{N-2} is a diagonal sign and gamma_{N-1} = -/+ i s 1: no gather
+ * (PAPER.md:238-242).  syk_otoc_block / syk_green_block: the term of F(t) / G(t) (PAPER.md:232 / 220) that starts
+ * from the reduced state d_psi in `sector`; the full-space value for psi = psi_U (+) psi_D is the sum of the two
+ * sectors' results.  Same work space (syk_otoc_workspace_bytes of either block), ownership and errors as syk_otoc. */
+int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out);
+int syk_apply_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
+                          void* stream);
+int syk_otoc_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int dtype, int i_W, int j_V, double beta,
+                   const double* t_grid, int n_t, void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work,
+                   size_t work_bytes, syk_stats* stats, void* stream);
+int syk_green_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int dtype, int n, double beta,
+                    const double* t_grid, int n_t, void* d_psi, double* G_out, const syk_krylov_opts* opts, void* d_work,
+                    size_t work_bytes, syk_stats* stats, void* stream);
+
 /* Batched over disorder realizations: realization r uses hams[r], state d_psi + r*batch_stride elements, and
  * writes F_out[r][n_t][2].  One work space is shared (realizations run back to back on `stream`). */
 int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,

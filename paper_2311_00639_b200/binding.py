@@ -71,6 +71,12 @@ _SIGNATURES = {
     "syk_otoc_workspace_bytes": (_i, [_vp, _i, _P(syk_krylov_opts), _P(_sz)]),
     "syk_otoc": (_i, [_vp, _i, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
     "syk_green": (_i, [_vp, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
+    "syk_build_parity_block": (_i, [_vp, _i, _P(_vp)]),
+    "syk_apply_gamma_block": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp]),
+    "syk_otoc_block": (_i, [_vp, _vp, _i, _i, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats),
+                            _vp]),
+    "syk_green_block": (_i, [_vp, _vp, _i, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats),
+                             _vp]),
     "syk_otoc_batched": (_i, [_P(_vp), _i, _i, _i, _i, _d, _vp, _i, _vp, _i64, _vp, _P(syk_krylov_opts), _vp, _sz,
                               _P(syk_stats), _vp]),
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
@@ -331,6 +337,42 @@ def syk_green(h, n, beta, t_grid, d_psi, d_work, opts=None, stream=None):
     _check(_lib.syk_green(_h(h), dtype_code(d_psi), int(n), float(beta), t.ctypes.data, len(t), _dptr(d_psi),
                           G.ctypes.data, _opts(opts), _dptr(d_work), d_work.numel() * d_work.element_size(),
                           ctypes.byref(st), _stream(stream)), "syk_green")
+    return G[:, 0] + 1j * G[:, 1], st.as_dict()
+
+
+def syk_build_parity_block(h, sector):
+    out = ctypes.c_void_p()
+    _check(_lib.syk_build_parity_block(_h(h), int(sector), ctypes.byref(out)), "syk_build_parity_block")
+    return Hamiltonian(out.value)
+
+
+def syk_apply_gamma_block(N, n, sector_out, d_in, d_out, gamma_norm=SYK_GAMMA_PAULI, stream=None):
+    _check(_lib.syk_apply_gamma_block(int(N), int(n), int(gamma_norm), int(sector_out), dtype_code(d_in), _dptr(d_in),
+                                      _dptr(d_out), _stream(stream)), "syk_apply_gamma_block")
+    return d_out
+
+
+def syk_otoc_block(h_even, h_odd, sector, i_W, j_V, beta, t_grid, d_psi, d_work, opts=None, stream=None):
+    """One parity sector's term of F(t); d_psi is the reduced state (destroyed)."""
+    t = np.ascontiguousarray(t_grid, dtype=np.float64)
+    F = np.zeros((len(t), 2), dtype=np.float64)
+    st = syk_stats()
+    _check(_lib.syk_otoc_block(_h(h_even), _h(h_odd), int(sector), dtype_code(d_psi), int(i_W), int(j_V), float(beta),
+                               t.ctypes.data, len(t), _dptr(d_psi), F.ctypes.data, _opts(opts), _dptr(d_work),
+                               d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
+           "syk_otoc_block")
+    return F[:, 0] + 1j * F[:, 1], st.as_dict()
+
+
+def syk_green_block(h_even, h_odd, sector, n, beta, t_grid, d_psi, d_work, opts=None, stream=None):
+    """One parity sector's term of G(t); d_psi is the reduced state (destroyed)."""
+    t = np.ascontiguousarray(t_grid, dtype=np.float64)
+    G = np.zeros((len(t), 2), dtype=np.float64)
+    st = syk_stats()
+    _check(_lib.syk_green_block(_h(h_even), _h(h_odd), int(sector), dtype_code(d_psi), int(n), float(beta),
+                                t.ctypes.data, len(t), _dptr(d_psi), G.ctypes.data, _opts(opts), _dptr(d_work),
+                                d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
+           "syk_green_block")
     return G[:, 0] + 1j * G[:, 1], st.as_dict()
 
 

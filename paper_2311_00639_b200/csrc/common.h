@@ -88,6 +88,8 @@ struct syk_ham {
     std::vector<std::complex<double>> c;       // [n_terms]
     std::vector<int32_t> quartet;              // [n_terms*4]
     std::vector<double> J;                     // [n_terms]
+    int block_of_N = 0;                        // parity block (syk_build_parity_block): N of the full Hamiltonian, else 0
+    int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable syk::DeviceTables dev;             // created on first device use
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
@@ -203,6 +205,9 @@ int launch_cdot(int dtype, uint64_t D, const void* d_a, const void* d_b, Lanczos
 int fetch_cdot(LanczosScalars* sc, double* re_im, cudaStream_t stream);   // host sum of the partials; synchronises
 int launch_normalise(int dtype, uint64_t D, void* d_v, LanczosScalars* sc, cudaStream_t stream);
 int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, cudaStream_t stream);
+// gamma_n of the FULL space (N Majoranas) between parity blocks on N/2-1 qubits; the result lies in sector_out
+int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
+                       cudaStream_t stream);
 int launch_random_fill(int N, uint64_t seed, uint32_t realization, int dtype, void* d_psi, LanczosScalars* sc,
                        cudaStream_t stream);
 int apply_h_kernel_kind(const syk_ham* h, int dtype);

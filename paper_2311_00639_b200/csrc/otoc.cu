@@ -14,9 +14,26 @@
 
 namespace syk {
 
-static int otoc_one(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
+// The space the pipelines run in: the full 2^(N/2) space (sector < 0: one Hamiltonian, JW gammas) or parity blocks
+// on N/2-1 qubits (R-BLOCK: hs[0] / hs[1] = even / odd block, a state in sector s evolves under
+// hs[s] and every gamma moves it to the other sector).
+struct Space {
+    const syk_ham* hs[2];
+    int sector;    // sector of the initial state; < 0 = full space
+    int N;         // Majoranas of the FULL Hamiltonian
+    int gamma_norm;
+    const syk_ham* ham(int sec) const { return sector < 0 ? hs[0] : hs[sec]; }
+    int gamma(int n, int sec_out, int dtype, const void* in, void* out, cudaStream_t st) const {
+        return sector < 0 ? launch_gamma(N, n, gamma_norm, dtype, in, out, st)
+                          : launch_gamma_block(N, n, gamma_norm, sec_out, dtype, in, out, st);
+    }
+};
+
+static int otoc_one(const Space& sp, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
                     void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
                     syk_stats* stats, cudaStream_t st) {
+    const syk_ham* h = sp.hs[0];
+    const int s0 = sp.sector < 0 ? 0 : sp.sector, s1 = sp.sector < 0 ? 0 : 1 - sp.sector;
     const uint64_t D = 1ull << h->L;
     const size_t vbytes = (size_t)D * elem_bytes(dtype);
     size_t kbytes = 0;
@@ -27,32 +44,32 @@ static int otoc_one(const syk_ham* h, int dtype, int i_W, int j_V, double beta, 
     char* r = phi + vbytes;
     char* kwork = r + vbytes;
     LanczosScalars* sc = (LanczosScalars*)kwork;   // the Krylov header doubles as reduction scratch between evolutions
-    const int N = h->N, gn = h->gamma_norm;
     int rc_soft = SYK_OK;
-    auto evolve = [&](void* v, double tre, double tim) -> int {
-        int rc = krylov_evolve_impl(h, dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+    auto evolve = [&](void* v, int sec, double tre, double tim) -> int {
+        int rc = krylov_evolve_impl(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
         if (rc == SYK_ENOCONV) {
             rc_soft = rc;
             return SYK_OK;
         }
         return rc;
     };
-    SYK_TRY(evolve(l, 0.0, -beta / 8.0));
-    SYK_TRY(launch_gamma(N, j_V, gn, dtype, l, phi, st));
-    SYK_TRY(evolve(phi, 0.0, -beta / 4.0));
+    // l lives in sector s0, phi in s1; r goes s0 -> s1 -> s0
+    SYK_TRY(evolve(l, s0, 0.0, -beta / 8.0));
+    SYK_TRY(sp.gamma(j_V, s1, dtype, l, phi, st));
+    SYK_TRY(evolve(phi, s1, 0.0, -beta / 4.0));
     double t_prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         const double t = t_grid[k], dt = t - t_prev;
         if (dt > 0.0) {
-            SYK_TRY(evolve(l, dt, 0.0));
-            SYK_TRY(evolve(phi, dt, 0.0));
+            SYK_TRY(evolve(l, s0, dt, 0.0));
+            SYK_TRY(evolve(phi, s1, dt, 0.0));
         }
         t_prev = t;
-        SYK_TRY(launch_gamma(N, i_W, gn, dtype, phi, r, st));
-        SYK_TRY(evolve(r, -t, -beta / 4.0));
-        SYK_TRY(launch_gamma(N, j_V, gn, dtype, r, r, st));
-        SYK_TRY(evolve(r, t, -beta / 4.0));
-        SYK_TRY(launch_gamma(N, i_W, gn, dtype, r, r, st));
+        SYK_TRY(sp.gamma(i_W, s0, dtype, phi, r, st));
+        SYK_TRY(evolve(r, s0, -t, -beta / 4.0));
+        SYK_TRY(sp.gamma(j_V, s1, dtype, r, r, st));
+        SYK_TRY(evolve(r, s1, t, -beta / 4.0));
+        SYK_TRY(sp.gamma(i_W, s0, dtype, r, r, st));
         SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
         SYK_TRY(fetch_cdot(sc, F_out + 2 * k, st));
     }
@@ -63,9 +80,11 @@ static int otoc_one(const syk_ham* h, int dtype, int i_W, int j_V, double beta, 
 //   G(t) = <psi| e^{(it-b/2)H} g_n e^{-iHt} g_n e^{-bH/2} |psi> = < E(t) l0 | g_n E(t) g_n l0 >,  l0 = E(-ib/2) psi,
 // so both sides advance incrementally along the t grid: two evolutions by dt per grid point, one gamma insertion,
 // one inner product.  Resident: l (in psi's buffer), phi, r + Krylov work.
-static int green_one(const syk_ham* h, int dtype, int n, double beta, const double* t_grid, int n_t, void* d_psi,
+static int green_one(const Space& sp, int dtype, int n, double beta, const double* t_grid, int n_t, void* d_psi,
                      double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
                      cudaStream_t st) {
+    const syk_ham* h = sp.hs[0];
+    const int s0 = sp.sector < 0 ? 0 : sp.sector, s1 = sp.sector < 0 ? 0 : 1 - sp.sector;
     const uint64_t D = 1ull << h->L;
     const size_t vbytes = (size_t)D * elem_bytes(dtype);
     size_t kbytes = 0;
@@ -76,31 +95,38 @@ static int green_one(const syk_ham* h, int dtype, int n, double beta, const doub
     char* r = phi + vbytes;
     char* kwork = r + vbytes;
     LanczosScalars* sc = (LanczosScalars*)kwork;
-    const int N = h->N, gn = h->gamma_norm;
     int rc_soft = SYK_OK;
-    auto evolve = [&](void* v, double tre, double tim) -> int {
-        int rc = krylov_evolve_impl(h, dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+    auto evolve = [&](void* v, int sec, double tre, double tim) -> int {
+        int rc = krylov_evolve_impl(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
         if (rc == SYK_ENOCONV) {
             rc_soft = rc;
             return SYK_OK;
         }
         return rc;
     };
-    SYK_TRY(evolve(l, 0.0, -beta / 2.0));
-    SYK_TRY(launch_gamma(N, n, gn, dtype, l, phi, st));
+    SYK_TRY(evolve(l, s0, 0.0, -beta / 2.0));
+    SYK_TRY(sp.gamma(n, s1, dtype, l, phi, st));
     double t_prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         const double dt = t_grid[k] - t_prev;
         if (dt > 0.0) {
-            SYK_TRY(evolve(l, dt, 0.0));
-            SYK_TRY(evolve(phi, dt, 0.0));
+            SYK_TRY(evolve(l, s0, dt, 0.0));
+            SYK_TRY(evolve(phi, s1, dt, 0.0));
         }
         t_prev = t_grid[k];
-        SYK_TRY(launch_gamma(N, n, gn, dtype, phi, r, st));
+        SYK_TRY(sp.gamma(n, s0, dtype, phi, r, st));
         SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
         SYK_TRY(fetch_cdot(sc, G_out + 2 * k, st));
     }
     return rc_soft;
+}
+
+static Space full_space(const syk_ham* h) { return Space{{h, h}, -1, h->N, h->gamma_norm}; }
+
+// the two blocks of one Hamiltonian: same N, same normalisation, sectors 0 and 1
+static bool blocks_ok(const syk_ham* he, const syk_ham* ho, int sector) {
+    return he && ho && (sector == 0 || sector == 1) && he->block_of_N >= 6 && he->block_of_N == ho->block_of_N &&
+           he->sector == 0 && ho->sector == 1 && he->gamma_norm == ho->gamma_norm;
 }
 
 static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
@@ -108,7 +134,8 @@ static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double b
     if (!h || (dtype != SYK_C64 && dtype != SYK_C128) || !d_psi || !d_work || n_t < 0 || (n_t > 0 && (!t_grid || !F_out)))
         return false;
     if (((uintptr_t)d_psi & 15) || ((uintptr_t)d_work & 15)) return false;
-    if (i_W < 0 || i_W >= h->N || j_V < 0 || j_V >= h->N || i_W == j_V || !(beta >= 0.0)) return false;
+    const int N = h->block_of_N ? h->block_of_N : h->N;   // operator indices refer to the full Hamiltonian
+    if (i_W < 0 || i_W >= N || j_V < 0 || j_V >= N || i_W == j_V || !(beta >= 0.0)) return false;
     double prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         if (!(t_grid[k] >= prev)) return false;
@@ -131,9 +158,10 @@ int syk_otoc_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts*
 int syk_otoc(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t, void* d_psi,
              double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
              void* stream) {
-    if (!syk::otoc_args_ok(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, d_work)) return SYK_EINVAL;
+    if (!syk::otoc_args_ok(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, d_work) || h->block_of_N)
+        return SYK_EINVAL;
     if (stats) *stats = syk_stats{};
-    return syk::otoc_one(h, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, opts, d_work, work_bytes, stats,
+    return syk::otoc_one(syk::full_space(h), dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, opts, d_work, work_bytes, stats,
                          (cudaStream_t)stream);
 }
 
@@ -141,10 +169,33 @@ int syk_green(const syk_ham* h, int dtype, int n, double beta, const double* t_g
               double* G_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
               void* stream) {
     // same argument rules as syk_otoc with a single operator index
-    if (!h || n < 0 || n >= h->N) return SYK_EINVAL;
+    if (!h || n < 0 || n >= h->N || h->block_of_N) return SYK_EINVAL;
     if (!syk::otoc_args_ok(h, dtype, n, n == 0 ? 1 : 0, beta, t_grid, n_t, d_psi, G_out, d_work)) return SYK_EINVAL;
     if (stats) *stats = syk_stats{};
-    return syk::green_one(h, dtype, n, beta, t_grid, n_t, d_psi, G_out, opts, d_work, work_bytes, stats,
+    return syk::green_one(syk::full_space(h), dtype, n, beta, t_grid, n_t, d_psi, G_out, opts, d_work, work_bytes, stats,
+                          (cudaStream_t)stream);
+}
+
+// Parity-block forms (R-BLOCK): one of the two terms of F / G, for a reduced state in `sector`.
+int syk_otoc_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int dtype, int i_W, int j_V, double beta,
+                   const double* t_grid, int n_t, void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work,
+                   size_t work_bytes, syk_stats* stats, void* stream) {
+    if (!syk::blocks_ok(h_even, h_odd, sector)) return SYK_EINVAL;
+    if (!syk::otoc_args_ok(h_even, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, d_work)) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    const syk::Space sp{{h_even, h_odd}, sector, h_even->block_of_N, h_even->gamma_norm};
+    return syk::otoc_one(sp, dtype, i_W, j_V, beta, t_grid, n_t, d_psi, F_out, opts, d_work, work_bytes, stats,
+                         (cudaStream_t)stream);
+}
+
+int syk_green_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int dtype, int n, double beta,
+                    const double* t_grid, int n_t, void* d_psi, double* G_out, const syk_krylov_opts* opts, void* d_work,
+                    size_t work_bytes, syk_stats* stats, void* stream) {
+    if (!syk::blocks_ok(h_even, h_odd, sector) || n < 0 || n >= h_even->block_of_N) return SYK_EINVAL;
+    if (!syk::otoc_args_ok(h_even, dtype, n, n == 0 ? 1 : 0, beta, t_grid, n_t, d_psi, G_out, d_work)) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    const syk::Space sp{{h_even, h_odd}, sector, h_even->block_of_N, h_even->gamma_norm};
+    return syk::green_one(sp, dtype, n, beta, t_grid, n_t, d_psi, G_out, opts, d_work, work_bytes, stats,
                           (cudaStream_t)stream);
 }
 
@@ -157,8 +208,9 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
     for (int r = 0; r < n_batch; ++r) {
         if (!hams[r] || hams[r]->N != hams[0]->N || batch_stride < ((int64_t)1 << hams[r]->L)) return SYK_EINVAL;
         char* psi = (char*)d_psi + (size_t)r * (size_t)batch_stride * syk::elem_bytes(dtype);
-        if (!syk::otoc_args_ok(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out, d_work)) return SYK_EINVAL;
-        int rc = syk::otoc_one(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out + (size_t)r * 2 * n_t, opts,
+        if (!syk::otoc_args_ok(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out, d_work) || hams[r]->block_of_N)
+            return SYK_EINVAL;
+        int rc = syk::otoc_one(syk::full_space(hams[r]), dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out + (size_t)r * 2 * n_t, opts,
                                d_work, work_bytes, stats, (cudaStream_t)stream);
         if (rc == SYK_ENOCONV) rc_soft = rc;
         else if (rc != SYK_OK) return rc;

@@ -159,6 +159,38 @@ int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets, const 
     return compile(N, gamma_norm, raw, out);
 }
 
+int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out) {
+    if (!h || !out || (sector != 0 && sector != 1) || h->block_of_N != 0 || h->N < 6) return SYK_EINVAL;
+    *out = nullptr;
+    const int L = h->L;
+    const uint64_t low = (1ull << (L - 1)) - 1;
+    std::vector<RawTerm> raw;
+    try {
+        raw.reserve(h->z.size());
+        for (size_t g = 0; g < h->x.size(); ++g)
+            for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1]; ++t) {
+                // c Z^z X^x restricted to the sector (R-BLOCK): the dropped top bit of the output index is
+                // parity(b') xor sector, so a Z on it contributes (-1)^sector and complements the low Z-mask
+                const bool z_top = (h->z[t] >> (L - 1)) & 1ull;
+                RawTerm r;
+                r.x = h->x[g] & low;
+                r.z = z_top ? (~h->z[t]) & low : h->z[t] & low;
+                r.c = (z_top && sector) ? -h->c[t] : h->c[t];
+                for (int k = 0; k < 4; ++k) r.q[k] = h->quartet[4 * (size_t)t + k];
+                r.J = h->J[t];
+                raw.push_back(r);
+            }
+    } catch (const std::bad_alloc&) {
+        return SYK_ENOMEM;
+    }
+    int rc = compile(h->N - 2, h->gamma_norm, raw, out);
+    if (rc == SYK_OK) {
+        (*out)->block_of_N = h->N;
+        (*out)->sector = sector;
+    }
+    return rc;
+}
+
 void syk_free_hamiltonian(syk_ham* h) {
     if (!h) return;
     syk::free_device_tables(h);

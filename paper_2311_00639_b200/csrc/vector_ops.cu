@@ -293,6 +293,27 @@ __global__ void __launch_bounds__(kThreads) gamma_kernel(const typename Cx<T>::t
     }
 }
 
+// Blocks of the two gammas of the dropped top qubit between parity sectors (R-BLOCK): no gather.
+//   mode 0: gamma_{N-2}: out[b'] = s (-1)^popcount(b') in[b']        mode 1: gamma_{N-1}: out[b'] = -i s sigma in[b']
+template <typename T>
+__global__ void __launch_bounds__(kThreads) gamma_top_kernel(const typename Cx<T>::type* in, typename Cx<T>::type* out,
+                                                             uint64_t n, int mode, T s_sigma) {
+    using C = typename Cx<T>::type;
+    GRID_STRIDE(b, n) {
+        const C v = in[b];
+        C o;
+        if (mode == 0) {
+            const T s = (__popc((uint32_t)b) & 1) ? -s_sigma : s_sigma;
+            o.x = s * v.x;
+            o.y = s * v.y;
+        } else {   // times -i: (x, y) -> (y, -x)
+            o.x = s_sigma * v.y;
+            o.y = -s_sigma * v.x;
+        }
+        out[b] = o;
+    }
+}
+
 #define DISPATCH(dtype, CALL_D, CALL_F) \
     do {                                \
         if ((dtype) == SYK_C128) {      \
@@ -396,6 +417,19 @@ int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* in, void* 
     return SYK_OK;
 }
 
+int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* in, void* out,
+                       cudaStream_t st) {
+    if (n < N - 2) return launch_gamma(N - 2, n, gamma_norm, dtype, in, out, st);   // string lives on the kept qubits
+    const uint64_t Dr = 1ull << (N / 2 - 1);
+    const int g = grid_for(Dr);
+    double s = gamma_norm == SYK_GAMMA_HALF ? 0.70710678118654752440 : 1.0;
+    const int mode = n - (N - 2);
+    if (mode == 1 && sector_out) s = -s;
+    DISPATCH(dtype, (gamma_top_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, Dr, mode, s)),
+             (gamma_top_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, Dr, mode, (float)s)));
+    return SYK_OK;
+}
+
 // Sum of the complex partials on the host (fixed order); synchronises the stream.
 int fetch_cdot(LanczosScalars* sc, double* re_im, cudaStream_t st) {
     static thread_local std::vector<double2> host;
@@ -425,6 +459,15 @@ size_t syk_reduce_scratch_bytes(void) { return (sizeof(syk::LanczosScalars) + 40
 static bool ok_vec(int N, int dtype, const void* p) {
     return N >= 4 && N <= 64 && (N % 2) == 0 && (dtype == SYK_C64 || dtype == SYK_C128) && p &&
            ((uintptr_t)p & 15) == 0;
+}
+
+int syk_apply_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
+                          void* stream) {
+    if (N < 6 || N > 64 || (N & 1) || n < 0 || n >= N || (dtype != SYK_C64 && dtype != SYK_C128) || !d_in || !d_out ||
+        (gamma_norm != SYK_GAMMA_PAULI && gamma_norm != SYK_GAMMA_HALF) || (sector_out != 0 && sector_out != 1))
+        return SYK_EINVAL;
+    if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return SYK_EINVAL;
+    return syk::launch_gamma_block(N, n, gamma_norm, sector_out, dtype, d_in, d_out, (cudaStream_t)stream);
 }
 
 int syk_apply_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, void* stream) {

@@ -598,3 +598,81 @@ def test_green_closed_form_and_errors(B, torch):
             B.syk_green(h, bad.get("n", 3), bad.get("beta", 1.0), bad.get("t", [0.0]), to_dev(torch, psi), wk, o)
     with pytest.raises(B.SykError):
         B.syk_green(h, 3, 1.0, [0.0], to_dev(torch, psi), work(torch, 1024), o)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-1 parity blocks (DESIGN.md R-BLOCK)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_parity_block_apply_H_and_gamma(B, torch, dt):
+    """apply_H on a block handle = oracle block matrix; gamma blocks (all n, both directions) = oracle blocks
+    selected from the Kronecker matrices; large enough for the tile kernels (N=28 -> 2^13 amplitudes per block)."""
+    from oracle import parity as opar
+    for N, k in ((12, None), (28, 4)):
+        L = N // 2
+        q, J = couplings(N, k, seed=6)
+        h = B.syk_build_from_terms(N, q, J)
+        v = inputs.gaussian_state(1 << L, 55, npdtype(dt))
+        for sector in (0, 1):
+            hb = B.syk_build_parity_block(h, sector)
+            vs = opar.restrict(v, L, sector)
+            full = opar.embed(vs.astype(np.complex128), L, sector)
+            ref = opar.restrict(ohm.matvec_sequential(N, q, J, full), L, sector)
+            d_out = torch.empty(1 << (L - 1), dtype=tdtype(torch, dt), device="cuda")
+            B.syk_apply_H(hb, to_dev(torch, vs), d_out)
+            assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt], (N, sector)
+            for n in sorted({0, 1, 2, 7, N - 3, N - 2, N - 1}):
+                gref = opar.restrict(ohm.apply_gamma(N, n, full), L, 1 - sector)
+                d_g = torch.empty_like(d_out)
+                B.syk_apply_gamma_block(N, n, 1 - sector, to_dev(torch, vs), d_g)
+                assert relerr(d_g.cpu().numpy(), gref) <= 1e-15 if dt == "c128" else 1e-7, (N, n, sector)
+                d_ip = to_dev(torch, vs)
+                B.syk_apply_gamma_block(N, n, 1 - sector, d_ip, d_ip)           # in place
+                assert torch.equal(torch.view_as_real(d_ip), torch.view_as_real(d_g))
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_parity_block_otoc_and_green(B, torch, dt):
+    """Block OTOC / Green function against the oracle's block pipeline (dense block propagators and gamma blocks),
+    and the sum over the two sectors against the full-space library calls ("+ swap UD")."""
+    from oracle import parity as opar
+    N, L = 16, 8
+    q, J = couplings(N, None, seed=0)
+    h = B.syk_build_from_terms(N, q, J)
+    he, ho = B.syk_build_parity_block(h, 0), B.syk_build_parity_block(h, 1)
+    props = [opar.BlockPropagator(N, q, J, s) for s in (0, 1)]
+    psi = inputs.gaussian_state(1 << L, 8, npdtype(dt))
+    t_grid = np.array([0.0, 0.5, 2.0, 4.5])
+    o = {"krylov_dim": 20}
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    wk = work(torch, B.syk_otoc_workspace_bytes(he, code, o))
+    for (iW, jV) in ((N - 1, N - 2), (0, 1), (5, N - 1)):
+        Fsum = 0
+        for s in (0, 1):
+            ps = opar.restrict(psi, L, s)
+            ref = opar.otoc_block_same_psi(props, N, iW, jV, 5.0, t_grid, ps.astype(np.complex128), s)
+            F, _ = B.syk_otoc_block(he, ho, s, iW, jV, 5.0, t_grid, to_dev(torch, ps), wk, o)
+            assert np.max(np.abs(F - ref)) <= TOL[dt] * max(abs(ref[0]), 1e-3), (iW, jV, s)
+            Fsum = Fsum + F
+        wkf = work(torch, B.syk_otoc_workspace_bytes(h, code, o))
+        Ffull, _ = B.syk_otoc(h, iW, jV, 5.0, t_grid, to_dev(torch, psi), wkf, o)
+        assert np.max(np.abs(Fsum - Ffull)) <= 4 * TOL[dt] * abs(Ffull[0])
+    Gsum = 0
+    for s in (0, 1):
+        ps = opar.restrict(psi, L, s)
+        ref = opar.green_block_same_psi(props, N, N - 1, 2.0, t_grid, ps.astype(np.complex128), s)
+        G, _ = B.syk_green_block(he, ho, s, N - 1, 2.0, t_grid, to_dev(torch, ps), wk, o)
+        assert np.max(np.abs(G - ref)) <= TOL[dt] * abs(ref[0]), s
+        Gsum = Gsum + G
+    Gfull, _ = B.syk_green(h, N - 1, 2.0, t_grid, to_dev(torch, psi), work(torch, B.syk_otoc_workspace_bytes(h, code, o)), o)
+    assert np.max(np.abs(Gsum - Gfull)) <= 4 * TOL[dt] * abs(Gfull[0])
+    # argument errors: blocks swapped, full handle where a block is expected, block where a full handle is expected
+    ps = to_dev(torch, opar.restrict(psi, L, 0))
+    for bad in (lambda: B.syk_otoc_block(ho, he, 0, 1, 2, 1.0, [0.0], ps, wk, o),
+                lambda: B.syk_otoc_block(h, h, 0, 1, 2, 1.0, [0.0], ps, wk, o),
+                lambda: B.syk_otoc_block(he, ho, 2, 1, 2, 1.0, [0.0], ps, wk, o),
+                lambda: B.syk_otoc_block(he, ho, 0, N, 2, 1.0, [0.0], ps, wk, o),
+                lambda: B.syk_otoc(he, 1, 2, 1.0, [0.0], ps, wk, o),
+                lambda: B.syk_green(he, 1, 1.0, [0.0], ps, wk, o)):
+        with pytest.raises(B.SykError):
+            bad()

@@ -200,3 +200,53 @@ def test_no_cpu_fallback_without_device(B):
     rc = B._lib.syk_apply_H(h.handle, B.SYK_C128, a, a + 256, None)
     assert rc == B.SYK_ECUDA
     assert B._lib.syk_last_cuda_error() != b""
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-1 parity blocks (DESIGN.md R-BLOCK)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gamma_norm", [0, 1])
+def test_parity_block_tables_bit_exact(B, gamma_norm):
+    """Tables of syk_build_parity_block against tables DERIVED from the dense block of every term matrix (the O4
+    recipe on the reduced basis: x' = column of the non-zero of row 0, c = that entry, bit q of z = 1 iff the
+    entry of row 2^q has the opposite sign), for both sectors."""
+    from oracle import parity as opar
+    N, L = 10, 5
+    q, J, _ = orng.sample_couplings(N, 0.5, seed=3, realization=1)
+    h = B.syk_build_from_terms(N, q, J, gamma_norm)
+    g = majorana.jw_gammas(N, gamma_norm)
+    for sector in (0, 1):
+        hb = B.syk_build_parity_block(h, sector)
+        info = hb.info()
+        assert info["N"] == N - 2 and info["dim"] == 1 << (L - 1) and info["n_terms"] == len(J)
+        tab = hb.tables()
+        idx = opar.sector_indices(L, sector).astype(np.int64)
+        ref = []
+        for (i, j, k, l), Jt in zip(q, J):
+            M = (Jt * (g[i] @ g[j] @ g[k] @ g[l]))[np.ix_(idx, idx)]
+            x = int(np.nonzero(M[0])[0][0])
+            c = M[0, x]
+            z = 0
+            for bit in range(L - 1):
+                e = M[1 << bit, (1 << bit) ^ x]
+                assert abs(abs(e) - abs(c)) <= 1e-15
+                if abs(e + c) <= 1e-15:
+                    z |= 1 << bit
+            ref.append((x, z, c, (int(i), int(j), int(k), int(l))))
+        ref.sort(key=lambda r: (r[0], r[1]))
+        xs = np.repeat(tab["x"], np.diff(tab["group_off"].astype(np.int64)))
+        assert [int(v) for v in xs] == [r[0] for r in ref]
+        assert [int(v) for v in tab["z"]] == [r[1] for r in ref]
+        assert [tuple(int(a) for a in row) for row in tab["quartet_of_term"]] == [r[3] for r in ref]
+        assert_coeff_equal(tab["c"], np.array([r[2] for r in ref]), gamma_norm)
+        # and the table form reproduces the block matrix on a vector
+        v = np.random.default_rng(5).normal(size=1 << (L - 1)) + 0j
+        Hs = opar.block_hamiltonian(N, q, J, sector, gamma_norm)
+        assert np.allclose(ohm.matvec_from_tables(tab, v), Hs @ v, atol=1e-13)
+        # a block of a block, bad sector, too small N
+        for bad in (lambda: B.syk_build_parity_block(hb, 0), lambda: B.syk_build_parity_block(h, 2)):
+            with pytest.raises(B.SykError):
+                bad()
+    h4 = B.syk_build_from_terms(4, np.array([[0, 1, 2, 3]], dtype=np.int32), np.array([1.0]))
+    with pytest.raises(B.SykError):
+        B.syk_build_parity_block(h4, 0)
