@@ -40,6 +40,9 @@ WORKLOADS = {
                     "i_W": 55, "j_V": 54},
     "N64_k2_c64": {"N": 64, "k": 2, "dtype": "c64", "krylov_dim": 8, "two_pass": 1, "dt": 0.5, "beta": 5.0,
                    "i_W": 63, "j_V": 62},
+    # the same N=56 workload in one parity block: 2^27 amplitudes, 2.1 GB vectors
+    "N56_k4_c128_block": {"N": 56, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
+                          "i_W": 55, "j_V": 54, "block": 1},
     # smaller shapes of the same path (parity-test sizes; handy for quick runs and ncu)
     "N48_k4_c128": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 16, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                     "i_W": 47, "j_V": 46},
@@ -225,7 +228,8 @@ def run_ours(args, wl, name):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     N, k = wl["N"], wl["k"]
-    D = 1 << (N // 2)
+    block = bool(wl.get("block"))
+    D = 1 << (N // 2 - (1 if block else 0))          # parity block: half the amplitudes
     tdt = torch.complex128 if wl["dtype"] == "c128" else torch.complex64
     code = B.SYK_C128 if wl["dtype"] == "c128" else B.SYK_C64
     eb = 16 if wl["dtype"] == "c128" else 8
@@ -237,6 +241,8 @@ def run_ours(args, wl, name):
     realization = rank * batch                       # independent realizations per rank (weak scaling)
 
     h0 = B.syk_build_hamiltonian(N, p, 0, realization)
+    if block:
+        h0 = B.syk_build_parity_block(h0, 0)
     info = h0.info()
     n_x, n_t = info["n_xmasks"], info["n_terms"]
     kbytes = B.syk_krylov_workspace_bytes(h0, code, opts)
@@ -244,10 +250,12 @@ def run_ours(args, wl, name):
     wk = torch.empty(kbytes + V, dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
     l = torch.empty((batch, D), dtype=tdt, device="cuda")
     r = torch.empty((batch, D), dtype=tdt, device="cuda")
+    Nvec = N - 2 if block else N                     # number of Majoranas that spans the stored vector
     for i in range(batch):
-        B.syk_random_state(N, 0, realization + i, r[i], scratch)
-        B.syk_apply_gamma(N, wl["j_V"], r[i], l[i])  # a second, different state for the bra side
+        B.syk_random_state(Nvec, 0, realization + i, r[i], scratch)
+        B.syk_apply_gamma(Nvec, 1, r[i], l[i])       # a second, different state for the bra side
     torch.cuda.synchronize()
+    sector = [0]                                     # parity block the state is in (every gamma flips it)
 
     stats_acc = {"n_matvec": 0, "model_bytes": 0.0, "n_substeps": 0}
 
@@ -255,9 +263,16 @@ def run_ours(args, wl, name):
         F = 0.0
         for i in range(batch):
             h = B.syk_build_hamiltonian(N, p, 0, realization + i)                     # a-1
-            B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                               # a-5 insertion (in place)
+            if block:
+                sector[0] ^= 1
+                hb = B.syk_build_parity_block(h, sector[0])                           # a-1, block of the new sector
+                h.close()
+                h = hb
+                B.syk_apply_gamma_block(N, wl["i_W"], sector[0], r[i], r[i])          # a-5 insertion (no gather)
+            else:
+                B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                           # a-5 insertion (in place)
             st = B.syk_krylov_evolve(h, r[i], tau[0], tau[1], wk, opts)               # a-2, a-3, a-4
-            F = B.syk_dot(N, l[i], r[i], scratch)                                     # a-5 inner product
+            F = B.syk_dot(Nvec, l[i], r[i], scratch)                                  # a-5 inner product
             stats_acc["n_matvec"] += st["n_matvec"]
             stats_acc["n_substeps"] += st["n_substeps"]
             stats_acc["model_bytes"] += st["model_bytes"] + 4.0 * V                   # gamma: 2V, dot: 2V
@@ -315,6 +330,10 @@ def run_ours(args, wl, name):
             tot = {"model_bytes": 0.0}
             for i in range(batch):
                 h = B.syk_build_hamiltonian(N, p, 0, realization + i)
+                if block:
+                    hb = B.syk_build_parity_block(h, 0)
+                    h.close()
+                    h = hb
                 tot["model_bytes"] += B.syk_krylov_evolve_host(h, host, tau[0], tau[1], wk, opts)["model_bytes"]
                 h.close()
             return tot
@@ -391,7 +410,7 @@ def run_ours(args, wl, name):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if wl["dtype"] == "c128" else "f32", "data": "synthetic",
-            "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2, "n_terms": n_t, "n_xmasks": n_x,
+            "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2 - (1 if block else 0), "parity_block": block, "n_terms": n_t, "n_xmasks": n_x,
                        "vector_bytes": V, "krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"],
                        "tau": list(tau), "realizations_per_gpu": batch,
                        "l2_policy": ("inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9)) if V > 3e8 else

@@ -15,6 +15,7 @@ Modules
   evolve       exact exp(-i tau H) by full diagonalisation; Chebyshev series     (O6, O8)
   otoc         same-psi and exact-trace regularised OTOC                        (O7)
   green        same-psi and exact-trace retarded Green function
+  pauli        generic sums of Pauli strings / spin chains by Kronecker products
   parity       parity blocks H_UU / H_DD, gamma blocks, block OTOC / Green function
   alg1         literal transcription of the paper's Algorithm 1 (Python + C)    (P6)
 

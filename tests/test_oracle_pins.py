@@ -10,7 +10,7 @@ import os
 import numpy as np
 import pytest
 
-from oracle import alg1, evolve, green, hamiltonian, majorana, otoc, parity, rng
+from oracle import alg1, evolve, green, hamiltonian, majorana, otoc, parity, pauli, rng
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -439,3 +439,27 @@ def test_P14_parity_blocks(gamma_norm):
     Gb = sum(parity.green_block_same_psi(props, N, N - 1, 1.5, t_grid, parity.restrict(v, L, sec), sec, gamma_norm)
              for sec in (0, 1))
     assert np.allclose(G, Gb, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P15 generic Pauli sums
+def test_P15_pauli_strings_and_spin_chains():
+    """(i) Z X = i Y for the textbook Y (R-Y), so the string (x=1, z=1, c=-i) is Y; a JW Majorana is the string the
+    term compiler uses; (ii) the periodic transverse-field Ising chain has the free-fermion ground energy
+    E0 = -sum_m sqrt(J^2 + h^2 - 2 J h cos(pi (2m+1)/L)) (even-parity sector, textbook); (iii) the Heisenberg chain
+    commutes with total S^z and two sites give the singlet/triplet levels -3J, +J."""
+    Y = np.array([[0, -1j], [1j, 0]])
+    assert np.allclose(pauli.string_matrix(1, 1, 1, -1j), Y, atol=0)
+    assert np.allclose(pauli.string_matrix(2, 0b10, 0b01, 1.0), np.kron(majorana.SX, majorana.SZ), atol=0)
+    g = majorana.jw_gammas(8)
+    assert np.allclose(pauli.string_matrix(4, 0b0100, 0b0011, 1.0), g[4], atol=0)        # gamma_4 = Z0 Z1 X2
+    assert np.allclose(pauli.string_matrix(4, 0b0100, 0b0111, -1j), g[5], atol=0)       # gamma_5 = Z0 Z1 Y2
+    L, J, h = 8, 1.0, 0.7
+    H = pauli.sum_matrix(L, pauli.transverse_ising_terms(L, J, h))
+    assert np.allclose(H, H.conj().T, atol=0)
+    k = np.pi * (2 * np.arange(L) + 1) / L
+    assert abs(np.linalg.eigvalsh(H)[0] + np.sum(np.sqrt(J * J + h * h - 2 * J * h * np.cos(k)))) < 1e-12
+    H2 = pauli.sum_matrix(2, pauli.heisenberg_terms(2, 1.0, 1.0, 1.0))
+    assert np.allclose(np.linalg.eigvalsh(H2), [-3.0, 1.0, 1.0, 1.0], atol=1e-13)
+    H6 = pauli.sum_matrix(6, pauli.heisenberg_terms(6, 1.0, 1.0, 0.5, periodic=True))
+    Sz = sum(pauli.string_matrix(6, 0, 1 << q) for q in range(6))
+    assert np.allclose(H6 @ Sz, Sz @ H6, atol=1e-13) and np.allclose(H6, H6.conj().T, atol=0)
