@@ -62,6 +62,15 @@ int syk_version(void);
 int syk_build_hamiltonian(int N, double p, uint64_t seed, uint32_t realization, int gamma_norm, syk_ham** out);
 int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets /* [n_terms][4] */,
                          const double* J /* [n_terms] */, int gamma_norm, syk_ham** out);
+/* Generic Hermitian sum of Pauli strings on L qubits (2 <= L <= 32; spin chains, Ising-type
+ * models through the same operator action).  String t is c_t Z^{z_t} X^{x_t} acting as
+ * (O v)[b] = c_t (-1)^popcount(b & z_t) v[b xor x_t] (R-SIGN; Y = -i Z X).  Strings must be Hermitian one by one:
+ * c_t real when popcount(x_t & z_t) is even, imaginary when odd; otherwise SYK_EINVAL (non-Hermitian operators
+ * need Arnoldi: out of scope).  Equal (x, z) are combined.  The handle works with syk_apply_H, syk_lanczos_run,
+ * syk_krylov_evolve and the work-space queries (dim = 2^L; syk_ham_info reports N = 2L); the Majorana calls
+ * (syk_otoc, syk_green, syk_build_parity_block) reject it. */
+int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, const uint64_t* z, const double* c_re_im,
+                                 syk_ham** out);
 void syk_free_hamiltonian(syk_ham* h);
 
 /* Sizes: any output pointer may be NULL. dim = 2^(N/2). */

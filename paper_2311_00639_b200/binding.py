@@ -54,6 +54,7 @@ _SIGNATURES = {
     "syk_version": (_i, []),
     "syk_build_hamiltonian": (_i, [_i, _d, _u64, _u32, _i, _P(_vp)]),
     "syk_build_from_terms": (_i, [_i, _i64, _vp, _vp, _i, _P(_vp)]),
+    "syk_build_from_pauli_strings": (_i, [_i, _i64, _vp, _vp, _vp, _P(_vp)]),
     "syk_free_hamiltonian": (None, [_vp]),
     "syk_ham_info": (_i, [_vp, _P(_i), _P(_i64), _P(_i64), _P(_i64)]),
     "syk_ham_tables": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -185,6 +186,18 @@ def syk_build_from_terms(N, quartets, J, gamma_norm=SYK_GAMMA_PAULI):
     out = ctypes.c_void_p()
     _check(_lib.syk_build_from_terms(int(N), len(Jc), q.ctypes.data, Jc.ctypes.data, int(gamma_norm),
                                      ctypes.byref(out)), "syk_build_from_terms")
+    return Hamiltonian(out.value)
+
+
+def syk_build_from_pauli_strings(L, terms):
+    """terms: iterable of (x, z, c) with c real or imaginary as Hermiticity demands (see include/syk.h)."""
+    terms = list(terms)
+    x = np.array([int(t[0]) for t in terms], dtype=np.uint64)
+    z = np.array([int(t[1]) for t in terms], dtype=np.uint64)
+    c = np.array([[complex(t[2]).real, complex(t[2]).imag] for t in terms], dtype=np.float64).reshape(-1, 2)
+    out = ctypes.c_void_p()
+    _check(_lib.syk_build_from_pauli_strings(int(L), len(terms), x.ctypes.data, z.ctypes.data, c.ctypes.data,
+                                             ctypes.byref(out)), "syk_build_from_pauli_strings")
     return Hamiltonian(out.value)
 
 

@@ -90,6 +90,7 @@ struct syk_ham {
     std::vector<double> J;                     // [n_terms]
     int block_of_N = 0;                        // parity block (syk_build_parity_block): N of the full Hamiltonian, else 0
     int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
+    bool generic = false;                      // built from caller-supplied Pauli strings (no Majorana meaning)
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable syk::DeviceTables dev;             // created on first device use
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)

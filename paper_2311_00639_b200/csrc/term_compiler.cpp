@@ -159,8 +159,39 @@ int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets, const 
     return compile(N, gamma_norm, raw, out);
 }
 
+int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, const uint64_t* z, const double* c_re_im,
+                                 syk_ham** out) {
+    if (!out || L < 2 || L > 32 || n_terms < 0 || (n_terms > 0 && (!x || !z || !c_re_im))) return SYK_EINVAL;
+    if (n_terms > 0xFFFFFFF0ll) return SYK_EINVAL;
+    *out = nullptr;
+    const uint64_t mask = L == 64 ? ~0ull : ((1ull << L) - 1);
+    std::vector<RawTerm> raw;
+    try {
+        raw.resize((size_t)n_terms);
+    } catch (const std::bad_alloc&) {
+        return SYK_ENOMEM;
+    }
+    for (int64_t t = 0; t < n_terms; ++t) {
+        if ((x[t] | z[t]) & ~mask) return SYK_EINVAL;
+        const double re = c_re_im[2 * t], im = c_re_im[2 * t + 1];
+        // Hermitian sum of independent strings: (c Z^z X^x)^+ = conj(c) (-1)^popcount(x & z) Z^z X^x, so c must be
+        // real when popcount(x & z) is even and imaginary when it is odd (the Lanczos driver needs H = H^+)
+        const bool odd = __builtin_popcountll(x[t] & z[t]) & 1;
+        if (!std::isfinite(re) || !std::isfinite(im) || (odd ? re != 0.0 : im != 0.0)) return SYK_EINVAL;
+        RawTerm& r = raw[(size_t)t];
+        r.x = x[t];
+        r.z = z[t];
+        r.c = {re, im};
+        for (int k = 0; k < 4; ++k) r.q[k] = -1;
+        r.J = 0.0;
+    }
+    int rc = compile(2 * L, SYK_GAMMA_PAULI, raw, out);
+    if (rc == SYK_OK) (*out)->generic = true;
+    return rc;
+}
+
 int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out) {
-    if (!h || !out || (sector != 0 && sector != 1) || h->block_of_N != 0 || h->N < 6) return SYK_EINVAL;
+    if (!h || !out || (sector != 0 && sector != 1) || h->block_of_N != 0 || h->generic || h->N < 6) return SYK_EINVAL;
     *out = nullptr;
     const int L = h->L;
     const uint64_t low = (1ull << (L - 1)) - 1;

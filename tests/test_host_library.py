@@ -250,3 +250,31 @@ def test_parity_block_tables_bit_exact(B, gamma_norm):
     h4 = B.syk_build_from_terms(4, np.array([[0, 1, 2, 3]], dtype=np.int32), np.array([1.0]))
     with pytest.raises(B.SykError):
         B.syk_build_parity_block(h4, 0)
+
+
+def test_pauli_string_builder(B):
+    """syk_build_from_pauli_strings: canonical tables, duplicates combined, Hermiticity rule, range checks; the
+    table form applied on the host reproduces the oracle's Kronecker-product matrix."""
+    from oracle import pauli as opauli
+    L = 6
+    terms = opauli.heisenberg_terms(L, 0.7, -0.4, 1.1, periodic=True) + opauli.transverse_ising_terms(L, 0.3, 0.9)
+    h = B.syk_build_from_pauli_strings(L, terms)
+    info = h.info()
+    assert info["N"] == 2 * L and info["dim"] == 1 << L
+    tab = h.tables()
+    assert info["n_terms"] == len(terms) - L            # the ZZ bonds occur twice and are combined
+    xs = np.repeat(tab["x"], np.diff(tab["group_off"].astype(np.int64)))
+    assert np.all(np.diff(xs.astype(np.int64)) >= 0)
+    H = opauli.sum_matrix(L, terms)
+    v = np.random.default_rng(1).normal(size=1 << L) + 1j * np.random.default_rng(2).normal(size=1 << L)
+    assert np.allclose(ohm.matvec_from_tables(tab, v), H @ v, atol=1e-13)
+    for bad in ([(1, 1, 1.0)],            # Y-like string needs an imaginary coefficient
+                [(1, 0, 1j)],             # X needs a real one
+                [(1 << L, 0, 1.0)],       # bit outside the chain
+                [(0, 1 << L, 1.0)]):
+        with pytest.raises(B.SykError):
+            B.syk_build_from_pauli_strings(L, bad)
+    with pytest.raises(B.SykError):
+        B.syk_build_from_pauli_strings(1, [(1, 0, 1.0)])
+    with pytest.raises(B.SykError):
+        B.syk_build_parity_block(h, 0)
