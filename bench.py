@@ -49,7 +49,7 @@ WORKLOADS = {
     # BASELINE.json configs[1] / configs[2] shapes: disorder realizations batched on one GPU (run back to back on one
     # stream; each step advances every realization by one time segment)
     "N32_k4_c128_x100": {"N": 32, "k": 4, "dtype": "c128", "krylov_dim": 12, "two_pass": 0, "dt": 0.1, "beta": 5.0,
-                         "i_W": 31, "j_V": 30, "batch": 100},
+                         "i_W": 31, "j_V": 30, "batch": 100, "lockstep": 1},
     "N48_k4_c128_x20": {"N": 48, "k": 4, "dtype": "c128", "krylov_dim": 30, "two_pass": 0, "dt": 0.5, "beta": 5.0,
                         "i_W": 47, "j_V": 46, "batch": 20},
     # BASELINE.json configs[2], dense p = 1 member: ALU-bound (194 580 terms on 10 903 X-masks, ~0.75 s per matvec)
@@ -259,7 +259,29 @@ def run_ours(args, wl, name):
 
     stats_acc = {"n_matvec": 0, "model_bytes": 0.0, "n_substeps": 0}
 
+    lockstep = bool(wl.get("lockstep")) and batch > 1
+    if lockstep:
+        wk_b = torch.empty(B.syk_krylov_workspace_bytes_batched(h0, batch, code, opts), dtype=torch.uint8, device="cuda")
+
+    def step_lockstep():
+        # every realization advances through the Lanczos recurrence in the same launches (grid.y = realization)
+        hams = [B.syk_build_hamiltonian(N, p, 0, realization + i) for i in range(batch)]     # a-1
+        for i in range(batch):
+            B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                                   # a-5 insertion
+        st = B.syk_krylov_evolve_batched(hams, r, D, tau[0], tau[1], wk_b, opts)          # a-2, a-3, a-4
+        F = 0.0
+        for i in range(batch):
+            F = B.syk_dot(N, l[i], r[i], scratch)                                         # a-5 inner product
+        stats_acc["n_matvec"] += st["n_matvec"]
+        stats_acc["n_substeps"] += st["n_substeps"]
+        stats_acc["model_bytes"] += st["model_bytes"] + 4.0 * V * batch
+        for h in hams:
+            h.close()
+        return F
+
     def step():
+        if lockstep:
+            return step_lockstep()
         F = 0.0
         for i in range(batch):
             h = B.syk_build_hamiltonian(N, p, 0, realization + i)                     # a-1
@@ -412,7 +434,7 @@ def run_ours(args, wl, name):
             "vs_baseline": None, "dtype": "f64" if wl["dtype"] == "c128" else "f32", "data": "synthetic",
             "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2 - (1 if block else 0), "parity_block": block, "n_terms": n_t, "n_xmasks": n_x,
                        "vector_bytes": V, "krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"],
-                       "tau": list(tau), "realizations_per_gpu": batch,
+                       "tau": list(tau), "realizations_per_gpu": batch, "lockstep_batched": lockstep,
                        "l2_policy": ("inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9)) if V > 3e8 else
                                     ("working set of one step %.2f GB > L2 (%d realizations x %d vectors of %.1f MB)"
                                      % (batch * (wl["krylov_dim"] + 2) * V / 1e9, batch, wl["krylov_dim"] + 2, V / 1e6)),

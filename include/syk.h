@@ -149,6 +149,16 @@ int syk_lanczos_run(const syk_ham* h, int dtype, const void* d_psi, int m, doubl
 int syk_krylov_evolve(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im,
                       const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream);
 
+/* Lock-step batched evolution: psi_r <- exp(-i tau H_r) psi_r for r < n_batch, psi_r at d_psi + r*batch_stride elements.
+ * Same conditions as the lock-step mode of syk_otoc_batched (else SYK_EINVAL); opts->two_pass must be 0.  Work space:
+ * syk_krylov_workspace_bytes_batched.  stats: n_matvec counts realization-matvecs, n_substeps the rounds, err_est the
+ * largest per-realization estimate. */
+int syk_krylov_workspace_bytes_batched(const syk_ham* h, int n_batch, int dtype, const syk_krylov_opts* opts,
+                                       size_t* bytes);
+int syk_krylov_evolve_batched(const syk_ham* const* hams, int n_batch, int dtype, void* d_psi, int64_t batch_stride,
+                              double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
+                              syk_stats* stats, void* stream);
+
 /* Same with a HOST vector (in/out): d_work must hold one extra vector in front of the Krylov work space, i.e.
  * D*elem_bytes + syk_krylov_workspace_bytes(). */
 int syk_krylov_evolve_host(const syk_ham* h, int dtype, void* h_psi, double tau_re, double tau_im,
@@ -198,8 +208,17 @@ int syk_green_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int
                     const double* t_grid, int n_t, void* d_psi, double* G_out, const syk_krylov_opts* opts, void* d_work,
                     size_t work_bytes, syk_stats* stats, void* stream);
 
-/* Batched over disorder realizations: realization r uses hams[r], state d_psi + r*batch_stride elements, and
- * writes F_out[r][n_t][2].  One work space is shared (realizations run back to back on `stream`). */
+/* Batched over disorder realizations: realization r uses hams[r], state d_psi + r*batch_stride
+ * elements, and writes F_out[r][n_t][2].  Two modes, chosen by the work space the caller passes:
+ *  - lock-step: work_bytes >= syk_otoc_batched_workspace_bytes(hams[0], n_batch, ...), all realizations have the same N,
+ *    one-pass Lanczos, and every term table fits the shared-memory budget of the 16 KiB-tile kernel (sparse H, small
+ *    and medium N).  Every kernel then runs with grid.y = realization: one launch per Lanczos step for the whole
+ *    batch, the host does the n_batch small exponentials between rounds.  batch_stride * element size must be a
+ *    multiple of 16 bytes.
+ *  - otherwise: one work space of syk_otoc_workspace_bytes is shared and the realizations run back to back.
+ * Results of the two modes agree to the Krylov tolerance (sub-steps are chosen per realization in both). */
+int syk_otoc_batched_workspace_bytes(const syk_ham* h, int n_batch, int dtype, const syk_krylov_opts* opts,
+                                     size_t* bytes);
 int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,
                      const double* t_grid, int n_t, void* d_psi, int64_t batch_stride, double* F_out,
                      const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream);

@@ -78,6 +78,10 @@ _SIGNATURES = {
                             _vp]),
     "syk_green_block": (_i, [_vp, _vp, _i, _i, _i, _d, _vp, _i, _vp, _vp, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats),
                              _vp]),
+    "syk_krylov_workspace_bytes_batched": (_i, [_vp, _i, _i, _P(syk_krylov_opts), _P(_sz)]),
+    "syk_krylov_evolve_batched": (_i, [_P(_vp), _i, _i, _vp, _i64, _d, _d, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats),
+                                       _vp]),
+    "syk_otoc_batched_workspace_bytes": (_i, [_vp, _i, _i, _P(syk_krylov_opts), _P(_sz)]),
     "syk_otoc_batched": (_i, [_P(_vp), _i, _i, _i, _i, _d, _vp, _i, _vp, _i64, _vp, _P(syk_krylov_opts), _vp, _sz,
                               _P(syk_stats), _vp]),
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
@@ -387,6 +391,30 @@ def syk_green_block(h_even, h_odd, sector, n, beta, t_grid, d_psi, d_work, opts=
                                 d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
            "syk_green_block")
     return G[:, 0] + 1j * G[:, 1], st.as_dict()
+
+
+def syk_krylov_workspace_bytes_batched(h, n_batch, dtype, opts=None):
+    n = ctypes.c_size_t()
+    _check(_lib.syk_krylov_workspace_bytes_batched(_h(h), int(n_batch), int(dtype), _opts(opts), ctypes.byref(n)),
+           "syk_krylov_workspace_bytes_batched")
+    return n.value
+
+
+def syk_krylov_evolve_batched(hams, d_psi, batch_stride, tau_re, tau_im, d_work, opts=None, stream=None):
+    arr = (ctypes.c_void_p * len(hams))(*[_h(h).value for h in hams])
+    st = syk_stats()
+    _check(_lib.syk_krylov_evolve_batched(arr, len(hams), dtype_code(d_psi), _dptr(d_psi), int(batch_stride),
+                                          float(tau_re), float(tau_im), _opts(opts), _dptr(d_work),
+                                          d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
+           "syk_krylov_evolve_batched")
+    return st.as_dict()
+
+
+def syk_otoc_batched_workspace_bytes(h, n_batch, dtype, opts=None):
+    n = ctypes.c_size_t()
+    _check(_lib.syk_otoc_batched_workspace_bytes(_h(h), int(n_batch), int(dtype), _opts(opts), ctypes.byref(n)),
+           "syk_otoc_batched_workspace_bytes")
+    return n.value
 
 
 def syk_otoc_batched(hams, i_W, j_V, beta, t_grid, d_psi, batch_stride, d_work, opts=None, stream=None):

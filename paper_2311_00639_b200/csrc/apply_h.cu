@@ -19,6 +19,8 @@
 //
 // Fused epilogue for the Lanczos step (a-3): out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, partial sums of
 // Re <in|out> per CTA (fp64), see common.h FusedArgs.
+#include <vector>
+
 #include "device_utils.cuh"
 
 namespace syk {
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(256) apply_h_generic_kernel(Params<T> p) {
 // TMA-pipelined tile kernel.  R = outputs per consumer thread; tile = R * 256 amplitudes = 16 KiB.
 // ---------------------------------------------------------------------------------------------------------
 template <typename T, int R, bool FUSED>
-__global__ void __launch_bounds__(kTmaThreads, 1) apply_h_tma_kernel(Params<T> p) {
+__device__ __forceinline__ void tma_body(const Params<T>& p) {
     using C = typename Cx<T>::type;
     constexpr int TILE = R * kConsumerThreads;
     static_assert(TILE * sizeof(C) == kTileBytes, "tile must be 16 KiB");
@@ -291,6 +293,38 @@ __global__ void __launch_bounds__(kTmaThreads, 1) apply_h_tma_kernel(Params<T> p
     }
 }
 
+template <typename T, int R, bool FUSED>
+__global__ void __launch_bounds__(kTmaThreads, 1) apply_h_tma_kernel(Params<T> p) {
+    tma_body<T, R, FUSED>(p);
+}
+
+// Batched over disorder realizations (configs[1]): grid.y = realization.  Every realization has its own
+// tables (tab[r]); the vectors and Lanczos scalars of realization r sit at base + r * stride bytes.  Small vectors:
+// few stages, so that two CTAs share an SM.
+template <typename T>
+struct BatchedParams {
+    const Params<T>* tab;
+    const char* in;
+    char* out;
+    const char* prev;
+    char* sc;
+    size_t s_in, s_out, s_prev, s_sc;
+    int j;
+};
+
+template <typename T, int R, bool FUSED>
+__global__ void __launch_bounds__(kTmaThreads, 2) apply_h_tma_batched_kernel(BatchedParams<T> bp) {
+    using C = typename Cx<T>::type;
+    Params<T> p = bp.tab[blockIdx.y];
+    const size_t r = blockIdx.y;
+    p.in = reinterpret_cast<const C*>(bp.in + r * bp.s_in);
+    p.out = reinterpret_cast<C*>(bp.out + r * bp.s_out);
+    p.prev = bp.prev ? reinterpret_cast<const C*>(bp.prev + r * bp.s_prev) : nullptr;
+    p.sc = bp.sc ? reinterpret_cast<LanczosScalars*>(bp.sc + r * bp.s_sc) : nullptr;
+    p.j = bp.j;
+    tma_body<T, R, FUSED>(p);
+}
+
 size_t tma_table_bytes(int n_groups, int n_terms, int n_loads, size_t csize) {
     size_t b = (size_t)n_terms * csize + 2 * kMaxStages * 8 + 40 * 8;
     b += (size_t)n_groups * 4 + (size_t)(n_groups + 1) * 4 + (size_t)n_terms * 4;
@@ -363,7 +397,111 @@ int launch_typed(const syk_ham* h, const void* d_in, void* d_out, const FusedArg
     return SYK_OK;
 }
 
+constexpr int kBatchedStages = 5;
+
+template <typename T, int R>
+int launch_batched_typed(const syk_ham* const* hams, int nb, void* d_tab, const void* in, size_t s_in, void* out,
+                         size_t s_out, const void* prev, size_t s_prev, void* sc, size_t s_sc, int j, bool upload,
+                         cudaStream_t stream) {
+    using C = typename Cx<T>::type;
+    const int k = sizeof(C) == 16 ? 1 : 0;
+    size_t table_max = 0;
+    std::vector<Params<T>> host;
+    if (upload) host.resize((size_t)nb);
+    for (int r = 0; r < nb; ++r) {
+        const syk_ham* h = hams[r];
+        const DeviceTables& d = h->dev;
+        const size_t tb = tma_table_bytes((int)h->n_groups(), (int)h->n_terms(), d.n_loads[k], sizeof(C));
+        table_max = tb > table_max ? tb : table_max;
+        if (!upload) continue;
+        Params<T>& p = host[(size_t)r];
+        p.in = nullptr;
+        p.out = nullptr;
+        p.prev = nullptr;
+        p.sc = nullptr;
+        p.j = 0;
+        p.gx = d.gx;
+        p.goff = d.goff;
+        p.tz = d.tz;
+        p.tc = k ? (const C*)d.tc128 : (const C*)d.tc64;
+        p.load_hi = d.load_hi[k];
+        p.load_g0 = d.load_g0[k];
+        p.n_groups = (int)h->n_groups();
+        p.n_terms = (int)h->n_terms();
+        p.n_loads = d.n_loads[k];
+        p.L = h->L;
+        p.nstage = kBatchedStages;
+    }
+    if (upload) {
+        SYK_CUDA(cudaMemcpyAsync(d_tab, host.data(), sizeof(Params<T>) * (size_t)nb, cudaMemcpyHostToDevice, stream));
+        SYK_CUDA(cudaStreamSynchronize(stream));   // `host` goes out of scope
+    }
+    const size_t smem = (size_t)kBatchedStages * kTileBytes + table_max;
+    if (smem > (size_t)kSmemLimit) return SYK_EINVAL;
+    BatchedParams<T> bp;
+    bp.tab = (const Params<T>*)d_tab;
+    bp.in = (const char*)in;
+    bp.out = (char*)out;
+    bp.prev = (const char*)prev;
+    bp.sc = (char*)sc;
+    bp.s_in = s_in;
+    bp.s_out = s_out;
+    bp.s_prev = s_prev;
+    bp.s_sc = s_sc;
+    bp.j = j;
+    const uint64_t n_tiles = 1ull << (hams[0]->L - kTileLog2[k]);
+    const int sms = num_sms();
+    if (sms <= 0) return SYK_ECUDA;
+    const unsigned gx = (unsigned)(n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms);
+    const dim3 grid(gx, (unsigned)nb);
+    if (sc) {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_tma_batched_kernel<T, R, true>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_tma_batched_kernel<T, R, true><<<grid, kTmaThreads, smem, stream>>>(bp);
+    } else {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_tma_batched_kernel<T, R, false>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_tma_batched_kernel<T, R, false><<<grid, kTmaThreads, smem, stream>>>(bp);
+    }
+    count_launch();
+    SYK_CUDA(cudaGetLastError());
+    return SYK_OK;
+}
+
 }  // namespace
+
+size_t batched_table_bytes(int nb) {
+    const size_t a = sizeof(Params<double>) > sizeof(Params<float>) ? sizeof(Params<double>) : sizeof(Params<float>);
+    return (a * (size_t)nb + 4095) & ~(size_t)4095;
+}
+
+// Can these realizations go through the batched tile kernel?  Same N, every table fits the shared-memory budget, the
+// vector spans at least one 16 KiB tile.
+bool batched_apply_ok(const syk_ham* const* hams, int nb, int dtype) {
+    if (!hams || nb < 1 || !hams[0]) return false;
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    for (int r = 0; r < nb; ++r) {
+        const syk_ham* h = hams[r];
+        if (!h || h->N != hams[0]->N || h->L < kTileLog2[k] || h->n_terms() == 0) return false;
+        const size_t tb = tma_table_bytes((int)h->n_groups(), (int)h->n_terms(), (int)h->n_groups() + 1, elem_bytes(dtype));
+        if (tb + (size_t)kBatchedStages * kTileBytes > (size_t)kSmemLimit / 2 - 1024) return false;   // two CTAs per SM
+    }
+    return true;
+}
+
+int launch_apply_h_batched(const syk_ham* const* hams, int nb, int dtype, void* d_tab, bool upload, const void* in,
+                           size_t s_in, void* out, size_t s_out, const void* prev, size_t s_prev, void* sc, size_t s_sc,
+                           int j, cudaStream_t stream) {
+    for (int r = 0; r < nb; ++r) SYK_TRY(ensure_device_tables(hams[r]));
+    profile_begin(stream);
+    const int rc = dtype == SYK_C128
+                       ? launch_batched_typed<double, 4>(hams, nb, d_tab, in, s_in, out, s_out, prev, s_prev, sc, s_sc, j,
+                                                         upload, stream)
+                       : launch_batched_typed<float, 8>(hams, nb, d_tab, in, s_in, out, s_out, prev, s_prev, sc, s_sc, j,
+                                                        upload, stream);
+    profile_end(stream);
+    return rc;
+}
 
 int apply_h_kernel_kind(const syk_ham* h, int dtype) {
     const int avail = tma_stages(h, dtype) >= 3 ? 1 : 0;

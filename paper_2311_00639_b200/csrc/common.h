@@ -148,7 +148,7 @@ struct LanczosScalars {
     int n_partial_dot;              // how many entries of partial_dot are valid
     int n_partial_nrm;
     int n_partial_cdot;
-    int pad;
+    int m_eff;                      // batched combine: effective Krylov dimension of this realization
 };
 
 // What the fused epilogue of apply_H does (all pointers device):
@@ -188,24 +188,45 @@ void free_dense_tables(const syk_ham* h);
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
                    cudaStream_t stream);
 
+// Batched launches over disorder realizations (grid.y = realization): pointer argument k of realization r is
+// base_k + r * stride_k bytes (a, b, c in the launcher's argument order), its LanczosScalars base + r * sc bytes.
+struct BatchStride { size_t a = 0, b = 0, c = 0, sc = 0; };
+struct Batch {
+    int n = 1;
+    BatchStride s;
+};
+
+// batched apply_H over realizations with the 16 KiB-tile kernel (apply_h.cu): d_tab = device array of
+// batched_table_bytes(nb) bytes that receives the per-realization table descriptors when `upload` is set
+size_t batched_table_bytes(int nb);
+bool batched_apply_ok(const syk_ham* const* hams, int nb, int dtype);
+int launch_apply_h_batched(const syk_ham* const* hams, int nb, int dtype, void* d_tab, bool upload, const void* in,
+                           size_t s_in, void* out, size_t s_out, const void* prev, size_t s_prev, void* sc, size_t s_sc,
+                           int j, cudaStream_t stream);
+
 // vector kernels (vector_ops.cu); all reductions go through LanczosScalars partial arrays
-int launch_norm2(int dtype, uint64_t D, const void* d_v, LanczosScalars* sc, cudaStream_t stream);
+int launch_norm2(int dtype, uint64_t D, const void* d_v, LanczosScalars* sc, cudaStream_t stream,
+                 const Batch& bt = Batch());
 // u_next = w - (alpha_j / nrm[j]) u_j in place on w, |u_next|^2 partials; alpha_j reduced from partial_dot.
 // When y != nullptr also y = y_scale * y + (coef[j]/nrm[j]) u_j  with y_scale = coef[1]/nrm[1] if first_y else 1.
 int launch_axpy_norm(int dtype, uint64_t D, void* d_w, const void* d_u, int j, LanczosScalars* sc, void* d_y,
-                     int first_y, cudaStream_t stream);
+                     int first_y, cudaStream_t stream, const Batch& bt = Batch());   // strides: w, u, y
 // finalises nrm[j] from partial_nrm (used after the last vector kernel of a run); 1 block
-int launch_finalize_nrm(int j, LanczosScalars* sc, cudaStream_t stream);
+int launch_finalize_nrm(int j, LanczosScalars* sc, cudaStream_t stream, const Batch& bt = Batch());
 // psi = sum_{j=1..m} (coef[j]/nrm[j]) u_j, u_1 = psi itself (in place), u_j (j >= 2) = vecs + (j-2)*stride_elems
 int launch_combine(int dtype, uint64_t D, void* d_psi, const void* d_vecs, uint64_t stride_elems, int m,
-                   LanczosScalars* sc, cudaStream_t stream);
+                   LanczosScalars* sc, cudaStream_t stream, const Batch& bt = Batch());   // m < 0: sc->m_eff; strides: psi, vecs
 // y = ys*y + (coef[j]/nrm[j]) u, ys = first_y ? coef[1]/nrm[1] : 1; u == nullptr drops the second term
 int launch_axpy_coef(int dtype, uint64_t D, void* d_y, const void* d_u, int j, int first_y, LanczosScalars* sc,
                      cudaStream_t stream);
-int launch_cdot(int dtype, uint64_t D, const void* d_a, const void* d_b, LanczosScalars* sc, cudaStream_t stream);
+int launch_cdot(int dtype, uint64_t D, const void* d_a, const void* d_b, LanczosScalars* sc, cudaStream_t stream,
+                const Batch& bt = Batch());
 int fetch_cdot(LanczosScalars* sc, double* re_im, cudaStream_t stream);   // host sum of the partials; synchronises
+int cdot_batched(int dtype, uint64_t D, const void* d_a, const void* d_b, LanczosScalars* sc, const Batch& bt,
+                 double* re_im /* [bt.n][2] */, cudaStream_t stream);
 int launch_normalise(int dtype, uint64_t D, void* d_v, LanczosScalars* sc, cudaStream_t stream);
-int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, cudaStream_t stream);
+int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, cudaStream_t stream,
+                 const Batch& bt = Batch());
 // gamma_n of the FULL space (N Majoranas) between parity blocks on N/2-1 qubits; the result lies in sector_out
 int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
                        cudaStream_t stream);
@@ -218,6 +239,11 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
                        const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
                        cudaStream_t stream);
 size_t krylov_header_bytes();
+size_t krylov_batched_bytes(const syk_ham* h0, int nb, int dtype, int m);
+int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, void* d_psi, size_t psi_stride_bytes,
+                               double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work,
+                               size_t work_bytes, syk_stats* stats, bool* tables_uploaded, cudaStream_t stream);
+int resolve_krylov_dim(const syk_ham* h, const syk_krylov_opts* o);
 
 // ---------------------------------------------------------------------------------------------------------
 // The counter-based generator R-RNG, host and device.

@@ -17,6 +17,7 @@
 #include <algorithm>
 #include <cmath>
 #include <complex>
+#include <cstddef>
 
 #include "common.h"
 
@@ -150,6 +151,59 @@ int effective_dim(int m, const double* alpha, const double* nrm, double eps) {
     return m;
 }
 
+// Host part of one sub-step: T_m from (alpha, nrm) -> effective dimension (happy breakdown), the longest sub-step hs
+// along the ray `dir` whose error estimate fits its share of the budget, and the coefficients coef[j] =
+// [exp(-i dir hs T) e_1]_j * nrm[1] (j = 1..me) of the result in the Lanczos basis.
+struct StepChoice {
+    int me;
+    double hs;
+    double err;
+    bool noconv;
+};
+
+StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, double tol, double len, double remaining,
+                       double eps_break, bool last_allowed, double2* coef) {
+    StepChoice ch{};
+    const int me = effective_dim(m, alpha, nrm, eps_break);
+    SmallExp se;
+    se.m = me;
+    se.dir = dir;
+    se.beta_next = me < m ? 0.0 : nrm[m + 1];
+    std::vector<double> A((size_t)me * me, 0.0);
+    for (int j = 1; j <= me; ++j) {
+        A[(size_t)(j - 1) * me + (j - 1)] = alpha[j];
+        if (j < me) A[(size_t)(j - 1) * me + j] = A[(size_t)j * me + (j - 1)] = nrm[j + 1];
+    }
+    jacobi_eig(me, A, se.theta, se.Q);
+    // longest sub-step whose error estimate fits its share of the budget
+    auto fits = [&](double hs) { return se.err(hs) <= tol * hs / len; };
+    double hs = remaining;
+    if (!fits(hs)) {
+        if (last_allowed) {
+            ch.noconv = true;   // forced: take the remainder in one step
+        } else {
+            double lo = 0.0, hi = remaining;
+            for (int it = 0; it < 60; ++it) {
+                const double mid = 0.5 * (lo + hi);
+                if (fits(mid)) lo = mid; else hi = mid;
+            }
+            hs = lo;
+            if (!(hs > 1e-9 * len)) {   // estimate never fits: Krylov space too small for this tolerance
+                ch.noconv = true;
+                hs = std::min(remaining, std::max(hi, 1e-6 * len));
+            }
+        }
+    }
+    ch.me = me;
+    ch.hs = hs;
+    ch.err = se.err(hs);
+    for (int j = 1; j <= me; ++j) {
+        const cplx v = se.comp(j - 1, hs) * nrm[1];
+        coef[j] = make_double2(v.real(), v.imag());
+    }
+    return ch;
+}
+
 bool valid_args(const syk_ham* h, int dtype, const void* psi, const void* work) {
     return h && (dtype == SYK_C64 || dtype == SYK_C128) && psi && work && ((uintptr_t)psi & 15) == 0 &&
            ((uintptr_t)work & 15) == 0;
@@ -211,46 +265,15 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
         SYK_TRY(launch_finalize_nrm(m + 1, c.sc, st));
         SYK_TRY(fetch_scalars(c, m, alpha.data(), nrm.data()));
         if (!(nrm[1] > 0.0)) return SYK_OK;   // zero vector stays zero
-        const int me = effective_dim(m, alpha.data(), nrm.data(), eps_break);
-
-        SmallExp se;
-        se.m = me;
-        se.dir = dir;
-        se.beta_next = me < m ? 0.0 : nrm[m + 1];
-        A.assign((size_t)me * me, 0.0);
-        for (int j = 1; j <= me; ++j) {
-            A[(size_t)(j - 1) * me + (j - 1)] = alpha[j];
-            if (j < me) A[(size_t)(j - 1) * me + j] = A[(size_t)j * me + (j - 1)] = nrm[j + 1];
-        }
-        jacobi_eig(me, A, se.theta, se.Q);
-
-        // longest sub-step whose error estimate fits its share of the budget
-        auto fits = [&](double hs) { return se.err(hs) <= tol * hs / len; };
-        double hs = remaining;
-        if (!fits(hs)) {
-            if (n_sub >= max_sub) {
-                rc = SYK_ENOCONV;   // forced: take the remainder in one step
-            } else {
-                double lo = 0.0, hi = remaining;
-                for (int it = 0; it < 60; ++it) {
-                    const double mid = 0.5 * (lo + hi);
-                    if (fits(mid)) lo = mid; else hi = mid;
-                }
-                hs = lo;
-                if (!(hs > 1e-9 * len)) {   // estimate never fits: Krylov space too small for this tolerance
-                    rc = SYK_ENOCONV;
-                    hs = std::min(remaining, std::max(hi, 1e-6 * len));
-                }
-            }
-        }
+        const StepChoice ch = choose_step(m, alpha.data(), nrm.data(), dir, tol, len, remaining, eps_break,
+                                          n_sub >= max_sub, coef.data());
+        const int me = ch.me;
+        const double hs = ch.hs;
+        if (ch.noconv) rc = SYK_ENOCONV;
         if (stats) {
-            stats->err_est += se.err(hs);
+            stats->err_est += ch.err;
             stats->krylov_dim_used = stats->krylov_dim_used == 0 ? me : std::min(stats->krylov_dim_used, me);
             stats->n_substeps += 1;
-        }
-        for (int j = 1; j <= me; ++j) {
-            const cplx v = se.comp(j - 1, hs) * nrm[1];
-            coef[j] = make_double2(v.real(), v.imag());
         }
         SYK_CUDA(cudaMemcpyAsync(c.sc->coef, coef.data(), sizeof(double2) * (size_t)(me + 1), cudaMemcpyHostToDevice, st));
         if (!two_pass) {
@@ -270,9 +293,151 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
     return rc;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Batched over disorder realizations (BASELINE configs[1]): every kernel runs with grid.y = realization,
+// so the nb realizations advance through the Lanczos recurrence in lock step and share launches; the host does the nb
+// small exponentials between two rounds.  One-pass only.  Work space: table descriptors | nb x (scalars header + m
+// vectors).  A realization that has reached its target time keeps coef = identity (psi unchanged) while the others
+// finish.
+// ---------------------------------------------------------------------------------------------------------
+int resolve_krylov_dim(const syk_ham* h, const syk_krylov_opts* o) { return resolve_dim(h, o); }
+
+size_t krylov_batched_bytes(const syk_ham* h0, int nb, int dtype, int m) {
+    const size_t v = ((size_t)1 << h0->L) * elem_bytes(dtype);
+    return batched_table_bytes(nb) + (size_t)nb * (krylov_header_bytes() + (size_t)m * v);
+}
+
+int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, void* d_psi, size_t psi_stride_bytes,
+                               double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work,
+                               size_t work_bytes, syk_stats* stats, bool* tables_uploaded, cudaStream_t st) {
+    const syk_ham* h0 = hams[0];
+    const int m = resolve_dim(h0, opts);
+    const double tol = (opts && opts->tol > 0) ? opts->tol : (dtype == SYK_C128 ? 1e-12 : 1e-6);
+    const int max_sub = (opts && opts->max_substeps > 0) ? opts->max_substeps : 100000;
+    const uint64_t D = 1ull << h0->L;
+    const size_t vbytes = (size_t)D * elem_bytes(dtype);
+    const size_t ws_stride = krylov_header_bytes() + (size_t)m * vbytes;
+    if (work_bytes < krylov_batched_bytes(h0, nb, dtype, m)) return SYK_ENOMEM;
+    char* tab = (char*)d_work;
+    char* ws = tab + batched_table_bytes(nb);                 // realization r: header at ws + r ws_stride, then m vectors
+    char* vecs = ws + krylov_header_bytes();
+    char* psi = (char*)d_psi;
+    const double len = std::hypot(tau_re, tau_im);
+    if (len == 0.0) return SYK_OK;
+    const cplx dir(tau_re / len, tau_im / len);
+    const double eps_break = dtype == SYK_C128 ? 1e-13 : 2e-6;
+    // buffer of u_j: j == 1 -> psi (user stride), else work vector j-2 (work-space stride)
+    auto buf = [&](int j) { return j == 1 ? psi : vecs + (size_t)(j - 2) * vbytes; };
+    auto stride = [&](int j) { return j == 1 ? psi_stride_bytes : ws_stride; };
+
+    std::vector<double> remaining((size_t)nb, len);
+    std::vector<double> alpha((size_t)nb * (kMaxKrylov + 2)), nrm((size_t)nb * (kMaxKrylov + 2));
+    std::vector<double2> coef((size_t)nb * (kMaxKrylov + 2));
+    std::vector<int> meff((size_t)nb, 1);
+    const size_t row = sizeof(double) * (kMaxKrylov + 2);
+    int rc = SYK_OK;
+    for (int n_sub = 1;; ++n_sub) {
+        bool any = false;
+        for (int r = 0; r < nb; ++r) any |= remaining[(size_t)r] > 1e-15 * len;
+        if (!any) break;
+        Batch b;
+        b.n = nb;
+        b.s.sc = ws_stride;
+        b.s.a = psi_stride_bytes;
+        SYK_TRY(launch_norm2(dtype, D, psi, (LanczosScalars*)ws, st, b));
+        for (int j = 1; j <= m; ++j) {
+            SYK_TRY(launch_apply_h_batched(hams, nb, dtype, tab, !*tables_uploaded, buf(j), stride(j), buf(j + 1),
+                                           stride(j + 1), j > 1 ? buf(j - 1) : nullptr, j > 1 ? stride(j - 1) : 0, ws,
+                                           ws_stride, j, st));
+            *tables_uploaded = true;
+            Batch ba;
+            ba.n = nb;
+            ba.s.a = stride(j + 1);
+            ba.s.b = stride(j);
+            ba.s.sc = ws_stride;
+            SYK_TRY(launch_axpy_norm(dtype, D, buf(j + 1), buf(j), j, (LanczosScalars*)ws, nullptr, 0, st, ba));
+            if (stats) stats->n_matvec += nb;
+        }
+        Batch bf;
+        bf.n = nb;
+        bf.s.sc = ws_stride;
+        SYK_TRY(launch_finalize_nrm(m + 1, (LanczosScalars*)ws, st, bf));
+        SYK_CUDA(cudaMemcpy2DAsync(alpha.data(), row, ws + offsetof(LanczosScalars, alpha), ws_stride, row, (size_t)nb,
+                                   cudaMemcpyDeviceToHost, st));
+        SYK_CUDA(cudaMemcpy2DAsync(nrm.data(), row, ws + offsetof(LanczosScalars, nrm), ws_stride, row, (size_t)nb,
+                                   cudaMemcpyDeviceToHost, st));
+        SYK_CUDA(cudaStreamSynchronize(st));
+        for (int r = 0; r < nb; ++r) {
+            const double* a = alpha.data() + (size_t)r * (kMaxKrylov + 2);
+            const double* nr = nrm.data() + (size_t)r * (kMaxKrylov + 2);
+            double2* cf = coef.data() + (size_t)r * (kMaxKrylov + 2);
+            for (int j = 0; j < kMaxKrylov + 2; ++j) cf[j] = make_double2(0.0, 0.0);
+            meff[(size_t)r] = 1;
+            if (!(remaining[(size_t)r] > 1e-15 * len) || !(nr[1] > 0.0)) {
+                cf[1] = make_double2(nr[1], 0.0);   // identity: psi stays what it is
+                remaining[(size_t)r] = 0.0;
+                continue;
+            }
+            const StepChoice ch = choose_step(m, a, nr, dir, tol, len, remaining[(size_t)r], eps_break,
+                                              n_sub >= max_sub, cf);
+            if (ch.noconv) rc = SYK_ENOCONV;
+            meff[(size_t)r] = ch.me;
+            remaining[(size_t)r] -= ch.hs;
+            if (stats) {
+                stats->err_est = std::max(stats->err_est, ch.err);
+                stats->krylov_dim_used = stats->krylov_dim_used == 0 ? ch.me : std::min(stats->krylov_dim_used, ch.me);
+            }
+        }
+        if (stats) {
+            stats->n_substeps += 1;
+            const double V = (double)vbytes;
+            for (int r = 0; r < nb; ++r)
+                stats->model_bytes += m * (((double)hams[r]->n_groups() + 3.0) * V + 3.0 * V) + V + (m + 1.0) * V;
+        }
+        SYK_CUDA(cudaMemcpy2DAsync(ws + offsetof(LanczosScalars, coef), ws_stride, coef.data(),
+                                   sizeof(double2) * (kMaxKrylov + 2), sizeof(double2) * (kMaxKrylov + 2), (size_t)nb,
+                                   cudaMemcpyHostToDevice, st));
+        SYK_CUDA(cudaMemcpy2DAsync(ws + offsetof(LanczosScalars, m_eff), ws_stride, meff.data(), sizeof(int), sizeof(int),
+                                   (size_t)nb, cudaMemcpyHostToDevice, st));
+        Batch bc;
+        bc.n = nb;
+        bc.s.a = psi_stride_bytes;
+        bc.s.b = ws_stride;
+        bc.s.sc = ws_stride;
+        SYK_TRY(launch_combine(dtype, D, psi, vecs, D, -1, (LanczosScalars*)ws, st, bc));
+        SYK_CUDA(cudaStreamSynchronize(st));   // coef / meff host buffers are reused in the next round
+    }
+    return rc;
+}
+
 }  // namespace syk
 
 extern "C" {
+
+int syk_krylov_workspace_bytes_batched(const syk_ham* h, int n_batch, int dtype, const syk_krylov_opts* opts,
+                                       size_t* bytes) {
+    if (!h || !bytes || n_batch < 1 || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->two_pass)) return SYK_EINVAL;
+    *bytes = syk::krylov_batched_bytes(h, n_batch, dtype, syk::resolve_dim(h, opts));
+    return SYK_OK;
+}
+
+int syk_krylov_evolve_batched(const syk_ham* const* hams, int n_batch, int dtype, void* d_psi, int64_t batch_stride,
+                              double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
+                              syk_stats* stats, void* stream) {
+    if (!hams || n_batch < 1 || !hams[0] || !syk::valid_args(hams[0], dtype, d_psi, d_work) || !std::isfinite(tau_re) ||
+        !std::isfinite(tau_im))
+        return SYK_EINVAL;
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->tol < 0 || opts->max_substeps < 0 || opts->two_pass))
+        return SYK_EINVAL;
+    if (batch_stride < ((int64_t)1 << hams[0]->L) || ((size_t)batch_stride * syk::elem_bytes(dtype)) % 16) return SYK_EINVAL;
+    if (!syk::batched_apply_ok(hams, n_batch, dtype)) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    bool uploaded = false;
+    return syk::krylov_evolve_batched_impl(hams, n_batch, dtype, d_psi, (size_t)batch_stride * syk::elem_bytes(dtype),
+                                           tau_re, tau_im, opts, d_work, work_bytes, stats, &uploaded,
+                                           (cudaStream_t)stream);
+}
 
 int syk_krylov_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes) {
     if (!h || !bytes || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;

@@ -10,6 +10,8 @@
 //   for each t_k:  l <- E(dt) l ; phi <- E(dt) phi
 //                  r <- g_W phi ; r <- E(-t - ib/4) r ; r <- g_V r ; r <- E(t - ib/4) r ; r <- g_W r ;  F_k = <l|r>
 // Resident vectors: l, phi, r + Krylov work (2 in two-pass mode: 5 in total, PAPER.md:249's v+3 with v = 2).
+#include <vector>
+
 #include "common.h"
 
 namespace syk {
@@ -121,6 +123,79 @@ static int green_one(const Space& sp, int dtype, int n, double beta, const doubl
     return rc_soft;
 }
 
+// The OTOC pipeline of otoc_one with every kernel batched over the realizations (grid.y) and the realizations advancing
+// through each evolution in lock step.  Work space: phi[nb] | r[nb] | batched Krylov work space.
+static size_t otoc_batched_bytes(const syk_ham* h0, int nb, int dtype, const syk_krylov_opts* opts) {
+    const size_t v = ((size_t)1 << h0->L) * elem_bytes(dtype);
+    return 2 * (size_t)nb * v + krylov_batched_bytes(h0, nb, dtype, resolve_krylov_dim(h0, opts));
+}
+
+static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int i_W, int j_V, double beta,
+                             const double* t_grid, int n_t, void* d_psi, size_t psi_stride, double* F_out,
+                             const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
+                             cudaStream_t st) {
+    const syk_ham* h0 = hams[0];
+    const uint64_t D = 1ull << h0->L;
+    const size_t v = (size_t)D * elem_bytes(dtype);
+    const int m = resolve_krylov_dim(h0, opts);
+    if (work_bytes < otoc_batched_bytes(h0, nb, dtype, opts)) return SYK_ENOMEM;
+    char* l = (char*)d_psi;
+    char* phi = (char*)d_work;
+    char* r = phi + (size_t)nb * v;
+    char* kwork = r + (size_t)nb * v;
+    const size_t kbytes = krylov_batched_bytes(h0, nb, dtype, m);
+    const size_t ws_stride = krylov_header_bytes() + (size_t)m * v;
+    LanczosScalars* sc = (LanczosScalars*)(kwork + batched_table_bytes(nb));   // realization 0's header
+    const int N = h0->N, gn = h0->gamma_norm;
+    bool uploaded = false;
+    int rc_soft = SYK_OK;
+    auto evolve = [&](void* vec, size_t stride, double tre, double tim) -> int {
+        int rc = krylov_evolve_batched_impl(hams, nb, dtype, vec, stride, tre, tim, opts, kwork, kbytes, stats, &uploaded,
+                                            st);
+        if (rc == SYK_ENOCONV) {
+            rc_soft = rc;
+            return SYK_OK;
+        }
+        return rc;
+    };
+    auto gamma = [&](int n, const void* in, size_t s_in, void* out, size_t s_out) -> int {
+        Batch b;
+        b.n = nb;
+        b.s.a = s_in;
+        b.s.b = s_out;
+        return launch_gamma(N, n, gn, dtype, in, out, st, b);
+    };
+    std::vector<double> dots((size_t)2 * nb);
+    SYK_TRY(evolve(l, psi_stride, 0.0, -beta / 8.0));
+    SYK_TRY(gamma(j_V, l, psi_stride, phi, v));
+    SYK_TRY(evolve(phi, v, 0.0, -beta / 4.0));
+    double t_prev = 0.0;
+    for (int k = 0; k < n_t; ++k) {
+        const double t = t_grid[k], dt = t - t_prev;
+        if (dt > 0.0) {
+            SYK_TRY(evolve(l, psi_stride, dt, 0.0));
+            SYK_TRY(evolve(phi, v, dt, 0.0));
+        }
+        t_prev = t;
+        SYK_TRY(gamma(i_W, phi, v, r, v));
+        SYK_TRY(evolve(r, v, -t, -beta / 4.0));
+        SYK_TRY(gamma(j_V, r, v, r, v));
+        SYK_TRY(evolve(r, v, t, -beta / 4.0));
+        SYK_TRY(gamma(i_W, r, v, r, v));
+        Batch b;
+        b.n = nb;
+        b.s.a = psi_stride;
+        b.s.b = v;
+        b.s.sc = ws_stride;
+        SYK_TRY(cdot_batched(dtype, D, l, r, sc, b, dots.data(), st));
+        for (int rr = 0; rr < nb; ++rr) {
+            F_out[((size_t)rr * n_t + k) * 2] = dots[2 * (size_t)rr];
+            F_out[((size_t)rr * n_t + k) * 2 + 1] = dots[2 * (size_t)rr + 1];
+        }
+    }
+    return rc_soft;
+}
+
 static Space full_space(const syk_ham* h) { return Space{{h, h}, -1, h->N, h->gamma_norm}; }
 
 // the two blocks of one Hamiltonian: same N, same normalisation, sectors 0 and 1
@@ -200,11 +275,33 @@ int syk_green_block(const syk_ham* h_even, const syk_ham* h_odd, int sector, int
                           (cudaStream_t)stream);
 }
 
+int syk_otoc_batched_workspace_bytes(const syk_ham* h, int n_batch, int dtype, const syk_krylov_opts* opts,
+                                     size_t* bytes) {
+    if (!h || !bytes || n_batch < 1 || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1)) return SYK_EINVAL;
+    *bytes = syk::otoc_batched_bytes(h, n_batch, dtype, opts);
+    return SYK_OK;
+}
+
 int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W, int j_V, double beta,
                      const double* t_grid, int n_t, void* d_psi, int64_t batch_stride, double* F_out,
                      const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream) {
     if (!hams || n_batch < 0) return SYK_EINVAL;
     if (stats) *stats = syk_stats{};
+    // lock-step batched pipeline when the realizations qualify (small N, tables in shared memory, one-pass) and the work
+    // space is large enough for it (syk_otoc_batched_workspace_bytes); else one realization after the other
+    if (n_batch >= 2 && hams[0] && !(opts && opts->two_pass) && syk::batched_apply_ok(hams, n_batch, dtype) &&
+        work_bytes >= syk::otoc_batched_bytes(hams[0], n_batch, dtype, opts)) {
+        for (int r = 0; r < n_batch; ++r) {
+            if (hams[r]->block_of_N || batch_stride < ((int64_t)1 << hams[r]->L)) return SYK_EINVAL;
+            char* psi = (char*)d_psi + (size_t)r * (size_t)batch_stride * syk::elem_bytes(dtype);
+            if (!syk::otoc_args_ok(hams[r], dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out, d_work)) return SYK_EINVAL;
+        }
+        if (((size_t)batch_stride * syk::elem_bytes(dtype)) % 16) return SYK_EINVAL;
+        return syk::otoc_batched_impl(hams, n_batch, dtype, i_W, j_V, beta, t_grid, n_t, d_psi,
+                                      (size_t)batch_stride * syk::elem_bytes(dtype), F_out, opts, d_work, work_bytes, stats,
+                                      (cudaStream_t)stream);
+    }
     int rc_soft = SYK_OK;
     for (int r = 0; r < n_batch; ++r) {
         if (!hams[r] || hams[r]->N != hams[0]->N || batch_stride < ((int64_t)1 << hams[r]->L)) return SYK_EINVAL;

@@ -8,6 +8,8 @@
 // partial -> fixed-order sum of partials; no atomics, bitwise reproducible.
 //
 // Vectors are processed in 16-byte units (one complex128 or two complex64) with grid-stride loops.
+#include <cstddef>
+
 #include "device_utils.cuh"
 
 namespace syk {
@@ -54,13 +56,21 @@ inline int grid_for(uint64_t units) {
     return (int)(blocks < cap ? blocks : cap);
 }
 
+// Batched launches (grid.y = realization): argument k of realization r lives at base_k + r * stride_k bytes.
+template <typename P>
+__device__ __forceinline__ P* at_batch(P* p, size_t stride) {
+    return p ? reinterpret_cast<P*>(reinterpret_cast<uintptr_t>(p) + (size_t)blockIdx.y * stride) : p;
+}
+
 #define GRID_STRIDE(i, n) \
     for (uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x; i < (n); i += (uint64_t)gridDim.x * kThreads)
 
 template <typename T>
 __global__ void __launch_bounds__(kThreads) norm2_kernel(const typename Unit<T>::V* __restrict__ v, uint64_t n,
-                                                         LanczosScalars* sc) {
+                                                         LanczosScalars* sc, BatchStride bs) {
     __shared__ double red[40];
+    v = at_batch(v, bs.a);
+    sc = at_batch(sc, bs.sc);
     double s = 0.0;
     GRID_STRIDE(i, n) {
         double a[4];
@@ -80,8 +90,12 @@ template <typename T, bool WITH_Y>
 __global__ void __launch_bounds__(kThreads) axpy_norm_kernel(typename Unit<T>::V* __restrict__ w,
                                                              const typename Unit<T>::V* __restrict__ u,
                                                              typename Unit<T>::V* y, uint64_t n, int j, int first_y,
-                                                             LanczosScalars* sc) {
+                                                             LanczosScalars* sc, BatchStride bs) {
     __shared__ double red[40];
+    w = at_batch(w, bs.a);
+    u = at_batch(u, bs.b);
+    y = at_batch(y, bs.c);
+    sc = at_batch(sc, bs.sc);
     const double nj = sc->nrm[j];
     const double dotsum = reduce_partials(sc->partial_dot, sc->n_partial_dot, red);
     const double alpha = nj > 0.0 ? dotsum / nj : 0.0;
@@ -130,8 +144,9 @@ __global__ void __launch_bounds__(kThreads) axpy_norm_kernel(typename Unit<T>::V
     }
 }
 
-__global__ void __launch_bounds__(kThreads) finalize_nrm_kernel(int j, LanczosScalars* sc) {
+__global__ void __launch_bounds__(kThreads) finalize_nrm_kernel(int j, LanczosScalars* sc, BatchStride bs) {
     __shared__ double red[40];
+    sc = at_batch(sc, bs.sc);
     const double n2 = reduce_partials(sc->partial_nrm, sc->n_partial_nrm, red);
     if (threadIdx.x == 0) sc->nrm[j] = sqrt(n2);
 }
@@ -140,8 +155,12 @@ __global__ void __launch_bounds__(kThreads) finalize_nrm_kernel(int j, LanczosSc
 template <typename T>
 __global__ void __launch_bounds__(kThreads) combine_kernel(typename Unit<T>::V* psi, const typename Unit<T>::V* vecs,
                                                            uint64_t stride, uint64_t n, int m,
-                                                           const LanczosScalars* __restrict__ sc) {
+                                                           const LanczosScalars* __restrict__ sc, BatchStride bs) {
     __shared__ double cr[kMaxKrylov + 2], ci[kMaxKrylov + 2];
+    psi = at_batch(psi, bs.a);
+    vecs = at_batch(vecs, bs.b);
+    sc = at_batch(sc, bs.sc);
+    if (m < 0) m = sc->m_eff;   // batched: every realization has its own effective Krylov dimension
     for (int j = 1 + threadIdx.x; j <= m; j += kThreads) {
         const double nj = sc->nrm[j];
         const double inv = nj > 0.0 ? 1.0 / nj : 0.0;
@@ -205,8 +224,11 @@ __global__ void __launch_bounds__(kThreads) axpy_coef_kernel(typename Unit<T>::V
 template <typename T>
 __global__ void __launch_bounds__(kThreads) cdot_kernel(const typename Unit<T>::V* __restrict__ a,
                                                         const typename Unit<T>::V* __restrict__ b, uint64_t n,
-                                                        LanczosScalars* sc) {
+                                                        LanczosScalars* sc, BatchStride bs) {
     __shared__ double red[40];
+    a = at_batch(a, bs.a);
+    b = at_batch(b, bs.b);
+    sc = at_batch(sc, bs.sc);
     double sr = 0.0, si = 0.0;
     GRID_STRIDE(i, n) {
         double av[4], bv[4];
@@ -224,6 +246,20 @@ __global__ void __launch_bounds__(kThreads) cdot_kernel(const typename Unit<T>::
         sc->partial_cdot[blockIdx.x] = make_double2(sr, si);
         if (blockIdx.x == 0) sc->n_partial_cdot = gridDim.x;
     }
+}
+
+// coef[0] <- sum of the complex partials (fixed order): the result slot of a batched inner product
+__global__ void __launch_bounds__(kThreads) finalize_cdot_kernel(LanczosScalars* sc, BatchStride bs) {
+    __shared__ double red[40];
+    sc = at_batch(sc, bs.sc);
+    double sr = 0.0, si = 0.0;
+    for (int i = threadIdx.x; i < sc->n_partial_cdot; i += kThreads) {
+        sr += sc->partial_cdot[i].x;
+        si += sc->partial_cdot[i].y;
+    }
+    sr = block_sum(sr, red);
+    si = block_sum(si, red);
+    if (threadIdx.x == 0) sc->coef[0] = make_double2(sr, si);
 }
 
 // v <- v / sqrt(sum partial_nrm)
@@ -270,8 +306,10 @@ __global__ void __launch_bounds__(kThreads) random_fill_kernel(typename Cx<T>::t
 //   gamma_{2q}   = s Z^{bit-1} X^{bit};  gamma_{2q+1} = -i s Z^{2 bit - 1} X^{bit}   (R-JW, R-SIGN)
 template <typename T>
 __global__ void __launch_bounds__(kThreads) gamma_kernel(const typename Cx<T>::type* in, typename Cx<T>::type* out,
-                                                         uint64_t half, int q, int odd, T s) {
+                                                         uint64_t half, int q, int odd, T s, BatchStride bs) {
     using C = typename Cx<T>::type;
+    in = at_batch(in, bs.a);
+    out = at_batch(out, bs.b);
     const uint64_t bit = 1ull << q;
     const uint32_t zmask = (uint32_t)(odd ? ((bit << 1) - 1) : (bit - 1));
     GRID_STRIDE(pidx, half) {
@@ -327,47 +365,49 @@ __global__ void __launch_bounds__(kThreads) gamma_top_kernel(const typename Cx<T
 
 }  // namespace
 
-int launch_norm2(int dtype, uint64_t D, const void* v, LanczosScalars* sc, cudaStream_t st) {
+int launch_norm2(int dtype, uint64_t D, const void* v, LanczosScalars* sc, cudaStream_t st, const Batch& bt) {
     const uint64_t n = n_units(dtype, D);
     const int g = grid_for(n);
-    DISPATCH(dtype, (norm2_kernel<double><<<g, kThreads, 0, st>>>((const double2*)v, n, sc)),
-             (norm2_kernel<float><<<g, kThreads, 0, st>>>((const float4*)v, n, sc)));
+    const dim3 gb(g, bt.n);
+    DISPATCH(dtype, (norm2_kernel<double><<<gb, kThreads, 0, st>>>((const double2*)v, n, sc, bt.s)),
+             (norm2_kernel<float><<<gb, kThreads, 0, st>>>((const float4*)v, n, sc, bt.s)));
     return SYK_OK;
 }
 
 int launch_axpy_norm(int dtype, uint64_t D, void* w, const void* u, int j, LanczosScalars* sc, void* y, int first_y,
-                     cudaStream_t st) {
+                     cudaStream_t st, const Batch& bt) {
     const uint64_t n = n_units(dtype, D);
-    const int g = grid_for(n);
+    const dim3 g(grid_for(n), bt.n);
     if (y) {
         DISPATCH(dtype,
                  (axpy_norm_kernel<double, true><<<g, kThreads, 0, st>>>((double2*)w, (const double2*)u, (double2*)y, n,
-                                                                        j, first_y, sc)),
+                                                                        j, first_y, sc, bt.s)),
                  (axpy_norm_kernel<float, true><<<g, kThreads, 0, st>>>((float4*)w, (const float4*)u, (float4*)y, n, j,
-                                                                       first_y, sc)));
+                                                                       first_y, sc, bt.s)));
     } else {
         DISPATCH(dtype,
                  (axpy_norm_kernel<double, false><<<g, kThreads, 0, st>>>((double2*)w, (const double2*)u, nullptr, n, j,
-                                                                         0, sc)),
+                                                                         0, sc, bt.s)),
                  (axpy_norm_kernel<float, false><<<g, kThreads, 0, st>>>((float4*)w, (const float4*)u, nullptr, n, j, 0,
-                                                                        sc)));
+                                                                        sc, bt.s)));
     }
     return SYK_OK;
 }
 
-int launch_finalize_nrm(int j, LanczosScalars* sc, cudaStream_t st) {
-    finalize_nrm_kernel<<<1, kThreads, 0, st>>>(j, sc);
+int launch_finalize_nrm(int j, LanczosScalars* sc, cudaStream_t st, const Batch& bt) {
+    finalize_nrm_kernel<<<dim3(1, bt.n), kThreads, 0, st>>>(j, sc, bt.s);
     count_launch();
     SYK_CUDA(cudaGetLastError());
     return SYK_OK;
 }
 
 int launch_combine(int dtype, uint64_t D, void* psi, const void* vecs, uint64_t stride_elems, int m,
-                   LanczosScalars* sc, cudaStream_t st) {
+                   LanczosScalars* sc, cudaStream_t st, const Batch& bt) {
     const uint64_t n = n_units(dtype, D), stride = n_units(dtype, stride_elems);
-    const int g = grid_for(n);
-    DISPATCH(dtype, (combine_kernel<double><<<g, kThreads, 0, st>>>((double2*)psi, (const double2*)vecs, stride, n, m, sc)),
-             (combine_kernel<float><<<g, kThreads, 0, st>>>((float4*)psi, (const float4*)vecs, stride, n, m, sc)));
+    const dim3 g(grid_for(n), bt.n);
+    DISPATCH(dtype,
+             (combine_kernel<double><<<g, kThreads, 0, st>>>((double2*)psi, (const double2*)vecs, stride, n, m, sc, bt.s)),
+             (combine_kernel<float><<<g, kThreads, 0, st>>>((float4*)psi, (const float4*)vecs, stride, n, m, sc, bt.s)));
     return SYK_OK;
 }
 
@@ -380,11 +420,13 @@ int launch_axpy_coef(int dtype, uint64_t D, void* y, const void* u, int j, int f
     return SYK_OK;
 }
 
-int launch_cdot(int dtype, uint64_t D, const void* a, const void* b, LanczosScalars* sc, cudaStream_t st) {
+int launch_cdot(int dtype, uint64_t D, const void* a, const void* b, LanczosScalars* sc, cudaStream_t st,
+                const Batch& bt) {
     const uint64_t n = n_units(dtype, D);
     const int g = grid_for(n);
-    DISPATCH(dtype, (cdot_kernel<double><<<g, kThreads, 0, st>>>((const double2*)a, (const double2*)b, n, sc)),
-             (cdot_kernel<float><<<g, kThreads, 0, st>>>((const float4*)a, (const float4*)b, n, sc)));
+    const dim3 gb(g, bt.n);
+    DISPATCH(dtype, (cdot_kernel<double><<<gb, kThreads, 0, st>>>((const double2*)a, (const double2*)b, n, sc, bt.s)),
+             (cdot_kernel<float><<<gb, kThreads, 0, st>>>((const float4*)a, (const float4*)b, n, sc, bt.s)));
     return SYK_OK;
 }
 
@@ -406,14 +448,15 @@ int launch_random_fill(int N, uint64_t seed, uint32_t realization, int dtype, vo
     return SYK_OK;
 }
 
-int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* in, void* out, cudaStream_t st) {
+int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* in, void* out, cudaStream_t st, const Batch& bt) {
     const uint64_t half = 1ull << (N / 2 - 1);
-    const int g = grid_for(half);
+    const dim3 g(grid_for(half), bt.n);
     const double s = gamma_norm == SYK_GAMMA_HALF ? 0.70710678118654752440 : 1.0;
     DISPATCH(dtype,
-             (gamma_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, half, n >> 1, n & 1, s)),
+             (gamma_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, half, n >> 1, n & 1, s,
+                                                          bt.s)),
              (gamma_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, half, n >> 1, n & 1,
-                                                         (float)s)));
+                                                         (float)s, bt.s)));
     return SYK_OK;
 }
 
@@ -427,6 +470,19 @@ int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, 
     if (mode == 1 && sector_out) s = -s;
     DISPATCH(dtype, (gamma_top_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, Dr, mode, s)),
              (gamma_top_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, Dr, mode, (float)s)));
+    return SYK_OK;
+}
+
+// Batched inner products: results[r] = <a_r|b_r>; synchronises the stream.
+int cdot_batched(int dtype, uint64_t D, const void* a, const void* b, LanczosScalars* sc, const Batch& bt, double* re_im,
+                 cudaStream_t st) {
+    SYK_TRY(launch_cdot(dtype, D, a, b, sc, st, bt));
+    finalize_cdot_kernel<<<dim3(1, bt.n), kThreads, 0, st>>>(sc, bt.s);
+    count_launch();
+    SYK_CUDA(cudaGetLastError());
+    SYK_CUDA(cudaMemcpy2DAsync(re_im, sizeof(double2), (const char*)sc + offsetof(LanczosScalars, coef), bt.s.sc,
+                               sizeof(double2), (size_t)bt.n, cudaMemcpyDeviceToHost, st));
+    SYK_CUDA(cudaStreamSynchronize(st));
     return SYK_OK;
 }
 

@@ -729,3 +729,83 @@ def test_spin_chain_apply_and_evolve(B, torch, dt):
         assert relerr(d.cpu().numpy(), exact) <= TOL[dt], tau
     with pytest.raises(B.SykError):
         B.syk_otoc(h2, 0, 1, 1.0, [0.0], to_dev(torch, psi), work(torch, B.syk_otoc_workspace_bytes(h2, code, o)), o)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# lock-step batched realizations (BASELINE configs[1] shape)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_krylov_evolve_batched_vs_exact(B, torch, dt):
+    """grid.y = realization: five different sparse Hamiltonians (one of them a single term, which breaks down after
+    two Lanczos steps while the others need sub-steps) evolved in lock step, padded batch stride, each against its
+    own exact propagator; and against the one-by-one library call."""
+    N, nb = 24, 5
+    D = 1 << (N // 2)
+    stride = D + 64
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    qs, Js = [], []
+    for r in range(nb):
+        q, J = couplings(N, 4, seed=20 + r)
+        if r == 2:
+            q, J = q[:1], np.array([0.9])
+        qs.append(q)
+        Js.append(J)
+    hams = [B.syk_build_from_terms(N, q, J) for q, J in zip(qs, Js)]
+    psis = np.zeros((nb, stride), dtype=npdtype(dt))
+    for r in range(nb):
+        psis[r, :D] = (1.0 + 0.3 * r) * inputs.gaussian_state(D, 300 + r, npdtype(dt))
+    psis[:, D:] = 7.0                                                    # padding must stay untouched
+    o = {"krylov_dim": 10}
+    wk = work(torch, B.syk_krylov_workspace_bytes_batched(hams[0], nb, code, o))
+    for tau in ((6.0, 0.0), (1.5, -1.0)):
+        d = to_dev(torch, psis.reshape(-1))
+        st = B.syk_krylov_evolve_batched(hams, d, stride, tau[0], tau[1], wk, o)
+        out = d.cpu().numpy().reshape(nb, stride)
+        assert np.all(out[:, D:] == 7.0)
+        assert st["n_substeps"] >= (2 if dt == "c128" else 1) and st["krylov_dim_used"] == 2   # single-term member: breakdown
+        wk1 = work(torch, B.syk_krylov_workspace_bytes(hams[0], code, o))
+        for r in range(nb):
+            prop = oev.ExactPropagator(N, qs[r], Js[r])
+            ref = prop.apply(complex(*tau), psis[r, :D].astype(np.complex128))
+            assert relerr(out[r, :D], ref) <= TOL[dt], (r, tau)
+            d1 = to_dev(torch, psis[r, :D].copy())
+            B.syk_krylov_evolve(hams[r], d1, tau[0], tau[1], wk1, o)
+            assert relerr(out[r, :D], d1.cpu().numpy()) <= TOL[dt]
+    # conditions of the lock-step mode
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve_batched(hams, d, stride, 1.0, 0.0, wk, {"krylov_dim": 10, "two_pass": 1})
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve_batched(hams, d, D - 1, 1.0, 0.0, wk, o)
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve_batched(hams, d, stride, 1.0, 0.0, work(torch, 4096), o)
+    small = [B.syk_build_hamiltonian(12, 1.0, 0, r) for r in range(2)]       # vector smaller than a tile
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve_batched(small, d, 64, 1.0, 0.0, wk, o)
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_otoc_batched_lockstep_vs_oracle(B, torch, dt):
+    """syk_otoc_batched in lock-step mode (work space of syk_otoc_batched_workspace_bytes) at N=24: each realization
+    against its own exact oracle, and against the back-to-back mode of the same call."""
+    N, nb = 24, 4
+    D = 1 << (N // 2)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    p = inputs.bernoulli_p(N, 4)
+    t_grid = np.array([0.0, 0.6, 1.5, 1.5, 3.0])
+    hams = [B.syk_build_hamiltonian(N, p, 0, r) for r in range(nb)]
+    psis = np.stack([orng.random_state(N, 0, r) for r in range(nb)]).astype(npdtype(dt))
+    o = {"krylov_dim": 14}
+    wk = work(torch, B.syk_otoc_batched_workspace_bytes(hams[0], nb, code, o))
+    n0 = B.syk_launch_count(reset=True)
+    F, st = B.syk_otoc_batched(hams, N - 1, N - 2, 5.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk, o)
+    n_lock = B.syk_launch_count(reset=True)
+    wk1 = work(torch, B.syk_otoc_workspace_bytes(hams[0], code, o))
+    F1, st1 = B.syk_otoc_batched(hams, N - 1, N - 2, 5.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk1, o)
+    n_seq = B.syk_launch_count(reset=True)
+    assert n_lock * 2 < n_seq                                             # the batch shares its launches
+    for r in range(nb):
+        q, J, _ = orng.sample_couplings(N, p, 0, r)
+        ref = ootoc.otoc_same_psi(oev.ExactPropagator(N, q, J), N, N - 1, N - 2, 5.0, t_grid,
+                                  psis[r].astype(np.complex128))
+        assert np.max(np.abs(F[r] - ref)) / abs(ref[0]) <= TOL[dt], r
+        assert np.max(np.abs(F[r] - F1[r])) / abs(ref[0]) <= 2 * TOL[dt], r
