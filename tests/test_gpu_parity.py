@@ -809,3 +809,32 @@ def test_otoc_batched_lockstep_vs_oracle(B, torch, dt):
                                   psis[r].astype(np.complex128))
         assert np.max(np.abs(F[r] - ref)) / abs(ref[0]) <= TOL[dt], r
         assert np.max(np.abs(F[r] - F1[r])) / abs(ref[0]) <= 2 * TOL[dt], r
+
+
+def test_otoc_run_and_sweep_scripts(B, torch):
+    """The two user-facing drivers of the package run end to end (small sizes) and agree with direct library calls."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-m", "paper_2311_00639_b200.otoc_run", "--N", "20", "--k", "4", "--tmax", "2",
+                          "--nt", "3", "--krylov-dim", "12"], cwd=root, capture_output=True, text=True, check=True)
+    d = json.loads(out.stdout.strip().splitlines()[-1])
+    N = 20
+    h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 4), 0, 0)
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    psi = torch.empty(1 << (N // 2), dtype=torch.complex128, device="cuda")
+    B.syk_random_state(N, 0, 0, psi, scratch)
+    o = {"krylov_dim": 12}
+    F, _ = B.syk_otoc(h, N - 1, N - 2, 5.0, np.linspace(0.0, 2.0, 3), psi, work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o)), o)
+    assert np.allclose(np.array(d["F_re"]) + 1j * np.array(d["F_im"]), F, atol=1e-12)
+    assert d["ratio_re"][0] == 1.0 and d["n_matvec"] > 0
+    outb = subprocess.run([sys.executable, "-m", "paper_2311_00639_b200.otoc_run", "--N", "20", "--k", "4", "--tmax", "1",
+                           "--nt", "2", "--krylov-dim", "12", "--block", "--green"], cwd=root, capture_output=True,
+                          text=True, check=True)
+    db = json.loads(outb.stdout.strip().splitlines()[-1])
+    assert db["parity_blocks"] and db["what"] == "green" and abs(db["ratio_re"][0] - 1.0) < 1e-15
+    sw = subprocess.run([sys.executable, "-m", "paper_2311_00639_b200.sweep", "--quick"], cwd=root, capture_output=True,
+                        text=True, check=True)
+    assert "| (i) k=4 |" in sw.stdout and "Affine fit" in sw.stdout
