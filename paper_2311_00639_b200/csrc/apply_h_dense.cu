@@ -109,7 +109,7 @@ __device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_
             do {
                 const uint4 cur = e;
                 ++t;
-                e = ent[t < (uint32_t)kChunkEntries ? t : (uint32_t)kChunkEntries - 1u];
+                e = ent[t];   // t <= ne <= kChunkEntries - 1: always inside the buffer
                 const uint32_t sgn = (uint32_t)__popc(bt & cur.x) << 31;
                 T a;
                 if constexpr (sizeof(T) == 8) a = __hiloint2double((int)(cur.w ^ sgn), (int)cur.z);
@@ -165,7 +165,9 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnPara
             for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 for (int l = 0; l < n_loads; ++l) {
                     const uint32_t hi = __ldg(&p.loads[l].hi);
-                    mbar_wait(bar_empty + 8 * slot, phase ^ 1u);
+                    // a load is consumed over ~10^5 cycles of arithmetic: poll slowly, a spinning lane would only
+                    // take issue slots from the two consumer warps on its scheduler (23 % of all instructions, ncu)
+                    while (!mbar_try_wait(bar_empty + 8 * slot, phase ^ 1u)) __nanosleep(2000);
                     mbar_arrive_expect_tx(bar_full + 8 * slot, TILE_BYTES);
                     const unsigned char* src =
                         reinterpret_cast<const unsigned char*>(p.in + ((uint64_t)(tile ^ hi) << kTileLog2D));
@@ -319,13 +321,13 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
         const uint32_t x = (uint32_t)h->x[g];
         const uint32_t hi = x >> kTileLog2D;
         const uint32_t nt = h->group_off[g + 1] - h->group_off[g];
-        if (nt + 1 > (uint32_t)kChunkEntries) return SYK_EINVAL;   // a group must fit one chunk (dense N <= 64: 497)
+        if (nt + 1 > (uint32_t)kChunkEntries - 1) return SYK_EINVAL;   // a group must fit one chunk (dense N <= 64: 497)
         const bool new_load = loads.empty() || loads.back().hi != hi;
         if (new_load) {
             if (!loads.empty()) loads.back().c1 = (uint32_t)chunks.size();
             loads.push_back(DenseLoad{hi, (uint32_t)chunks.size(), 0u, 0u});
         }
-        if (new_load || chunks.back().ne + nt + 1 > (uint32_t)kChunkEntries)
+        if (new_load || chunks.back().ne + nt + 1 > (uint32_t)kChunkEntries - 1)   // one spare entry: read-ahead
             chunks.push_back(DenseChunk{(uint32_t)entries.size(), 0u, 0u, 0u});
         uint32_t flags = 0, occ = 0;
         const size_t header_at = entries.size();
