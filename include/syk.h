@@ -5,7 +5,9 @@
  *
  * Conventions common to every call
  *   - Every function returns an int: SYK_OK (0) or a negative error code.  Nothing throws, prints or exits.
- *   - N = number of Majorana fermions, even, 4 <= N <= 64.  L = N/2 qubits, D = 2^L amplitudes.
+ *   - N = number of Majorana fermions, even, 4 <= N <= 64.  L = N/2 qubits, D = 2^L amplitudes.  (N = 66 can be built
+ *     and cut into parity blocks of 32 qubits, which every call accepts; the full N = 66 handle itself only serves
+ *     syk_ham_info / syk_ham_tables / syk_build_parity_block.)
  *   - A state vector is a contiguous array of D complex numbers, interleaved (re, im); `dtype` says whether the
  *     components are float (SYK_C64, 8 bytes per amplitude) or double (SYK_C128, 16 bytes per amplitude).
  *     Basis index b = sum_q bit_q 2^q, qubit 0 = least significant bit (R-ENDIAN).

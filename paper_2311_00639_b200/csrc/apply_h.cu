@@ -516,6 +516,7 @@ int apply_h_kernel_kind(const syk_ham* h, int dtype) {
 
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
                    cudaStream_t stream) {
+    if (h->L > 32) return SYK_EINVAL;   // N = 66: only the parity blocks (32 qubits) can be applied
     SYK_TRY(ensure_device_tables(h));
     const int kind = apply_h_kernel_kind(h, dtype);
     profile_begin(stream);

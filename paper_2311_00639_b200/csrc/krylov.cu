@@ -205,7 +205,7 @@ StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, 
 }
 
 bool valid_args(const syk_ham* h, int dtype, const void* psi, const void* work) {
-    return h && (dtype == SYK_C64 || dtype == SYK_C128) && psi && work && ((uintptr_t)psi & 15) == 0 &&
+    return h && h->L <= 32 && (dtype == SYK_C64 || dtype == SYK_C128) && psi && work && ((uintptr_t)psi & 15) == 0 &&
            ((uintptr_t)work & 15) == 0;
 }
 
@@ -440,7 +440,7 @@ int syk_krylov_evolve_batched(const syk_ham* const* hams, int n_batch, int dtype
 }
 
 int syk_krylov_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes) {
-    if (!h || !bytes || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    if (!h || h->L > 32 || !bytes || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
     if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1)) return SYK_EINVAL;
     const int m = syk::resolve_dim(h, opts);
     const size_t v = ((size_t)1 << h->L) * syk::elem_bytes(dtype);

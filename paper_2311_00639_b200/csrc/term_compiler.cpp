@@ -106,7 +106,7 @@ bool make_term(int N, int gamma_norm, const int32_t* q, double J, RawTerm* t) {
 }
 
 bool valid_common(int N, int gamma_norm, syk_ham** out) {
-    return out && N >= 4 && N <= 64 && (N % 2) == 0 &&
+    return out && N >= 4 && N <= 66 && (N % 2) == 0 &&   // N = 66: only its parity blocks (32 qubits) can be applied
            (gamma_norm == SYK_GAMMA_PAULI || gamma_norm == SYK_GAMMA_HALF);
 }
 

@@ -519,7 +519,7 @@ static bool ok_vec(int N, int dtype, const void* p) {
 
 int syk_apply_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
                           void* stream) {
-    if (N < 6 || N > 64 || (N & 1) || n < 0 || n >= N || (dtype != SYK_C64 && dtype != SYK_C128) || !d_in || !d_out ||
+    if (N < 6 || N > 66 || (N & 1) || n < 0 || n >= N || (dtype != SYK_C64 && dtype != SYK_C128) || !d_in || !d_out ||
         (gamma_norm != SYK_GAMMA_PAULI && gamma_norm != SYK_GAMMA_HALF) || (sector_out != 0 && sector_out != 1))
         return SYK_EINVAL;
     if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return SYK_EINVAL;

@@ -168,3 +168,40 @@ def test_lockstep_pacing_does_not_change_results(B):
         B.syk_set_lockstep(-1, 0)
     with pytest.raises(B.SykError):
         B.syk_set_lockstep(4, 31)
+
+
+def test_apply_H_N66_parity_block_sampled(B):
+    """Beyond the paper's largest size (N = 64): N = 66 in one parity block (32 qubits, 2 x 34.4 GB in
+    complex64).  Outputs sampled at random reduced indices b' against the oracle's monomial rows of the FULL 33-qubit
+    term matrices (row b = b' | (parity(b') xor sector) << 32; the columns, all in the same sector, are read back
+    through their low 32 bits), plus the second-moment sum rule."""
+    import torch
+    if _free_gb() < 72:
+        pytest.skip("needs 72 GB of device memory")
+    N, sector = 66, 1
+    p = inputs.bernoulli_p(N, 2)
+    q, J, _ = orng.sample_couplings(N, p, 0, 0)
+    h = B.syk_build_hamiltonian(N, p, 0, 0)
+    hb = B.syk_build_parity_block(h, sector)
+    assert hb.info()["n_terms"] == len(J) and hb.info()["dim"] == 1 << 32
+    assert B.syk_apply_H_kernel_kind(hb, B.SYK_C64) == 3
+    Dr = 1 << 32
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    d_in = torch.empty(Dr, dtype=torch.complex64, device="cuda")
+    d_out = torch.empty(Dr, dtype=torch.complex64, device="cuda")
+    B.syk_random_state(N - 2, 0, 5, d_in, scratch)
+    B.syk_apply_H(hb, d_in, d_out)
+    torch.cuda.synchronize()
+    bp = inputs.sample_indices(Dr, 800, seed=23)
+    top = (ohm._popcount_parity(bp) ^ sector).astype(np.uint64)
+    full = bp | (top << np.uint64(32))
+    cols, vals = ohm.hamiltonian_rows(N, q, J, full)
+    assert np.all((ohm._popcount_parity(cols.reshape(-1)) & 1) == sector)          # H conserves parity
+    low = (cols & np.uint64(Dr - 1)).astype(np.int64).reshape(-1)
+    src = d_in[torch.from_numpy(low).cuda()].cpu().numpy().astype(np.complex128).reshape(cols.shape)
+    ref = (vals * src).sum(axis=0)
+    got = d_out[torch.from_numpy(bp.astype(np.int64)).cuda()].cpu().numpy().astype(np.complex128)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-5
+    n2 = B.syk_dot(N - 2, d_out, d_out, scratch).real
+    assert abs(n2 / float(np.sum(J ** 2)) - 1.0) <= 5e-3
+    assert abs(B.syk_dot(N - 2, d_in, d_out, scratch).imag) <= 1e-6

@@ -158,7 +158,7 @@ def test_argument_errors(B):
     f = B._lib.syk_build_hamiltonian
     assert f(7, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # odd N
     assert f(2, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # N < 4
-    assert f(66, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL      # N > 64
+    assert f(68, 0.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL      # N > 66 (66 only for parity blocks)
     assert f(8, 0.0, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # p = 0
     assert f(8, 1.5, 0, 0, 0, ctypes.byref(out)) == B.SYK_EINVAL       # p > 1
     assert f(8, 0.5, 0, 0, 2, ctypes.byref(out)) == B.SYK_EINVAL       # gamma_norm
@@ -278,3 +278,26 @@ def test_pauli_string_builder(B):
         B.syk_build_from_pauli_strings(1, [(1, 0, 1.0)])
     with pytest.raises(B.SykError):
         B.syk_build_parity_block(h, 0)
+
+
+def test_N66_only_through_parity_blocks(B):
+    """N = 66 (33 qubits) can be built and cut into parity blocks of 32 qubits; the block tables obey the same structure
+    rules as any table (sorted, even-popcount X-masks inside 32 bits, coefficient real iff popcount(x & z) even)."""
+    N = 66
+    h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, 2), 0, 0)
+    info = h.info()
+    assert info["N"] == 66 and info["dim"] == 1 << 33 and info["n_terms"] > 60
+    for sector in (0, 1):
+        hb = B.syk_build_parity_block(h, sector)
+        ib = hb.info()
+        assert ib["N"] == 64 and ib["dim"] == 1 << 32 and ib["n_terms"] == info["n_terms"]
+        tab = hb.tables()
+        assert np.all(tab["x"] < (1 << 32)) and np.all(tab["z"] < (1 << 32))
+        assert np.all(np.diff(tab["x"].astype(np.int64)) > 0)
+        xs = np.repeat(tab["x"], np.diff(tab["group_off"].astype(np.int64)))
+        par = np.array([bin(int(a) & int(b)).count("1") & 1 for a, b in zip(xs, tab["z"])])
+        assert np.all((tab["c"].imag != 0) == (par == 1)) and np.all((tab["c"].real != 0) == (par == 0))
+    with pytest.raises(B.SykError):
+        B.syk_krylov_workspace_bytes(h, B.SYK_C64, {"krylov_dim": 4})
+    with pytest.raises(B.SykError):
+        B.syk_build_hamiltonian(68, 1e-4, 0, 0)
