@@ -40,6 +40,7 @@
 #include <atomic>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "device_utils.cuh"
@@ -92,40 +93,67 @@ __device__ __forceinline__ void st_fused_scalars(LanczosScalars* sc, int j, doub
 __device__ __forceinline__ double st_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
 __device__ __forceinline__ float st_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 
-// One term applied to the RC accumulators of output chunk OC.  `pb` = the thread's position inside the staged
-// source chunk; `w` = sign-carrying word of the coefficient times the sign of (thread, tile, chunk); the slices of
-// the chunk are walked in Gray-code order so that consecutive signs differ by one uniform XOR.
-template <typename T, int R, int RC, int OC, bool IMAG>
+// A consumer thread owns one 16-byte ELEMENT per slice: one complex128 amplitude, or a pair of adjacent complex64
+// amplitudes (index bit 0) -- so both precisions move 16 bytes per LDS and a slice is 4 KiB.  PAIR amplitudes per
+// element, TB index bits inside a slice.
+template <typename T> struct El;
+template <> struct El<double> { static constexpr int PAIR = 1, TB = 8; };
+template <> struct El<float> { static constexpr int PAIR = 2, TB = 9; };
+constexpr uint32_t kSliceBytes = kConsumerThreads * 16;
+
+// One term applied to the RC slices of output chunk OC.  `pb` = the thread's element inside the staged source chunk;
+// `w` = sign-carrying word of the coefficient times the sign of (thread, tile, chunk); the slices of the chunk are
+// walked in Gray-code order so that consecutive signs differ by one uniform XOR.  complex64: `aux` = (z & 1) << 31, the
+// relative sign of the second amplitude of the pair; SWAP = the mask flips index bit 0 (the pair arrives swapped).
+template <typename T, int R, int RC, int OC, bool IMAG, bool SWAP>
 __device__ __forceinline__ void accumulate_chunk(const unsigned char* __restrict__ pb, uint32_t xr_lo, uint32_t zr_lo,
-                                                 uint32_t a_lo, uint32_t w, T (&ar)[R], T (&ai)[R]) {
-    using C = typename Cx<T>::type;
+                                                 uint32_t aux, uint32_t w, T (&ar)[R * El<T>::PAIR],
+                                                 T (&ai)[R * El<T>::PAIR]) {
 #pragma unroll
     for (int i = 0; i < RC; ++i) {
         const int rl = i ^ (i >> 1);
         if (i > 0) w ^= (zr_lo * (0x80000000u / (uint32_t)(i & -i))) & 0x80000000u;   // z bit ctz(i) -> bit 31; a shift after unrolling
-        T a;
-        if constexpr (sizeof(T) == 8) a = __hiloint2double((int)w, (int)a_lo);
-        else a = __uint_as_float(w);
-        const C v = *reinterpret_cast<const C*>(pb + ((((uint32_t)rl ^ xr_lo) << kThreadBits) * (uint32_t)sizeof(C)));
+        const unsigned char* src = pb + (((uint32_t)rl ^ xr_lo) * kSliceBytes);
         constexpr int r0 = OC * RC;
-        if constexpr (IMAG) {   // (i a)(vx + i vy) = -a vy + i a vx
-            ar[r0 + rl] = st_fma(-a, v.y, ar[r0 + rl]);
-            ai[r0 + rl] = st_fma(a, v.x, ai[r0 + rl]);
+        if constexpr (sizeof(T) == 8) {
+            const double a = __hiloint2double((int)w, (int)aux);   // aux = low word of the coefficient
+            const double2 v = *reinterpret_cast<const double2*>(src);
+            if constexpr (IMAG) {   // (i a)(vx + i vy) = -a vy + i a vx
+                ar[r0 + rl] = st_fma(-a, v.y, ar[r0 + rl]);
+                ai[r0 + rl] = st_fma(a, v.x, ai[r0 + rl]);
+            } else {
+                ar[r0 + rl] = st_fma(a, v.x, ar[r0 + rl]);
+                ai[r0 + rl] = st_fma(a, v.y, ai[r0 + rl]);
+            }
         } else {
-            ar[r0 + rl] = st_fma(a, v.x, ar[r0 + rl]);
-            ai[r0 + rl] = st_fma(a, v.y, ai[r0 + rl]);
+            const float a0 = __uint_as_float(w), a1 = __uint_as_float(w ^ aux);
+            const float4 v = *reinterpret_cast<const float4*>(src);
+            const float s0x = SWAP ? v.z : v.x, s0y = SWAP ? v.w : v.y, s1x = SWAP ? v.x : v.z, s1y = SWAP ? v.y : v.w;
+            const int k0 = 2 * (r0 + rl), k1 = k0 + 1;
+            if constexpr (IMAG) {
+                ar[k0] = st_fma(-a0, s0y, ar[k0]);
+                ai[k0] = st_fma(a0, s0x, ai[k0]);
+                ar[k1] = st_fma(-a1, s1y, ar[k1]);
+                ai[k1] = st_fma(a1, s1x, ai[k1]);
+            } else {
+                ar[k0] = st_fma(a0, s0x, ar[k0]);
+                ai[k0] = st_fma(a0, s0y, ai[k0]);
+                ar[k1] = st_fma(a1, s1x, ar[k1]);
+                ai[k1] = st_fma(a1, s1y, ai[k1]);
+            }
         }
     }
 }
 
-template <typename T, int R, int RC, int OC, bool IMAG>
+template <typename T, int R, int RC, int OC, bool IMAG, bool SWAP>
 __device__ __forceinline__ void dispatch_chunk(uint32_t oc, const unsigned char* pb, uint32_t xr_lo, uint32_t zr_lo,
-                                               uint32_t a_lo, uint32_t w, T (&ar)[R], T (&ai)[R]) {
+                                               uint32_t aux, uint32_t w, T (&ar)[R * El<T>::PAIR],
+                                               T (&ai)[R * El<T>::PAIR]) {
     if constexpr (OC + 1 == R / RC) {
-        accumulate_chunk<T, R, RC, OC, IMAG>(pb, xr_lo, zr_lo, a_lo, w, ar, ai);
+        accumulate_chunk<T, R, RC, OC, IMAG, SWAP>(pb, xr_lo, zr_lo, aux, w, ar, ai);
     } else {
-        if (oc == (uint32_t)OC) accumulate_chunk<T, R, RC, OC, IMAG>(pb, xr_lo, zr_lo, a_lo, w, ar, ai);
-        else dispatch_chunk<T, R, RC, OC + 1, IMAG>(oc, pb, xr_lo, zr_lo, a_lo, w, ar, ai);
+        if (oc == (uint32_t)OC) accumulate_chunk<T, R, RC, OC, IMAG, SWAP>(pb, xr_lo, zr_lo, aux, w, ar, ai);
+        else dispatch_chunk<T, R, RC, OC + 1, IMAG, SWAP>(oc, pb, xr_lo, zr_lo, aux, w, ar, ai);
     }
 }
 
@@ -136,7 +164,8 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
     constexpr int R = 1 << NR;
     constexpr int RC = 1 << LRC;                                  // slices per ring chunk
     constexpr int NC = R / RC;                                    // chunks per tile
-    constexpr uint32_t SLICE_BYTES = kConsumerThreads * sizeof(C);
+    constexpr uint32_t SLICE_BYTES = kSliceBytes;                 // 256 elements of 16 bytes
+    constexpr int PAIR = El<T>::PAIR, TB = El<T>::TB;
     constexpr uint32_t RUN_BYTES = kRun * SLICE_BYTES;
     constexpr uint32_t CHUNK_BYTES = RC * SLICE_BYTES;
     static_assert(R % RC == 0 && RC % kRun == 0 && LRC >= kFixedR, "tile = whole chunks = whole runs");
@@ -237,10 +266,10 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             uint32_t base = 0;
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
-            const uint32_t bt = base | (uint32_t)tid;
-            T ar[R], ai[R];
+            const uint32_t bt = base | ((uint32_t)tid << (TB - 8));   // index of the element's first amplitude, r bits 0
+            T ar[R * PAIR], ai[R * PAIR];
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
+            for (int r = 0; r < R * PAIR; ++r) {
                 ar[r] = 0;
                 ai[r] = 0;
             }
@@ -251,14 +280,25 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                     const unsigned char* cp = smem + (size_t)pos * CHUNK_BYTES;
                     for (int t = t0; t < t1; ++t) {
                         const uint4 e = tab.term[t];
-                        const uint32_t xt = e.x & 255u, xr = (e.x >> 8) & 63u, zr = (e.x >> 16) & 63u;
+                        const uint32_t xt = e.x & 511u, xr = (e.x >> 9) & 63u, zr = (e.x >> 16) & 63u;
                         const uint32_t oc = c ^ (xr >> LRC);
-                        const unsigned char* pb = cp + (((uint32_t)tid ^ xt) * (uint32_t)sizeof(C));
+                        const unsigned char* pb = cp + (((uint32_t)tid ^ (xt >> (TB - 8))) * 16u);
                         const uint32_t sgn = (uint32_t)(__popc(bt & e.y) + __popc((oc << LRC) & zr)) << 31;
                         const uint32_t w = (sizeof(T) == 8 ? e.w : e.z) ^ sgn;
                         constexpr uint32_t lo = (uint32_t)RC - 1u;
-                        if (e.x >> 31) dispatch_chunk<T, R, RC, 0, true>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
-                        else dispatch_chunk<T, R, RC, 0, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
+                        if constexpr (sizeof(T) == 8) {
+                            if (e.x >> 31) dispatch_chunk<T, R, RC, 0, true, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
+                            else dispatch_chunk<T, R, RC, 0, false, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
+                        } else {
+                            const uint32_t aux = (e.y & 1u) << 31;   // second amplitude of the pair: index bit 0 set
+                            if (e.x >> 31) {
+                                if (xt & 1u) dispatch_chunk<T, R, RC, 0, true, true>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
+                                else dispatch_chunk<T, R, RC, 0, true, false>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
+                            } else {
+                                if (xt & 1u) dispatch_chunk<T, R, RC, 0, false, true>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
+                                else dispatch_chunk<T, R, RC, 0, false, false>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
+                            }
+                        }
                     }
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_empty + 8 * pos);
@@ -268,22 +308,69 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                     }
                 }
             }
-            // epilogue: slice r of the tile is 256 consecutive amplitudes
+            // epilogue: slice r of the tile is 256 consecutive elements; one 16-byte store per thread and slice
+            using E = typename std::conditional<sizeof(T) == 8, double2, float4>::type;
+            auto emit = [&](int r, const E* mine_p, const E* prev_p) {
+                const uint64_t b = (uint64_t)(bt | tab.dep_r[r]);
+                E o;
+                if constexpr (sizeof(T) == 8) {
+                    if constexpr (FUSED) {
+                        const E mine = *mine_p;
+                        double orr = ar[r] * s_in, oi = ai[r] * s_in;
+                        if (prev_p) {
+                            const E pv = *prev_p;
+                            orr -= s_prev * pv.x;
+                            oi -= s_prev * pv.y;
+                        }
+                        o.x = orr;
+                        o.y = oi;
+                        dot += mine.x * o.x + mine.y * o.y;
+                    } else {
+                        o.x = ar[r];
+                        o.y = ai[r];
+                    }
+                } else {
+                    if constexpr (FUSED) {
+                        const E mine = *mine_p;
+                        double o0r = (double)ar[2 * r] * s_in, o0i = (double)ai[2 * r] * s_in;
+                        double o1r = (double)ar[2 * r + 1] * s_in, o1i = (double)ai[2 * r + 1] * s_in;
+                        if (prev_p) {
+                            const E pv = *prev_p;
+                            o0r -= s_prev * (double)pv.x;
+                            o0i -= s_prev * (double)pv.y;
+                            o1r -= s_prev * (double)pv.z;
+                            o1i -= s_prev * (double)pv.w;
+                        }
+                        o.x = (float)o0r;
+                        o.y = (float)o0i;
+                        o.z = (float)o1r;
+                        o.w = (float)o1i;
+                        dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y +
+                               (double)mine.z * (double)o.z + (double)mine.w * (double)o.w;
+                    } else {
+                        o.x = ar[2 * r];
+                        o.y = ai[2 * r];
+                        o.z = ar[2 * r + 1];
+                        o.w = ai[2 * r + 1];
+                    }
+                }
+                *reinterpret_cast<E*>(p.out + b) = o;
+            };
             if constexpr (FUSED) {
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     mbar_wait(bar_full + 8 * pos, phase);
-                    const C* mine_s = reinterpret_cast<const C*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
+                    const E* mine_s = reinterpret_cast<const E*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
                     const int pos_in = pos;
                     if (++pos == nring) {
                         pos = 0;
                         phase ^= 1u;
                     }
-                    const C* prev_s = nullptr;
+                    const E* prev_s = nullptr;
                     int pos_prev = 0;
                     if (p.prev) {
                         mbar_wait(bar_full + 8 * pos, phase);
-                        prev_s = reinterpret_cast<const C*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
+                        prev_s = reinterpret_cast<const E*>(smem + (size_t)pos * CHUNK_BYTES) + tid;
                         pos_prev = pos;
                         if (++pos == nring) {
                             pos = 0;
@@ -291,22 +378,8 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                         }
                     }
 #pragma unroll
-                    for (int rl = 0; rl < RC; ++rl) {
-                        const int r = c * RC + rl;
-                        const uint64_t b = (uint64_t)(bt | tab.dep_r[r]);
-                        const C mine = mine_s[rl * kConsumerThreads];
-                        double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
-                        if (prev_s) {
-                            const C pv = prev_s[rl * kConsumerThreads];
-                            orr -= s_prev * (double)pv.x;
-                            oi -= s_prev * (double)pv.y;
-                        }
-                        C o;
-                        o.x = (T)orr;
-                        o.y = (T)oi;
-                        dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
-                        p.out[b] = o;
-                    }
+                    for (int rl = 0; rl < RC; ++rl)
+                        emit(c * RC + rl, mine_s + rl * kConsumerThreads, prev_s ? prev_s + rl * kConsumerThreads : nullptr);
                     __syncwarp();
                     if (lane == 0) {
                         mbar_arrive(bar_empty + 8 * pos_in);
@@ -315,12 +388,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 }
             } else {
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    C o;
-                    o.x = ar[r];
-                    o.y = ai[r];
-                    p.out[(uint64_t)(bt | tab.dep_r[r])] = o;
-                }
+                for (int r = 0; r < R; ++r) emit(r, nullptr, nullptr);
             }
         }
         if (FUSED) {
@@ -340,10 +408,11 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
     }
 }
 
-// NR (log2 accumulators per thread) and LRC (log2 slices per ring chunk) per dtype index (SYK_C64 = 0, SYK_C128 = 1):
-// 128 KiB tiles in two 64 KiB chunks
-constexpr int kStNR[2] = {6, 5};
-constexpr int kStLRC[2] = {5, 4};
+// Per dtype index (SYK_C64 = 0, SYK_C128 = 1): index bits inside a slice (a complex64 element is a pair of amplitudes),
+// NR = log2 slices per tile, LRC = log2 slices per ring chunk: 128 KiB tiles in two 64 KiB chunks for both
+constexpr int kStTB[2] = {9, 8};
+constexpr int kStNR[2] = {5, 5};
+constexpr int kStLRC[2] = {4, 4};
 
 uint32_t extract_bits(uint32_t v, const int* pos, int n) {
     uint32_t r = 0;
@@ -363,8 +432,9 @@ struct LayoutCost {
 
 // #loads = distinct x outside the tile bits; #passes = distinct x outside tile + window bits.  seq = the free
 // positions (index bits >= 11): seq[0..nr) are the free r bits, seq[nr..nr+kWindowBits) the window bits.
-LayoutCost layout_cost(const std::vector<uint32_t>& xs, const std::vector<int>& seq, int nr, std::vector<uint32_t>& tmp) {
-    uint32_t tile = (1u << (kThreadBits + kFixedR)) - 1u;
+LayoutCost layout_cost(const std::vector<uint32_t>& xs, const std::vector<int>& seq, int nr, std::vector<uint32_t>& tmp,
+                       int tb) {
+    uint32_t tile = (1u << (tb + kFixedR)) - 1u;
     for (int i = 0; i < nr; ++i) tile |= 1u << seq[i];
     uint32_t win = tile;
     for (int i = nr; i < nr + kWindowBits && i < (int)seq.size(); ++i) win |= 1u << seq[i];
@@ -381,13 +451,13 @@ LayoutCost layout_cost(const std::vector<uint32_t>& xs, const std::vector<int>& 
 
 // Deterministic first-improvement hill climbing over swaps that move a bit between the classes r / window / rest,
 // started from the identity layout (free r bits = 11.., window = the next 7).  nr = number of FREE r bits.
-void choose_layout(const std::vector<uint32_t>& xs, int L, int nr, std::vector<int>& seq) {
+void choose_layout(const std::vector<uint32_t>& xs, int L, int nr, std::vector<int>& seq, int tb) {
     seq.clear();
-    for (int q = kThreadBits + kFixedR; q < L; ++q) seq.push_back(q);
+    for (int q = tb + kFixedR; q < L; ++q) seq.push_back(q);
     const int n = (int)seq.size();
     const int nw = std::min(kWindowBits, n - nr);
     std::vector<uint32_t> tmp;
-    int cur = layout_cost(xs, seq, nr, tmp).total();
+    int cur = layout_cost(xs, seq, nr, tmp, tb).total();
     auto cls = [&](int i) { return i < nr ? 0 : (i < nr + nw ? 1 : 2); };
     for (int sweep = 0; sweep < 16; ++sweep) {
         bool improved = false;
@@ -395,7 +465,7 @@ void choose_layout(const std::vector<uint32_t>& xs, int L, int nr, std::vector<i
             for (int j = i + 1; j < n; ++j) {
                 if (cls(i) == cls(j)) continue;
                 std::swap(seq[i], seq[j]);
-                const int c = layout_cost(xs, seq, nr, tmp).total();
+                const int c = layout_cost(xs, seq, nr, tmp, tb).total();
                 if (c < cur) {
                     cur = c;
                     improved = true;
@@ -413,16 +483,16 @@ void choose_layout(const std::vector<uint32_t>& xs, int L, int nr, std::vector<i
 
 bool build_st_table(const syk_ham* h, int dtype, StTable& tab) {
     const int k = dtype == SYK_C128 ? 1 : 0;
-    const int nr = kStNR[k];
+    const int nr = kStNR[k], tb = kStTB[k];
     const size_t nt = h->z.size();
-    if (nt == 0 || nt > (size_t)kStMaxTerms || h->L < kThreadBits + nr) return false;
+    if (nt == 0 || nt > (size_t)kStMaxTerms || h->L < tb + nr) return false;
     std::vector<uint32_t> xs;
     for (size_t g = 0; g < h->x.size(); ++g) xs.push_back((uint32_t)h->x[g]);
     std::vector<int> seq;
-    choose_layout(xs, h->L, nr - kFixedR, seq);
-    const int n_outer = h->L - kThreadBits - nr;
+    choose_layout(xs, h->L, nr - kFixedR, seq, tb);
+    const int n_outer = h->L - tb - nr;
     std::vector<int> pvec;
-    for (int i = 0; i < kFixedR; ++i) pvec.push_back(kThreadBits + i);
+    for (int i = 0; i < kFixedR; ++i) pvec.push_back(tb + i);
     for (int i = 0; i < nr - kFixedR; ++i) pvec.push_back(seq[i]);
     const int* P = pvec.data();
     const int* O = seq.data() + (nr - kFixedR);
@@ -444,7 +514,8 @@ bool build_st_table(const syk_ham* h, int dtype, StTable& tab) {
             it.key = extract_bits(x, O, n_outer);
             it.xo = x & omask;
             it.order = (uint32_t)items.size();
-            it.e.x = (x & 255u) | (extract_bits(x, P, nr) << 8) | (extract_bits(z, P, nr) << 16) | (imag ? 0x80000000u : 0u);
+            it.e.x = (x & ((1u << tb) - 1u)) | (extract_bits(x, P, nr) << 9) | (extract_bits(z, P, nr) << 16) |
+                     (imag ? 0x80000000u : 0u);
             it.e.y = z;
             if (dtype == SYK_C128) {
                 uint64_t bits;
@@ -480,7 +551,7 @@ bool build_st_table(const syk_ham* h, int dtype, StTable& tab) {
     tab.nr = nr;
     for (int s = 0; s < 64; ++s) tab.dep_r[s] = s < (1 << nr) ? deposit_bits((uint32_t)s, P, nr) : 0u;
     for (int i = 0; i < 32; ++i) tab.outer_pos[i] = i < n_outer ? (uint8_t)O[i] : 0;
-    uint32_t tile = 255u;
+    uint32_t tile = (1u << tb) - 1u;
     for (int i = 0; i < nr; ++i) tile |= 1u << P[i];
     tab.tile_mask = tile;
     return true;
@@ -501,7 +572,7 @@ template <typename T, int NR, int LRC>
 int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_out, const FusedArgs& fa,
               cudaStream_t stream) {
     using C = typename Cx<T>::type;
-    constexpr size_t kChunkBytes = ((size_t)1 << LRC) * kConsumerThreads * sizeof(C);
+    constexpr size_t kChunkBytes = ((size_t)1 << LRC) * kSliceBytes;
     StParams<T> p;
     p.in = (const C*)d_in;
     p.out = (C*)d_out;
@@ -544,7 +615,7 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
 // 0 if the handle cannot use the kernel, else log2 of its tile size in amplitudes
 int scatter_tile_log2(const syk_ham* h, int dtype, bool forced) {
     const int k = dtype == SYK_C128 ? 1 : 0;
-    const int tl = kThreadBits + kStNR[k];
+    const int tl = kStTB[k] + kStNR[k];
     if (h->n_terms() == 0 || h->n_terms() > kStMaxTerms || h->L < tl) return 0;
     // automatic choice: at least ~4 rounds of 128 KiB tiles on 148 SMs
     if (!forced && h->L < tl + 10) return 0;

@@ -55,7 +55,8 @@ struct RtCache {
 constexpr int kStMaxTerms = 1024;
 constexpr int kStMaxLoads = 1024;
 struct StTable {
-    // term t: .x = low 8 bits of x | (r bits of x) << 8 | (r bits of z) << 16 | (coefficient is imaginary) << 31 ;
+    // term t: .x = in-slice bits of x (8 / 9 for complex128 / complex64) | (r bits of x) << 9 | (r bits of z) << 16 |
+    //         (coefficient is imaginary) << 31 ;
     //         .y = Z-mask ; (.z, .w) = bits of the signed magnitude a (double), or .z = bits of (float) a
     uint4 term[kStMaxTerms];
     uint32_t load_xo[kStMaxLoads];         // x restricted to the outer bit positions, per load (sorted by tile counter)

@@ -58,8 +58,8 @@ __device__ __forceinline__ double reduce_partials(const double* p, int n, double
 // than L2 holds (ncu, N = 64: 5 % hit rate), so the producers pace each other: loads are counted in epochs of
 // `epoch_len`; a producer that starts epoch e first reports epoch e-1 as issued (one atomicAdd on a ring of
 // kSyncRing counters) and then waits until all gridDim.x CTAs have reported epoch e-1-lag.  Timing only: no data
-// depends on it, results stay bitwise equal.  All CTAs are co-resident (grid <= number of SMs, one CTA per SM), so
-// the wait cannot deadlock.
+// depends on it, results stay bitwise equal.  All CTAs are co-resident (grid <= number of SMs, one CTA per SM) and the
+// wait is bounded, so it cannot deadlock.
 __device__ __forceinline__ void lockstep_gate(uint32_t* sync, uint32_t e, uint32_t lag) {
     if (e == 0) return;
     atomicAdd(sync + ((e - 1) % kSyncRing), 1u);
@@ -67,7 +67,9 @@ __device__ __forceinline__ void lockstep_gate(uint32_t* sync, uint32_t e, uint32
     const uint32_t f = e - 1 - lag;
     const uint32_t target = gridDim.x * (f / kSyncRing + 1);
     const volatile uint32_t* c = sync + (f % kSyncRing);
-    while (*c < target) __nanosleep(64);
+    // bounded wait (~2 ms): pacing is an optimisation, never a dependency -- if the counters are disturbed (two launches
+    // on one handle in flight on different streams) the CTA simply runs on unpaced
+    for (int spins = 0; *c < target && spins < 32768; ++spins) __nanosleep(64);
 }
 
 // ---- mbarrier and bulk async copy (TMA unit, non-tensor form: SASS UBLKCP) -------------------------------

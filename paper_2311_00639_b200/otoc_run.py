@@ -69,18 +69,17 @@ def main():
         # vectors with weight 1/2 each (the Haar ensemble up to O(D^-1/2) fluctuations of the sector weights)
         he, ho = B.syk_build_parity_block(h, 0), B.syk_build_parity_block(h, 1)
         half = 1 << (L - 1)
-        ps = [torch.empty(half, dtype=tdt, device="cuda") for _ in (0, 1)]
-        for s in (0, 1):
-            B.syk_random_state(N - 2, args.seed, 2 * args.realization + s, ps[s], scratch)   # each has norm 1
+        ps = torch.empty(half, dtype=tdt, device="cuda")       # one sector at a time: N = 66 needs all of the memory
         wk = torch.empty(B.syk_otoc_workspace_bytes(he, code, opts), dtype=torch.uint8, device="cuda")
         torch.cuda.synchronize()
         t1 = time.perf_counter()
         F = 0
         for s in (0, 1):
+            B.syk_random_state(N - 2, args.seed, 2 * args.realization + s, ps, scratch)      # norm 1
             if args.green:
-                Fs, st = B.syk_green_block(he, ho, s, iW, args.beta, t_grid, ps[s], wk, opts)
+                Fs, st = B.syk_green_block(he, ho, s, iW, args.beta, t_grid, ps, wk, opts)
             else:
-                Fs, st = B.syk_otoc_block(he, ho, s, iW, jV, args.beta, t_grid, ps[s], wk, opts)
+                Fs, st = B.syk_otoc_block(he, ho, s, iW, jV, args.beta, t_grid, ps, wk, opts)
             F = F + 0.5 * Fs      # F is quadratic in psi: |psi_U|^2 = |psi_D|^2 = 1/2 for the jointly normalised state
             for key in stats_tot:
                 stats_tot[key] += st[key]
