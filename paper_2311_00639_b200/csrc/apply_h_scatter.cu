@@ -8,12 +8,13 @@
 // (x restricted to the bits outside a tile).  Both counts depend on WHICH qubits are the tile / window bits, and
 // the X-masks of a sparse SYK Hamiltonian are random 2- and 4-subsets of the qubits, so the host picks the bits
 // (choose_layout: hill climbing on  #loads + 2 #passes):
-//   * thread bits  : index bits 0..7 (256 consecutive amplitudes, one per consumer thread);
-//   * r bits       : NR further bit positions P[0..NR-1]; a thread keeps the R = 2^NR amplitudes
-//                    base | deposit(r, P) | tid  in registers (128 KiB of accumulators per SM).  P[0..2] = 8, 9, 10
-//                    (a "run" of 8 slices = 2048 consecutive amplitudes = one cp.async.bulk: the TMA unit costs
-//                    ~85 clk per copy, measured, so 2-4 KiB copies cannot feed an SM); the other NR-3 r bits sit
-//                    ANYWHERE in the index;
+//   * slice bits   : index bits 0..TB-1: a slice = 256 consecutive 16-byte ELEMENTS, one per consumer thread; an
+//                    element is one complex128 amplitude (TB = 8) or a pair of adjacent complex64 amplitudes
+//                    (TB = 9: both precisions move 16 bytes per LDS and per store);
+//   * r bits       : NR = 5 further bit positions P[0..4]; a thread keeps the R = 32 elements
+//                    base | deposit(r, P) | element  in registers (128 KiB of accumulators per SM).  P[0..2] = TB..TB+2
+//                    (a "run" of 8 slices = 32 KiB contiguous = one cp.async.bulk: the TMA unit costs ~85 clk per
+//                    copy, measured, so 2-4 KiB copies cannot feed an SM); the other 2 r bits sit ANYWHERE in the index;
 //   * outer bits   : the rest, in an order O[0..]: the tile counter tau is deposited into them, O[0] fastest, so
 //                    the 148 tiles in flight differ in O[0..7] only -- those are the L2-window bits.
 // No data is permuted: a source tile is fetched run by run (cp.async.bulk, TMA unit, SASS UBLKCP; completion on
@@ -26,7 +27,7 @@
 // (uniformly) to the code that owns the accumulator registers of chunk oc.
 //
 // Per (amplitude, term): one LDS, two FMAs (the coefficient is exactly real or exactly imaginary: c = J s^4 times
-// 1, -1, i, -i); the sign is popcount((base | tid) & z) once per (term, chunk) and thread plus a Gray-code walk
+// 1, -1, i, -i); the sign is popcount((base | element) & z) once per (term, chunk) and thread plus a Gray-code walk
 // over the slices of a chunk (one XOR each).  Per-term data comes from the __grid_constant__ table (constant
 // bank).  No atomics on data, one write per output: bitwise reproducible.
 //
@@ -56,7 +57,6 @@ constexpr int kConsumerThreads = kConsumerWarps * 32;
 // (setmaxnreg, per warpgroup): 2 x 232 + 40 <= 512 registers per lane on every SM sub-partition.
 constexpr int kThreads = kConsumerThreads + 128;
 constexpr int kConsumerRegs = 232, kProducerRegs = 40;
-constexpr int kThreadBits = 8;
 constexpr int kRun = 8;                            // consecutive slices per bulk copy (r bits 0..2 = index bits 8..10)
 constexpr int kMaxRing = 16;
 constexpr int kSmemLimit = 232448;                 // 227 KiB opt-in maximum per CTA on sm_100
