@@ -39,7 +39,6 @@ constexpr int kTile = 1 << kTileLog2D;
 constexpr int kMaxSlots = 6;
 constexpr int kSmemLimit = 232448;
 constexpr int kMiscBytes = 2 * kMaxSlots * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, reduction scratch, table buffers
-constexpr int kTableBufBytes = 2 * 512 * 16;
 
 // The table is ONE stream of 16-byte entries, cut into chunks of <= kChunkEntries entries that hold whole groups:
 //   group header : .x = tile-local X-mask, .y = number of terms that follow, .z = 1 real / 2 imaginary / 3 both,

@@ -256,7 +256,7 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
 
     double remaining = len;
     int rc = SYK_OK;
-    std::vector<double> alpha(kMaxKrylov + 2), nrm(kMaxKrylov + 2), A;
+    std::vector<double> alpha(kMaxKrylov + 2), nrm(kMaxKrylov + 2);
     std::vector<double2> coef(kMaxKrylov + 2);
     int n_sub = 0;
     while (remaining > 1e-15 * len) {
