@@ -5,19 +5,20 @@
 //
 // Here the vector traffic is negligible (a few hundred source tiles per output tile, all L2 hits) and the work is
 // the T sign-accumulates per amplitude: plain ALU.  Three things keep that cheap:
-//   * the thread owns R = 16 amplitudes  base | tid | r << 8  (r = index bits 8..11), so everything that depends on
-//     the term only (table read, popcount of the tile/thread part of the sign) is paid once per 16 amplitudes;
-//   * the r-dependence of the sign is a WALSH FUNCTION of r:  (-1)^popcount(r & zr),  zr = bits 8..11 of z.  So the
-//     terms of a group are first binned by zr -- one add per TERM into one of 16 registers (terms come sorted by
+//   * the thread owns R = 8 amplitudes  base | tid | r << 9  (r = index bits 9..11), so everything that depends on
+//     the term only (table read, popcount of the tile/thread part of the sign) is paid once per 8 amplitudes;
+//   * the r-dependence of the sign is a WALSH FUNCTION of r:  (-1)^popcount(r & zr),  zr = bits 9..11 of z.  So the
+//     terms of a group are first binned by zr -- one add per TERM into one of 8 registers (terms come sorted by
 //     bin, so the register is a compile-time index of an unrolled walk over the bins that occur) -- and
-//     S_g(r) for the 16 r is the Walsh-Hadamard transform of the bins: 64 adds per group instead of 16 per term;
+//     S_g(r) for the 8 r is the Walsh-Hadamard transform of the bins: 24 adds per group instead of 8 per term;
 //   * c_t is exactly real or exactly imaginary (J s^4 times 1, -1, i, -i): two real bin arrays, no complex adds.
 // Then one complex multiply-add per (group, amplitude) with the source read from the staged tile.
 //
-// Source tiles (2^12 amplitudes: 64 / 32 KiB) come through the same cp.async.bulk ring as in the other tile kernels
-// (one producer lane, mbarriers); the table (a few MB, streamed once per output tile) is staged chunk by chunk in
-// shared memory by the consumers themselves, double buffered, so the inner loops read it with broadcast LDS (read
-// from global with warp-uniform addresses, each term cost an exposed L2 latency: 1120 ms per N = 48 matvec).
+// Source tiles (2^12 amplitudes: 64 / 32 KiB) come by cp.async.bulk into a double buffer (thread 0 issues the next
+// one, mbarrier completion); the table (a few MB, streamed once per output tile) is staged chunk by chunk in shared
+// memory by the threads themselves, double buffered, so the inner loops read it with broadcast LDS (read from global
+// with warp-uniform addresses, each term cost an exposed L2 latency: 1120 ms per N = 48 matvec).
+// History at N = 48 dense complex128: generic kernel 2390 ms; 8 warps x 16 amplitudes 692 ms; this shape 488 ms.
 // No atomics on data, one write per output: bitwise reproducible.  Fused Lanczos epilogue as in apply_h.cu.
 #include <algorithm>
 #include <cstring>
@@ -30,20 +31,21 @@ namespace syk {
 
 namespace {
 
-constexpr int kConsumerWarps = 8;
-constexpr int kConsumerThreads = kConsumerWarps * 32;
-constexpr int kThreads = kConsumerThreads + 32;
-constexpr int kR = 16;                             // amplitudes per thread
-constexpr int kTileLog2D = 12;                     // 256 threads x 16
+// 16 warps, every thread a consumer (four warps per scheduler hide the dependent chain of a term: table LDS ->
+// popcount -> sign -> add; with 8 warps and 16 amplitudes per thread the schedulers were 35 % busy); thread 0 also
+// issues the bulk copies -- a source tile is consumed over ~10^5 cycles, so a plain double buffer is enough.
+constexpr int kThreadBitsD = 9;
+constexpr int kConsumerThreads = 1 << kThreadBitsD;
+constexpr int kThreads = kConsumerThreads;
+constexpr int kR = 8;                              // amplitudes per thread
+constexpr int kTileLog2D = 12;                     // 512 threads x 8
 constexpr int kTile = 1 << kTileLog2D;
-constexpr int kMaxSlots = 6;
-constexpr int kSmemLimit = 232448;
-constexpr int kMiscBytes = 2 * kMaxSlots * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, reduction scratch, table buffers
+constexpr int kMiscBytes = 2 * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, reduction scratch, table buffers
 
 // The table is ONE stream of 16-byte entries, cut into chunks of <= kChunkEntries entries that hold whole groups:
 //   group header : .x = tile-local X-mask, .y = number of terms that follow, .z = 1 real / 2 imaginary / 3 both,
-//                  .w = which of the 32 bins occur
-//   term         : .x = Z-mask, .y = bin = zr (bits 8..11 of z) + 16 if the coefficient is imaginary; terms of a
+//                  .w = which of the 16 bins occur
+//   term         : .x = Z-mask, .y = bin = zr (bits 9..11 of z) + 8 if the coefficient is imaginary; terms of a
 //                  group are sorted by bin and bit 8 of .y marks the last term of a bin,
 //                  (.z, .w) = bits of the signed magnitude a (double) or .z = bits of (float) a
 // The consumers copy chunk k+1 into shared memory while they work on chunk k (double buffer), so every table read
@@ -83,7 +85,7 @@ __device__ __forceinline__ void dn_fused_scalars(LanczosScalars* sc, int j, doub
 
 // in-place Walsh-Hadamard transform: s[r] = sum_z c[z] (-1)^popcount(r & z)
 template <typename T>
-__device__ __forceinline__ void wht16(T (&c)[kR]) {
+__device__ __forceinline__ void wht(T (&c)[kR]) {
 #pragma unroll
     for (int h = 1; h < kR; h <<= 1) {
 #pragma unroll
@@ -129,21 +131,19 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnPara
     constexpr uint32_t kChunk = 16384;
 
     extern __shared__ __align__(128) unsigned char smem[];
-    C* stages = reinterpret_cast<C*>(smem);
-    unsigned char* q = smem + (size_t)p.nslot * TILE_BYTES;
-    uint4* tbuf = reinterpret_cast<uint4*>(q);      // 2 x kChunkEntries table entries
+    C* stages = reinterpret_cast<C*>(smem);                       // 2 tile slots
+    unsigned char* q = smem + (size_t)2 * TILE_BYTES;
+    uint4* tbuf = reinterpret_cast<uint4*>(q);                    // 2 x kChunkEntries table entries
     q += 2 * kChunkEntries * sizeof(uint4);
     uint64_t* bars = reinterpret_cast<uint64_t*>(q);
-    q += 2 * kMaxSlots * 8;
+    q += 2 * 8;
     double* red = reinterpret_cast<double*>(q);
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kMaxSlots);
+    const int tid = threadIdx.x;
+    const uint32_t bar_full = smem_u32(bars);
     if (tid == 0) {
-        for (int s = 0; s < p.nslot; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, kConsumerWarps);
-        }
+        mbar_init(bar_full, 1);
+        mbar_init(bar_full + 8, 1);
         mbar_fence_init();
     }
     __syncthreads();
@@ -152,151 +152,126 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnPara
     if (FUSED) dn_fused_scalars(p.sc, p.j, red, s_in, s_prev);
 
     const uint32_t n_tiles = 1u << (p.L - kTileLog2D);
-    const int nslot = p.nslot, n_loads = p.n_loads;
+    const int n_loads = p.n_loads;
     double dot = 0.0;
 
-    if (warp == kConsumerWarps) {
-        // ---------------- producer: one lane streams source tiles into the ring ----------------
-        if (lane == 0) {
-            int slot = 0;
-            uint32_t phase = 0;
-            const uint32_t stage0 = smem_u32(stages);
-            for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-                for (int l = 0; l < n_loads; ++l) {
-                    const uint32_t hi = __ldg(&p.loads[l].hi);
-                    // a load is consumed over ~10^5 cycles of arithmetic: poll slowly, a spinning lane would only
-                    // take issue slots from the two consumer warps on its scheduler (23 % of all instructions, ncu)
-                    while (!mbar_try_wait(bar_empty + 8 * slot, phase ^ 1u)) __nanosleep(2000);
-                    mbar_arrive_expect_tx(bar_full + 8 * slot, TILE_BYTES);
-                    const unsigned char* src =
-                        reinterpret_cast<const unsigned char*>(p.in + ((uint64_t)(tile ^ hi) << kTileLog2D));
-                    const uint32_t dst = stage0 + (uint32_t)slot * TILE_BYTES;
+    // source tile of load l of output tile `tile` into slot s (thread 0 only; completion on full[s])
+    auto issue = [&](uint32_t tile, int l, uint32_t s) {
+        const uint32_t hi = __ldg(&p.loads[l].hi);
+        mbar_arrive_expect_tx(bar_full + 8 * s, TILE_BYTES);
+        const unsigned char* src = reinterpret_cast<const unsigned char*>(p.in + ((uint64_t)(tile ^ hi) << kTileLog2D));
+        const uint32_t dst = smem_u32(stages) + s * TILE_BYTES;
 #pragma unroll
-                    for (uint32_t c = 0; c < TILE_BYTES; c += kChunk) bulk_load(dst + c, src + c, kChunk, bar_full + 8 * slot);
-                    if (++slot == nslot) {
-                        slot = 0;
-                        phase ^= 1u;
-                    }
-                }
-            }
+        for (uint32_t c = 0; c < TILE_BYTES; c += kChunk) bulk_load(dst + c, src + c, kChunk, bar_full + 8 * s);
+    };
+
+    // table stream: this thread's entry of the chunk being prefetched
+    uint32_t ck = 0;                           // chunk whose copy sits in tbuf[ck & 1] after the next barrier
+    uint4 pre;
+    auto fetch = [&](uint32_t c) {             // global -> register (chunk c)
+        const uint32_t e0 = __ldg(&p.chunks[c].e0), ne = __ldg(&p.chunks[c].ne);
+        pre = (uint32_t)tid < ne ? __ldg(p.entries + e0 + tid) : make_uint4(0, 0, 0, 0);
+    };
+    auto stash = [&](uint32_t c) { tbuf[(c & 1u) * kChunkEntries + tid] = pre; };
+    fetch(0);
+    stash(0);
+    uint32_t g = 0;                            // loads consumed by this CTA: slot g & 1, parity (g >> 1) & 1
+    if (tid == 0 && blockIdx.x < n_tiles) issue(blockIdx.x, 0, 0);
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint32_t base = tile << kTileLog2D;
+        const uint32_t bt = base | (uint32_t)tid;
+        T ar[kR], ai[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            ar[r] = 0;
+            ai[r] = 0;
         }
-        __syncwarp();
-    } else {
-        // ---------------- consumers ----------------
-        int slot = 0;
-        uint32_t phase = 0;
-        // table stream: this thread's two entries of the chunk being prefetched
-        uint32_t ck = 0;                       // chunk whose copy sits in tbuf[ck & 1] after the next barrier
-        uint4 pre0, pre1;
-        auto fetch = [&](uint32_t c) {         // global -> registers (chunk c, wrapping around the table)
-            const DenseChunk ch = *reinterpret_cast<const DenseChunk*>(&p.chunks[c]);
-            const uint32_t i0 = (uint32_t)tid, i1 = (uint32_t)tid + kConsumerThreads;
-            pre0 = i0 < ch.ne ? __ldg(p.entries + ch.e0 + i0) : make_uint4(0, 0, 0, 0);
-            pre1 = i1 < ch.ne ? __ldg(p.entries + ch.e0 + i1) : make_uint4(0, 0, 0, 0);
-        };
-        auto stash = [&](uint32_t c) {         // registers -> shared buffer (c & 1)
-            uint4* dst = tbuf + (c & 1u) * kChunkEntries;
-            dst[tid] = pre0;
-            dst[tid + kConsumerThreads] = pre1;
-        };
-        fetch(0);
-        stash(0);
-        for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-            const uint32_t base = tile << kTileLog2D;
-            const uint32_t bt = base | (uint32_t)tid;
-            T ar[kR], ai[kR];
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                ar[r] = 0;
-                ai[r] = 0;
+        for (int l = 0; l < n_loads; ++l, ++g) {
+            const uint32_t slot = g & 1u;
+            __syncthreads();                   // everyone has finished with the other slot (load g - 1)
+            if (tid == 0) {                    // prefetch the next load: a load is ~10^5 cycles of arithmetic
+                if (l + 1 < n_loads) issue(tile, l + 1, slot ^ 1u);
+                else if (tile + gridDim.x < n_tiles) issue(tile + gridDim.x, 0, slot ^ 1u);
             }
-            for (int l = 0; l < n_loads; ++l) {
-                const uint32_t c0 = __ldg(&p.loads[l].c0), c1 = __ldg(&p.loads[l].c1);
-                mbar_wait(bar_full + 8 * slot, phase);
-                const C* sp = stages + (size_t)slot * kTile;
-                for (uint32_t c = c0; c < c1; ++c, ++ck) {
-                    // chunk c is in tbuf[ck & 1] once every consumer has stashed it; the other buffer is free again
-                    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
-                    const uint32_t cn = c + 1 == (uint32_t)p.n_chunks ? 0u : c + 1;
-                    fetch(cn);
-                    const uint32_t ne = __ldg(&p.chunks[c].ne);
-                    const uint4* ent = tbuf + (ck & 1u) * kChunkEntries;
-                    uint32_t i = 0;
-                    while (i < ne) {
-                        const uint4 gh = ent[i];               // group header
-                        const uint32_t i_end = i + 1 + gh.y;
-                        T cr[kR], ci[kR];
+            const uint32_t c0 = __ldg(&p.loads[l].c0), c1 = __ldg(&p.loads[l].c1);
+            mbar_wait(bar_full + 8 * slot, (g >> 1) & 1u);
+            const C* sp = stages + (size_t)slot * kTile;
+            for (uint32_t c = c0; c < c1; ++c, ++ck) {
+                // chunk c is in tbuf[ck & 1] once every thread has stashed it; the other buffer is free again
+                __syncthreads();
+                const uint32_t cn = c + 1 == (uint32_t)p.n_chunks ? 0u : c + 1;
+                fetch(cn);
+                const uint32_t ne = __ldg(&p.chunks[c].ne);
+                const uint4* ent = tbuf + (ck & 1u) * kChunkEntries;
+                uint32_t i = 0;
+                while (i < ne) {
+                    const uint4 gh = ent[i];   // group header
+                    const uint32_t i_end = i + 1 + gh.y;
+                    T cr[kR], ci[kR];
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) {
+                        cr[r] = 0;
+                        ci[r] = 0;
+                    }
+                    // terms are sorted by bin; .w of the header says which bins occur, bit 8 of a term's .y closes
+                    // its bin.  The stream is read one entry ahead whatever the bin structure is.
+                    uint32_t t = i + 1;
+                    uint4 e = ent[t];
+                    walk_bins<T, 0>(ent, t, e, gh.w, bt, cr, ci);
+                    i = i_end;
+                    const C* pb = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
+                    const uint32_t xr = gh.x >> kThreadBitsD;
+                    if (gh.z == 1u) {          // real coefficients only
+                        wht(cr);
 #pragma unroll
                         for (int r = 0; r < kR; ++r) {
-                            cr[r] = 0;
-                            ci[r] = 0;
+                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                            ar[r] += cr[r] * v.x;
+                            ai[r] += cr[r] * v.y;
                         }
-                        // terms are sorted by bin; .w of the header says which bins occur, bit 8 of a term's .y closes
-                        // its bin.  The stream is read one entry ahead whatever the bin structure is.
-                        uint32_t t = i + 1;
-                        uint4 e = ent[t];
-                        walk_bins<T, 0>(ent, t, e, gh.w, bt, cr, ci);
-                        i = i_end;
-                        const C* pb = sp + ((uint32_t)tid ^ (gh.x & 255u));
-                        const uint32_t xr = gh.x >> 8;
-                        if (gh.z == 1u) {          // real coefficients only
-                            wht16(cr);
+                    } else if (gh.z == 2u) {   // imaginary coefficients only
+                        wht(ci);
 #pragma unroll
-                            for (int r = 0; r < kR; ++r) {
-                                const C v = pb[((uint32_t)r ^ xr) << 8];
-                                ar[r] += cr[r] * v.x;
-                                ai[r] += cr[r] * v.y;
-                            }
-                        } else if (gh.z == 2u) {   // imaginary coefficients only
-                            wht16(ci);
+                        for (int r = 0; r < kR; ++r) {
+                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                            ar[r] -= ci[r] * v.y;
+                            ai[r] += ci[r] * v.x;
+                        }
+                    } else {
+                        wht(cr);
+                        wht(ci);
 #pragma unroll
-                            for (int r = 0; r < kR; ++r) {
-                                const C v = pb[((uint32_t)r ^ xr) << 8];
-                                ar[r] -= ci[r] * v.y;
-                                ai[r] += ci[r] * v.x;
-                            }
-                        } else {
-                            wht16(cr);
-                            wht16(ci);
-#pragma unroll
-                            for (int r = 0; r < kR; ++r) {
-                                const C v = pb[((uint32_t)r ^ xr) << 8];
-                                ar[r] += cr[r] * v.x - ci[r] * v.y;
-                                ai[r] += cr[r] * v.y + ci[r] * v.x;
-                            }
+                        for (int r = 0; r < kR; ++r) {
+                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                            ar[r] += cr[r] * v.x - ci[r] * v.y;
+                            ai[r] += cr[r] * v.y + ci[r] * v.x;
                         }
                     }
-                    stash(ck + 1);
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
-                if (++slot == nslot) {
-                    slot = 0;
-                    phase ^= 1u;
-                }
+                stash(ck + 1);
             }
-            // epilogue (a tile takes milliseconds of arithmetic here: the latency of these global reads is nothing)
+        }
+        // epilogue (a tile takes milliseconds of arithmetic here: the latency of these global reads is nothing)
 #pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const uint64_t b = (uint64_t)base + (uint32_t)tid + r * kConsumerThreads;
-                C o;
-                if (FUSED) {
-                    const C mine = __ldg(p.in + b);
-                    double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
-                    if (p.prev) {
-                        const C pv = p.prev[b];
-                        orr -= s_prev * (double)pv.x;
-                        oi -= s_prev * (double)pv.y;
-                    }
-                    o.x = (T)orr;
-                    o.y = (T)oi;
-                    dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
-                } else {
-                    o.x = ar[r];
-                    o.y = ai[r];
+        for (int r = 0; r < kR; ++r) {
+            const uint64_t b = (uint64_t)base + (uint32_t)tid + r * kConsumerThreads;
+            C o;
+            if (FUSED) {
+                const C mine = __ldg(p.in + b);
+                double orr = (double)ar[r] * s_in, oi = (double)ai[r] * s_in;
+                if (p.prev) {
+                    const C pv = p.prev[b];
+                    orr -= s_prev * (double)pv.x;
+                    oi -= s_prev * (double)pv.y;
                 }
-                p.out[b] = o;
+                o.x = (T)orr;
+                o.y = (T)oi;
+                dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+            } else {
+                o.x = ar[r];
+                o.y = ai[r];
             }
+            p.out[b] = o;
         }
     }
     if (FUSED) {
@@ -341,7 +316,7 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
             const uint32_t z = (uint32_t)h->z[t];
             uint4 e;
             e.x = z;
-            e.y = ((z >> 8) & 15u) | (imag ? 16u : 0u);
+            e.y = ((z >> kThreadBitsD) & (uint32_t)(kR - 1)) | (imag ? (uint32_t)kR : 0u);
             if (dtype == SYK_C128) {
                 uint64_t bits;
                 std::memcpy(&bits, &a, 8);
@@ -423,14 +398,13 @@ int launch_dn(const syk_ham* h, const DenseCache& dc, const void* d_in, void* d_
     p.sc = fa.sc;
     p.j = fa.j;
     p.L = h->L;
-    p.nslot = (int)((kSmemLimit - kMiscBytes) / kTileBytes);
-    if (p.nslot > kMaxSlots) p.nslot = kMaxSlots;
+    p.nslot = 2;
     p.loads = (const DenseLoad*)dc.blob;
     p.chunks = (const DenseChunk*)((const unsigned char*)dc.blob + dc.off_groups);
     p.entries = (const uint4*)((const unsigned char*)dc.blob + dc.off_terms);
     p.n_loads = dc.n_loads;
     p.n_chunks = dc.n_chunks;
-    const size_t smem = (size_t)p.nslot * kTileBytes + kMiscBytes;
+    const size_t smem = 2 * kTileBytes + kMiscBytes;
     const int sms = num_sms();
     if (sms <= 0) return SYK_ECUDA;
     const uint64_t n_tiles = 1ull << (h->L - kTileLog2D);
