@@ -18,7 +18,7 @@
 // one, mbarrier completion); the table (a few MB, streamed once per output tile) is staged chunk by chunk in shared
 // memory by the threads themselves, double buffered, so the inner loops read it with broadcast LDS (read from global
 // with warp-uniform addresses, each term cost an exposed L2 latency: 1120 ms per N = 48 matvec).
-// History at N = 48 dense complex128: generic kernel 2390 ms; 8 warps x 16 amplitudes 692 ms; this shape 488 ms.
+// History at N = 48 dense complex128: generic kernel 2390 ms; 8 warps x 16 amplitudes 692 ms; this shape 450 ms.
 // No atomics on data, one write per output: bitwise reproducible.  Fused Lanczos epilogue as in apply_h.cu.
 #include <algorithm>
 #include <cstring>
@@ -108,16 +108,15 @@ __device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_
         if (occ & (1u << B)) {
             uint32_t last;
             do {
-                const uint4 cur = e;
-                ++t;
-                e = ent[t];   // t <= ne <= kChunkEntries - 1: always inside the buffer
-                const uint32_t sgn = (uint32_t)__popc(bt & cur.x) << 31;
+                const uint32_t sgn = (uint32_t)__popc(bt & e.x) << 31;
                 T a;
-                if constexpr (sizeof(T) == 8) a = __hiloint2double((int)(cur.w ^ sgn), (int)cur.z);
-                else a = __uint_as_float(cur.z ^ sgn);
+                if constexpr (sizeof(T) == 8) a = __hiloint2double((int)(e.w ^ sgn), (int)e.z);
+                else a = __uint_as_float(e.z ^ sgn);
                 if constexpr (B < kR) cr[B] += a;
                 else ci[B - kR] += a;
-                last = cur.y & 256u;
+                last = e.y & 256u;
+                ++t;
+                e = ent[t];   // t <= ne <= kChunkEntries - 1: always inside the buffer; four warps per scheduler hide it
             } while (!last);
         }
         walk_bins<T, B + 1>(ent, t, e, occ, bt, cr, ci);
