@@ -29,6 +29,7 @@ def main():
     ap.add_argument("--tol", type=float, default=0.0, help="0 = library default (1e-12 / 1e-6)")
     ap.add_argument("--block", action="store_true", help="work in the parity blocks (half-size vectors)")
     ap.add_argument("--green", action="store_true", help="Green function G(t) of gamma_{N-1} instead of the OTOC")
+    ap.add_argument("--batch", type=int, default=0, help="disorder realizations 0..batch-1 in lock step (syk_otoc_batched)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--realization", type=int, default=0)
     args = ap.parse_args()
@@ -45,6 +46,9 @@ def main():
     opts = {"krylov_dim": args.krylov_dim, "two_pass": int(args.two_pass), "tol": args.tol}
     t_grid = np.linspace(0.0, args.tmax, args.nt)
     iW, jV = N - 1, N - 2
+
+    if args.batch > 0:
+        return run_batch(args, B, torch, N, L, tdt, code, p, opts, t_grid, iW, jV)
 
     t0 = time.perf_counter()
     h = B.syk_build_hamiltonian(N, p, args.seed, args.realization)
@@ -93,6 +97,35 @@ def main():
            "seconds_setup": t1 - t0, "seconds_curve": t2 - t1, "seconds_per_point": (t2 - t1) / len(t_grid),
            "n_matvec": stats_tot["n_matvec"], "n_substeps": stats_tot["n_substeps"],
            "peak_device_GB": torch.cuda.max_memory_allocated() / 1e9}
+    print(json.dumps(out), flush=True)
+
+
+def run_batch(args, B, torch, N, L, tdt, code, p, opts, t_grid, iW, jV):
+    """BASELINE configs[1] shape: `batch` disorder realizations advanced in lock step (grid.y = realization); prints the
+    disorder-averaged curve both ways (mean of ratios, ratio of means: DESIGN.md R-F)."""
+    nb, D = args.batch, 1 << L
+    t0 = time.perf_counter()
+    hams = [B.syk_build_hamiltonian(N, p, args.seed, r) for r in range(nb)]
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    psi = torch.empty((nb, D), dtype=tdt, device="cuda")
+    for r in range(nb):
+        B.syk_random_state(N, args.seed, r, psi[r], scratch)
+    wk = torch.empty(B.syk_otoc_batched_workspace_bytes(hams[0], nb, code, opts), dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    B.syk_launch_count(reset=True)
+    t1 = time.perf_counter()
+    F, st = B.syk_otoc_batched(hams, iW, jV, args.beta, t_grid, psi, D, wk, opts)
+    torch.cuda.synchronize()
+    t2 = time.perf_counter()
+    ratio = (F / F[:, :1]).real
+    out = {"what": "otoc_batched", "N": N, "k": args.k, "beta": args.beta, "dtype": args.dtype, "realizations": nb,
+           "krylov_dim": args.krylov_dim, "n_points": len(t_grid), "t_max": float(t_grid[-1]),
+           "mean_of_ratios": ratio.mean(axis=0).tolist(),
+           "ratio_of_means": (F.mean(axis=0) / F.mean(axis=0)[0]).real.tolist(),
+           "std_of_ratios_last": float(ratio[:, -1].std()),
+           "seconds_setup": t1 - t0, "seconds_all_curves": t2 - t1, "seconds_per_point_per_realization": (t2 - t1) / len(t_grid) / nb,
+           "n_matvec": st["n_matvec"], "rounds": st["n_substeps"], "kernel_launches": B.syk_launch_count(),
+           "lanczos_steps_per_s": st["n_matvec"] / (t2 - t1), "peak_device_GB": torch.cuda.max_memory_allocated() / 1e9}
     print(json.dumps(out), flush=True)
 
 
