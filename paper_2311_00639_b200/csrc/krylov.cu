@@ -18,6 +18,7 @@
 #include <cmath>
 #include <complex>
 #include <cstddef>
+#include <thread>
 
 #include "common.h"
 
@@ -183,7 +184,7 @@ StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, 
             ch.noconv = true;   // forced: take the remainder in one step
         } else {
             double lo = 0.0, hi = remaining;
-            for (int it = 0; it < 60; ++it) {
+            for (int it = 0; it < 40; ++it) {
                 const double mid = 0.5 * (lo + hi);
                 if (fits(mid)) lo = mid; else hi = mid;
             }
@@ -367,19 +368,40 @@ int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, vo
         SYK_CUDA(cudaMemcpy2DAsync(nrm.data(), row, ws + offsetof(LanczosScalars, nrm), ws_stride, row, (size_t)nb,
                                    cudaMemcpyDeviceToHost, st));
         SYK_CUDA(cudaStreamSynchronize(st));
+        // the nb small exponentials are independent: spread them over a few host threads
+        std::vector<StepChoice> choice((size_t)nb);
+        std::vector<char> active((size_t)nb, 0);
+        auto work = [&](int r0, int r1) {
+            for (int r = r0; r < r1; ++r) {
+                const double* a = alpha.data() + (size_t)r * (kMaxKrylov + 2);
+                const double* nr = nrm.data() + (size_t)r * (kMaxKrylov + 2);
+                double2* cf = coef.data() + (size_t)r * (kMaxKrylov + 2);
+                for (int j = 0; j < kMaxKrylov + 2; ++j) cf[j] = make_double2(0.0, 0.0);
+                if (!(remaining[(size_t)r] > 1e-15 * len) || !(nr[1] > 0.0)) {
+                    cf[1] = make_double2(nr[1], 0.0);   // identity: psi stays what it is
+                    continue;
+                }
+                active[(size_t)r] = 1;
+                choice[(size_t)r] = choose_step(m, a, nr, dir, tol, len, remaining[(size_t)r], eps_break,
+                                                n_sub >= max_sub, cf);
+            }
+        };
+        {
+            const int n_thr = std::max(1, std::min({nb, 8, (int)std::thread::hardware_concurrency()}));
+            std::vector<std::thread> pool;
+            const int per = (nb + n_thr - 1) / n_thr;
+            for (int k = 1; k < n_thr; ++k)
+                if (k * per < nb) pool.emplace_back(work, k * per, std::min(nb, (k + 1) * per));
+            work(0, std::min(nb, per));
+            for (auto& th : pool) th.join();
+        }
         for (int r = 0; r < nb; ++r) {
-            const double* a = alpha.data() + (size_t)r * (kMaxKrylov + 2);
-            const double* nr = nrm.data() + (size_t)r * (kMaxKrylov + 2);
-            double2* cf = coef.data() + (size_t)r * (kMaxKrylov + 2);
-            for (int j = 0; j < kMaxKrylov + 2; ++j) cf[j] = make_double2(0.0, 0.0);
             meff[(size_t)r] = 1;
-            if (!(remaining[(size_t)r] > 1e-15 * len) || !(nr[1] > 0.0)) {
-                cf[1] = make_double2(nr[1], 0.0);   // identity: psi stays what it is
+            if (!active[(size_t)r]) {
                 remaining[(size_t)r] = 0.0;
                 continue;
             }
-            const StepChoice ch = choose_step(m, a, nr, dir, tol, len, remaining[(size_t)r], eps_break,
-                                              n_sub >= max_sub, cf);
+            const StepChoice& ch = choice[(size_t)r];
             if (ch.noconv) rc = SYK_ENOCONV;
             meff[(size_t)r] = ch.me;
             remaining[(size_t)r] -= ch.hs;
