@@ -49,12 +49,16 @@ def time_apply(B, torch, h, tdt, N, reps=5):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--quick", action="store_true", help="N <= 48 only (a few seconds)")
+    ap.add_argument("--lockstep", action="store_true",
+                    help="instead: sweep syk_set_lockstep(epoch, lag) for the two headline workloads and tile kernels")
     args = ap.parse_args()
     import torch
     from . import binding as B, inputs
 
     if not torch.cuda.is_available():
         raise SystemExit("sweep needs a CUDA device: the library has no CPU path")
+    if args.lockstep:
+        return lockstep_sweep(B, torch, inputs, args.quick)
     rows = []
 
     def run(label, N, h, tdt):
@@ -88,6 +92,48 @@ def main():
         slope, icpt = np.polyfit(x, y, 1)
         resid = float(np.max(np.abs(slope * x + icpt - y) / y))
         print(f"\nAffine fit of (i): time = {icpt:.3f} ms + {slope:.4f} ms x D_x, worst relative residual {resid:.3f}")
+
+
+def lockstep_sweep(B, torch, inputs, quick):
+    """Pacing of the persistent CTAs (syk_set_lockstep): plain syk_apply_H, minimum of 3 launches in ms, for the
+    register-tile (kind 2) and scatter-tile (kind 3) kernels; outputs are checked to be bitwise equal across settings."""
+    settings = [(0, 0), (1, 1), (2, 1), (2, 2), (4, 1), (4, 2), (8, 1), (8, 2), (16, 1), (32, 1)]
+    cases = [(48, 4, torch.complex128)] if quick else [(56, 4, torch.complex128), (64, 2, torch.complex64)]
+    print("| workload | kernel | " + " | ".join("free" if e == 0 else f"({e},{lag})" for e, lag in settings) + " |")
+    print("|---|---|" + "---|" * len(settings))
+    try:
+        for N, k, tdt in cases:
+            D = 1 << (N // 2)
+            h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, k), 0, 0)
+            scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+            a = torch.empty(D, dtype=tdt, device="cuda")
+            b = torch.empty(D, dtype=tdt, device="cuda")
+            B.syk_random_state(N, 0, 0, a, scratch)
+            for kind in (2, 3):
+                B.syk_set_apply_H_kernel(h, kind)
+                cells, ref = [], None
+                for e, lag in settings:
+                    B.syk_set_lockstep(e, lag)
+                    B.syk_apply_H(h, a, b)
+                    torch.cuda.synchronize()
+                    ts = []
+                    for _ in range(3):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        B.syk_apply_H(h, a, b)
+                        e1.record()
+                        torch.cuda.synchronize()
+                        ts.append(e0.elapsed_time(e1))
+                    chk = torch.view_as_real(b[: 1 << 20]).double().sum().item()
+                    ref = chk if ref is None else ref
+                    cells.append(f"{min(ts):.1f}" + ("" if chk == ref else " (!)"))
+                    print(f"# N={N} kind={kind} ({e},{lag}): {min(ts):.2f} ms", file=sys.stderr, flush=True)
+                name = "c128" if tdt == torch.complex128 else "c64"
+                print(f"| N={N} k={k} {name} | {kind} | " + " | ".join(cells) + " |")
+            del a, b
+            torch.cuda.empty_cache()
+    finally:
+        B.syk_set_lockstep(8, 1)
 
 
 if __name__ == "__main__":
