@@ -205,3 +205,39 @@ def test_apply_H_N66_parity_block_sampled(B):
     n2 = B.syk_dot(N - 2, d_out, d_out, scratch).real
     assert abs(n2 / float(np.sum(J ** 2)) - 1.0) <= 5e-3
     assert abs(B.syk_dot(N - 2, d_in, d_out, scratch).imag) <= 1e-6
+
+
+@pytest.mark.parametrize("N,k,seed", [(46, 4, 0), (46, 1, 1), (48, 8, 2), (50, 2, 3), (50, 16, 4), (52, 4, 5)])
+def test_scatter_kernel_many_layouts_sampled(B, N, k, seed):
+    """The scatter-tile kernel picks its tile / window bits per Hamiltonian: different seeds and sparsities give
+    different layouts (free r bits low, high, adjacent; few or many loads).  Sampled outputs of both precisions against
+    the oracle's monomial rows, plain and through a forced register-tile run of the same product."""
+    import torch
+    D = 1 << (N // 2)
+    p = inputs.bernoulli_p(N, k)
+    q, J, _ = orng.sample_couplings(N, p, seed, 0)
+    h = B.syk_build_hamiltonian(N, p, seed, 0)
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    idx = inputs.sample_indices(D, 300, seed=31 + seed)
+    didx = torch.from_numpy(idx.astype(np.int64)).cuda()
+    for tdt, tol in ((torch.complex128, 1e-10), (torch.complex64, 1e-5)):
+        code = B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64
+        B.syk_set_apply_H_kernel(h, 3)
+        if B.syk_apply_H_kernel_kind(h, code) != 3:
+            pytest.skip("more than 1024 terms")
+        lay = B.syk_apply_H_layout(h, code)
+        assert 1 <= lay["n_passes"] <= lay["n_loads"] <= h.info()["n_xmasks"]
+        assert lay["tile_mask"] & 0x7FF == 0x7FF and lay["window_mask"] & lay["tile_mask"] == lay["tile_mask"]
+        d_in = torch.empty(D, dtype=tdt, device="cuda")
+        d_out = torch.empty(D, dtype=tdt, device="cuda")
+        B.syk_random_state(N, seed, 7, d_in, scratch)
+        B.syk_apply_H(h, d_in, d_out)
+        ref = _oracle_samples(N, q, J, idx, d_in)
+        got = d_out[didx].cpu().numpy().astype(np.complex128)
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= tol, (N, k, seed, lay)
+        B.syk_set_apply_H_kernel(h, 2)
+        d_out2 = torch.empty(D, dtype=tdt, device="cuda")
+        B.syk_apply_H(h, d_in, d_out2)
+        diff = float(torch.linalg.vector_norm(d_out - d_out2) / torch.linalg.vector_norm(d_out2))
+        assert diff <= tol
+        del d_in, d_out, d_out2
