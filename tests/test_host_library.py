@@ -301,3 +301,26 @@ def test_N66_only_through_parity_blocks(B):
         B.syk_krylov_workspace_bytes(h, B.SYK_C64, {"krylov_dim": 4})
     with pytest.raises(B.SykError):
         B.syk_build_hamiltonian(68, 1e-4, 0, 0)
+
+
+def test_scatter_layout_choice_on_host(B):
+    """The per-Hamiltonian tile layout of the scatter-tile kernel (host-side hill climbing): deterministic, never worse
+    than the identity layout (tile = low bits), consistent with a direct count from the X-masks, and it does reduce
+    loads and passes for the two headline Hamiltonians."""
+    for N, k, code, tb in ((56, 4, B.SYK_C128, 8), (64, 2, B.SYK_C64, 9), (48, 4, B.SYK_C128, 8)):
+        p = inputs.bernoulli_p(N, k)
+        h = B.syk_build_hamiltonian(N, p, 0, 0)
+        lay = B.syk_apply_H_layout(h, code)
+        lay2 = B.syk_apply_H_layout(B.syk_build_hamiltonian(N, p, 0, 0), code)
+        assert lay == lay2
+        x = [int(v) for v in h.tables()["x"]]
+        tile, win = lay["tile_mask"], lay["window_mask"]
+        assert bin(tile).count("1") == tb + 5 and tile & ((1 << (tb + 3)) - 1) == (1 << (tb + 3)) - 1
+        assert win & tile == tile and bin(win).count("1") == min(tb + 5 + 7, N // 2)
+        assert lay["n_loads"] == len({v & ~tile for v in x})
+        assert lay["n_passes"] == len({v & ~win for v in x})
+        ident_tile = (1 << (tb + 5)) - 1
+        ident_win = (1 << min(tb + 12, N // 2)) - 1
+        assert lay["n_loads"] + 2 * lay["n_passes"] <= len({v & ~ident_tile for v in x}) + 2 * len({v & ~ident_win for v in x})
+        if N >= 56:
+            assert lay["n_loads"] < len({v & ~ident_tile for v in x}) and lay["n_passes"] < len({v & ~ident_win for v in x})
