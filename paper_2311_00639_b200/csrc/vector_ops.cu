@@ -49,9 +49,7 @@ inline uint64_t n_units(int dtype, uint64_t D) { return dtype == SYK_C128 ? D : 
 
 inline int grid_for(uint64_t units) {
     const int sms = num_sms();
-    // at least 8 units per thread: the reducing kernels pay a fixed prologue / epilogue per block (sum of the previous
-    // kernel's partials, block reduction), which dominated the small vectors of the batched path
-    uint64_t blocks = (units + (uint64_t)kThreads * 8 - 1) / ((uint64_t)kThreads * 8);
+    uint64_t blocks = (units + kThreads - 1) / kThreads;
     uint64_t cap = (uint64_t)(sms > 0 ? sms : 1) * 8;
     if (cap > (uint64_t)kMaxPartials) cap = kMaxPartials;
     if (blocks < 1) blocks = 1;
