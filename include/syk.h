@@ -232,7 +232,8 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
  * 3 = TMA-pipelined scatter-tile gather (128 KiB tiles on index bits chosen per Hamiltonian; sparse H with
  *     1..1024 terms and D >= 2^23 / 2^24),
  * 4 = dense-table kernel (many terms per X-mask: terms binned by the Walsh index of their Z-mask and transformed once per
- *     X-mask; chosen for > 1024 terms with >= 4 terms per X-mask and D >= 2^16; holds its own device table). */
+ *     X-mask; chosen for > 1024 terms with >= 4 terms per X-mask and D >= 2^12; holds its own device table and, for
+ *     vectors with fewer tiles than SMs, a scratch buffer for partial sums). */
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
 /* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 / 4 as above
  * (a kind the handle cannot use falls back to the next lower one). */

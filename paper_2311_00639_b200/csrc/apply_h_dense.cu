@@ -123,6 +123,177 @@ __device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_
     }
 }
 
+// All groups of one staged table chunk applied to the thread's kR accumulators; `sp` = the staged source tile.
+template <typename T>
+__device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uint32_t ne, const typename Cx<T>::type* sp,
+                                              uint32_t bt, int tid, T (&ar)[kR], T (&ai)[kR]) {
+    using C = typename Cx<T>::type;
+    uint32_t i = 0;
+    while (i < ne) {
+        const uint4 gh = ent[i];   // group header
+        const uint32_t i_end = i + 1 + gh.y;
+        T cr[kR], ci[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            cr[r] = 0;
+            ci[r] = 0;
+        }
+        // terms are sorted by bin; .w of the header says which bins occur, bit 8 of a term's .y closes its bin
+        uint32_t t = i + 1;
+        uint4 e = ent[t];
+        walk_bins<T, 0>(ent, t, e, gh.w, bt, cr, ci);
+        i = i_end;
+        const C* pb = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
+        const uint32_t xr = gh.x >> kThreadBitsD;
+        if (gh.z == 1u) {          // real coefficients only
+            wht(cr);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                ar[r] += cr[r] * v.x;
+                ai[r] += cr[r] * v.y;
+            }
+        } else if (gh.z == 2u) {   // imaginary coefficients only
+            wht(ci);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                ar[r] -= ci[r] * v.y;
+                ai[r] += ci[r] * v.x;
+            }
+        } else {
+            wht(cr);
+            wht(ci);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
+                ar[r] += cr[r] * v.x - ci[r] * v.y;
+                ai[r] += cr[r] * v.y + ci[r] * v.x;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Small vectors (fewer tiles than SMs: dense N <= 38 in a parity block, N <= 36 in the full space): the table is cut
+// into `split` contiguous ranges of chunks and work item (tile, s) applies range s to tile `tile`, writing its partial
+// sums to scratch; a second kernel adds the `split` partials in a fixed order and does the (fused) epilogue.  No
+// atomics: still bitwise reproducible.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+struct DnSplitParams {
+    using C = typename Cx<T>::type;
+    const C* in;
+    C* partial;                 // [split][D]
+    int L;
+    int split;
+    const uint32_t* range;      // [split + 1] chunk indices
+    const DenseChunk* chunks;   // .pad0 = hi of the load the chunk belongs to
+    const uint4* entries;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads, 1) apply_h_dense_split_kernel(const DnSplitParams<T> p) {
+    using C = typename Cx<T>::type;
+    constexpr uint32_t TILE_BYTES = kTile * sizeof(C);
+    constexpr uint32_t kChunk = 16384;
+    extern __shared__ __align__(128) unsigned char smem[];
+    C* stage = reinterpret_cast<C*>(smem);
+    uint4* tbuf = reinterpret_cast<uint4*>(smem + TILE_BYTES);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + TILE_BYTES + kChunkEntries * sizeof(uint4));
+    const int tid = threadIdx.x;
+    const uint32_t bar_full = smem_u32(bar);
+    if (tid == 0) {
+        mbar_init(bar_full, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const uint32_t tile = blockIdx.x / (uint32_t)p.split, s = blockIdx.x % (uint32_t)p.split;
+    const uint32_t base = tile << kTileLog2D;
+    const uint32_t bt = base | (uint32_t)tid;
+    T ar[kR], ai[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        ar[r] = 0;
+        ai[r] = 0;
+    }
+    uint32_t cur_hi = 0xffffffffu, n_loaded = 0;
+    const uint32_t cA = __ldg(p.range + s), cB = __ldg(p.range + s + 1);
+    for (uint32_t c = cA; c < cB; ++c) {
+        const uint32_t e0 = __ldg(&p.chunks[c].e0), ne = __ldg(&p.chunks[c].ne), hi = __ldg(&p.chunks[c].pad0);
+        __syncthreads();   // everyone is done with the staged tile and the staged table chunk
+        const bool new_tile = hi != cur_hi;
+        if (new_tile) {
+            if (tid == 0) {
+                mbar_arrive_expect_tx(bar_full, TILE_BYTES);
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(p.in + ((uint64_t)(tile ^ hi) << kTileLog2D));
+#pragma unroll
+                for (uint32_t k = 0; k < TILE_BYTES; k += kChunk) bulk_load(smem_u32(stage) + k, src + k, kChunk, bar_full);
+            }
+            cur_hi = hi;
+        }
+        tbuf[tid] = (uint32_t)tid < ne ? __ldg(p.entries + e0 + tid) : make_uint4(0, 0, 0, 0);
+        __syncthreads();
+        if (new_tile) {
+            mbar_wait(bar_full, n_loaded & 1u);
+            ++n_loaded;
+        }
+        process_chunk<T>(tbuf, ne, stage, bt, tid, ar, ai);
+    }
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        C o;
+        o.x = ar[r];
+        o.y = ai[r];
+        p.partial[((uint64_t)s << p.L) + (uint64_t)base + (uint32_t)tid + r * kConsumerThreads] = o;
+    }
+}
+
+// out[b] = sum_s partial[s][b] (fixed order) with the epilogue of the other apply_H kernels
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(256) dense_reduce_kernel(const typename Cx<T>::type* partial, int split, int L,
+                                                           const typename Cx<T>::type* in, typename Cx<T>::type* out,
+                                                           const typename Cx<T>::type* prev, LanczosScalars* sc, int j) {
+    using C = typename Cx<T>::type;
+    __shared__ double red[40];
+    double s_in = 1.0, s_prev = 0.0;
+    if (FUSED) dn_fused_scalars(sc, j, red, s_in, s_prev);
+    const uint64_t D = 1ull << L;
+    double dot = 0.0;
+    for (uint64_t b = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; b < D; b += (uint64_t)gridDim.x * blockDim.x) {
+        T ar = 0, ai = 0;
+        for (int s = 0; s < split; ++s) {
+            const C v = partial[((uint64_t)s << L) + b];
+            ar += v.x;
+            ai += v.y;
+        }
+        C o;
+        if (FUSED) {
+            const C mine = in[b];
+            double orr = (double)ar * s_in, oi = (double)ai * s_in;
+            if (prev) {
+                const C pv = prev[b];
+                orr -= s_prev * (double)pv.x;
+                oi -= s_prev * (double)pv.y;
+            }
+            o.x = (T)orr;
+            o.y = (T)oi;
+            dot += (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+        } else {
+            o.x = ar;
+            o.y = ai;
+        }
+        out[b] = o;
+    }
+    if (FUSED) {
+        double s = block_sum(dot, red);
+        if (threadIdx.x == 0) {
+            sc->partial_dot[blockIdx.x] = s;
+            if (blockIdx.x == 0) sc->n_partial_dot = gridDim.x;
+        }
+    }
+}
+
 template <typename T, bool FUSED>
 __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnParams<T> p) {
     using C = typename Cx<T>::type;
@@ -202,51 +373,7 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnPara
                 fetch(cn);
                 const uint32_t ne = __ldg(&p.chunks[c].ne);
                 const uint4* ent = tbuf + (ck & 1u) * kChunkEntries;
-                uint32_t i = 0;
-                while (i < ne) {
-                    const uint4 gh = ent[i];   // group header
-                    const uint32_t i_end = i + 1 + gh.y;
-                    T cr[kR], ci[kR];
-#pragma unroll
-                    for (int r = 0; r < kR; ++r) {
-                        cr[r] = 0;
-                        ci[r] = 0;
-                    }
-                    // terms are sorted by bin; .w of the header says which bins occur, bit 8 of a term's .y closes
-                    // its bin.  The stream is read one entry ahead whatever the bin structure is.
-                    uint32_t t = i + 1;
-                    uint4 e = ent[t];
-                    walk_bins<T, 0>(ent, t, e, gh.w, bt, cr, ci);
-                    i = i_end;
-                    const C* pb = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
-                    const uint32_t xr = gh.x >> kThreadBitsD;
-                    if (gh.z == 1u) {          // real coefficients only
-                        wht(cr);
-#pragma unroll
-                        for (int r = 0; r < kR; ++r) {
-                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                            ar[r] += cr[r] * v.x;
-                            ai[r] += cr[r] * v.y;
-                        }
-                    } else if (gh.z == 2u) {   // imaginary coefficients only
-                        wht(ci);
-#pragma unroll
-                        for (int r = 0; r < kR; ++r) {
-                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                            ar[r] -= ci[r] * v.y;
-                            ai[r] += ci[r] * v.x;
-                        }
-                    } else {
-                        wht(cr);
-                        wht(ci);
-#pragma unroll
-                        for (int r = 0; r < kR; ++r) {
-                            const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                            ar[r] += cr[r] * v.x - ci[r] * v.y;
-                            ai[r] += cr[r] * v.y + ci[r] * v.x;
-                        }
-                    }
-                }
+                process_chunk<T>(ent, ne, sp, bt, tid, ar, ai);
                 stash(ck + 1);
             }
         }
@@ -301,7 +428,7 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
             loads.push_back(DenseLoad{hi, (uint32_t)chunks.size(), 0u, 0u});
         }
         if (new_load || chunks.back().ne + nt + 1 > (uint32_t)kChunkEntries - 1)   // one spare entry: read-ahead
-            chunks.push_back(DenseChunk{(uint32_t)entries.size(), 0u, 0u, 0u});
+            chunks.push_back(DenseChunk{(uint32_t)entries.size(), 0u, hi, 0u});
         uint32_t flags = 0, occ = 0;
         const size_t header_at = entries.size();
         entries.push_back(make_uint4(x & (uint32_t)(kTile - 1), nt, 0u, 0u));
@@ -366,6 +493,29 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
     dc.off_terms = off_e;
     dc.n_loads = (int)loads.size();
     dc.n_chunks = (int)chunks.size();
+    // small vectors: split the chunk list over several CTAs per tile (apply_h_dense_split_kernel)
+    dc.split = 1;
+    const int sms = num_sms();
+    const uint64_t n_tiles = 1ull << (h->L - kTileLog2D);
+    if (sms > 0 && n_tiles * 2 <= (uint64_t)sms && chunks.size() >= 2) {
+        int split = (int)((uint64_t)(2 * sms) / n_tiles);
+        if (split > (int)chunks.size()) split = (int)chunks.size();
+        if (split > 64) split = 64;
+        std::vector<uint32_t> range((size_t)split + 1);
+        for (int s2 = 0; s2 <= split; ++s2) range[(size_t)s2] = (uint32_t)((uint64_t)chunks.size() * s2 / split);
+        const size_t pbytes = (size_t)split * ((size_t)elem_bytes(dtype) << h->L);
+        void* scratch = nullptr;
+        SYK_CUDA(cudaMalloc(&scratch, pbytes + 4096));
+        cudaError_t e2 = cudaMemcpy((char*)scratch + pbytes, range.data(), range.size() * 4, cudaMemcpyHostToDevice);
+        if (e2 != cudaSuccess) {
+            cudaFree(scratch);
+            set_cuda_error(e2, "cudaMemcpy(dense split ranges)");
+            return SYK_ECUDA;
+        }
+        dc.partial = scratch;
+        dc.range = (const uint32_t*)((char*)scratch + pbytes);
+        dc.split = split;
+    }
     return SYK_OK;
 }
 
@@ -378,6 +528,7 @@ int get_dense_tables(const syk_ham* h, int dtype, const DenseCache** out) {
     DenseCache& dc = *h->dn[k];
     if (dc.blob && dc.device != dev) {
         cudaFree(dc.blob);
+        if (dc.partial) cudaFree(dc.partial);
         dc = DenseCache();
     }
     if (!dc.blob) SYK_TRY(build_dense_tables(h, dtype, dc));
@@ -406,6 +557,31 @@ int launch_dn(const syk_ham* h, const DenseCache& dc, const void* d_in, void* d_
     const size_t smem = 2 * kTileBytes + kMiscBytes;
     const int sms = num_sms();
     if (sms <= 0) return SYK_ECUDA;
+    if (dc.split > 1) {
+        DnSplitParams<T> sp;
+        sp.in = (const C*)d_in;
+        sp.partial = (C*)dc.partial;
+        sp.L = h->L;
+        sp.split = dc.split;
+        sp.range = dc.range;
+        sp.chunks = p.chunks;
+        sp.entries = p.entries;
+        const size_t smem2 = kTileBytes + (size_t)kChunkEntries * sizeof(uint4) + 64;
+        const unsigned n_items = (unsigned)((1ull << (h->L - kTileLog2D)) * (uint64_t)dc.split);
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_dense_split_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+        apply_h_dense_split_kernel<T><<<n_items, kThreads, smem2, stream>>>(sp);
+        const uint64_t D = 1ull << h->L;
+        const unsigned gr = (unsigned)std::min<uint64_t>((D + 255) / 256, (uint64_t)sms * 4);
+        if (fa.sc)
+            dense_reduce_kernel<T, true><<<gr, 256, 0, stream>>>((const C*)dc.partial, dc.split, h->L, (const C*)d_in, (C*)d_out,
+                                                                (const C*)fa.prev, fa.sc, fa.j);
+        else
+            dense_reduce_kernel<T, false><<<gr, 256, 0, stream>>>((const C*)dc.partial, dc.split, h->L, (const C*)d_in, (C*)d_out,
+                                                                 nullptr, nullptr, 0);
+        count_launch(2);
+        SYK_CUDA(cudaGetLastError());
+        return SYK_OK;
+    }
     const uint64_t n_tiles = 1ull << (h->L - kTileLog2D);
     const int grid = (int)(n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms);
     if (fa.sc) {
@@ -422,12 +598,12 @@ int launch_dn(const syk_ham* h, const DenseCache& dc, const void* d_in, void* d_
 
 }  // namespace
 
-// Can the handle use the dense-table kernel?  Automatic choice: many terms per X-mask and at least 16 tiles (measured at
-// N = 38 dense in one parity block, 64 tiles: 6 ms per product against 22 ms with the generic kernel).
+// Can the handle use the dense-table kernel?  Automatic choice: many terms per X-mask (vectors with fewer tiles than SMs
+// take the split form: the table is shared out over several CTAs per tile).
 bool dense_kernel_ok(const syk_ham* h, bool forced) {
     if (h->n_terms() == 0 || h->L < kTileLog2D) return false;
     if (forced) return true;
-    return h->L >= kTileLog2D + 4 && h->n_terms() >= 4 * h->n_groups() && h->n_terms() > kRtMaxTerms;
+    return h->n_terms() >= 4 * h->n_groups() && h->n_terms() > kRtMaxTerms;   // any vector of at least one tile
 }
 
 int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
@@ -442,6 +618,7 @@ void free_dense_tables(const syk_ham* h) {
     for (int k = 0; k < 2; ++k) {
         if (h->dn[k]) {
             if (h->dn[k]->blob) cudaFree(h->dn[k]->blob);
+            if (h->dn[k]->partial) cudaFree(h->dn[k]->partial);
             delete h->dn[k];
             h->dn[k] = nullptr;
         }

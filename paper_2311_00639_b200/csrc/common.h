@@ -76,6 +76,10 @@ struct DenseCache {
     int device = -1;
     size_t off_groups = 0, off_terms = 0;   // byte offsets of the chunk list and of the entry stream
     int n_loads = 0, n_chunks = 0;
+    // small vectors: `split` CTAs per tile, each with a range of chunks; partial sums in `partial` ([split][D], owned)
+    int split = 1;
+    void* partial = nullptr;
+    const uint32_t* range = nullptr;
 };
 }  // namespace syk
 
