@@ -83,9 +83,10 @@ struct SmallExp {
             acc += Q[(size_t)j * m + k] * std::exp(cplx(0.0, -1.0) * dir * (s * theta[k])) * Q[k];
         return acc;
     }
+    // |exp(-i dir s T) e_1|: Q is orthogonal, so the norm is that of the coefficient vector in the eigenbasis
     double result_norm(double s) const {
         double n2 = 0.0;
-        for (int j = 0; j < m; ++j) n2 += std::norm(comp(j, s));
+        for (int k = 0; k < m; ++k) n2 += std::norm(std::exp(cplx(0.0, -1.0) * dir * (s * theta[k]))) * Q[k] * Q[k];
         return std::sqrt(n2);
     }
     double residual(double s) const { return beta_next * std::abs(comp(m - 1, s)); }
@@ -184,7 +185,7 @@ StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, 
             ch.noconv = true;   // forced: take the remainder in one step
         } else {
             double lo = 0.0, hi = remaining;
-            for (int it = 0; it < 40; ++it) {
+            for (int it = 0; it < 14; ++it) {   // the step length needs no precision: `lo` always fits the budget
                 const double mid = 0.5 * (lo + hi);
                 if (fits(mid)) lo = mid; else hi = mid;
             }
