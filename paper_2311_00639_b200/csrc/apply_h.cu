@@ -122,6 +122,74 @@ __global__ void __launch_bounds__(256) apply_h_generic_kernel(Params<T> p) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// generic kernel for tiny vectors with many X-masks (dense N <= 24: 256..4096 amplitudes, thousands of terms): one
+// amplitude per LANE, the groups shared out over the 32 warps of the block (warp w takes groups w, w + 32, ...), partial
+// sums added across warps in a fixed order.  The plain generic kernel walks all terms serially in every thread
+// (75 us per product at N = 16 dense); this one is bounded by launch latency.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(1024) apply_h_small_kernel(Params<T> p) {
+    using C = typename Cx<T>::type;
+    __shared__ double red[40];
+    __shared__ T part[32][32][2];
+    double s_in = 1.0, s_prev = 0.0;
+    if (FUSED) fused_prologue(p.sc, p.j, red, s_in, s_prev);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t b32 = blockIdx.x * 32u + (uint32_t)lane;
+    T ar = 0, ai = 0;
+    for (int g = warp; g < p.n_groups; g += 32) {
+        const uint32_t x = __ldg(p.gx + g);
+        const uint32_t t0 = __ldg(p.goff + g), t1 = __ldg(p.goff + g + 1);
+        T cr = 0, ci = 0;
+        for (uint32_t t = t0; t < t1; ++t) {
+            const uint32_t sbit = (__popc(b32 & __ldg(p.tz + t)) & 1u) << 31;
+            const C c = __ldg(p.tc + t);
+            cr += flip_sign(c.x, sbit);
+            ci += flip_sign(c.y, sbit);
+        }
+        const C v = __ldg(p.in + (b32 ^ x));
+        ar += cr * v.x - ci * v.y;
+        ai += cr * v.y + ci * v.x;
+    }
+    part[warp][lane][0] = ar;
+    part[warp][lane][1] = ai;
+    __syncthreads();
+    double dot = 0.0;
+    if (warp == 0) {
+        T sr = 0, si = 0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) {
+            sr += part[w][lane][0];
+            si += part[w][lane][1];
+        }
+        C o;
+        if (FUSED) {
+            const C mine = __ldg(p.in + b32);
+            double orr = (double)sr * s_in, oi = (double)si * s_in;
+            if (p.prev) {
+                const C pv = p.prev[b32];
+                orr -= s_prev * (double)pv.x;
+                oi -= s_prev * (double)pv.y;
+            }
+            o.x = (T)orr;
+            o.y = (T)oi;
+            dot = (double)mine.x * (double)o.x + (double)mine.y * (double)o.y;
+        } else {
+            o.x = sr;
+            o.y = si;
+        }
+        p.out[b32] = o;
+    }
+    if (FUSED) {
+        double s = block_sum(dot, red);
+        if (threadIdx.x == 0) {
+            p.sc->partial_dot[blockIdx.x] = s;
+            if (blockIdx.x == 0) p.sc->n_partial_dot = gridDim.x;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // TMA-pipelined tile kernel.  R = outputs per consumer thread; tile = R * 256 amplitudes = 16 KiB.
 // ---------------------------------------------------------------------------------------------------------
 template <typename T, int R, bool FUSED>
@@ -382,6 +450,12 @@ int launch_typed(const syk_ham* h, const void* d_in, void* d_out, const FusedArg
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             apply_h_tma_kernel<T, R, false><<<grid, kTmaThreads, smem, stream>>>(p);
         }
+    } else if (h->L >= 5 && h->L <= 12 && p.n_groups >= 64) {
+        const int grid = (int)(1u << (h->L - 5));
+        if (fused)
+            apply_h_small_kernel<T, true><<<grid, 1024, 0, stream>>>(p);
+        else
+            apply_h_small_kernel<T, false><<<grid, 1024, 0, stream>>>(p);
     } else {
         const uint64_t D = 1ull << h->L;
         uint64_t blocks = (D + 255) / 256;
