@@ -14,8 +14,14 @@
  *   - Pointers named d_* are DEVICE pointers owned by the caller, 16-byte aligned; pointers named h_* and all
  *     other pointers are HOST pointers.  The library never allocates device vectors: work space is passed in
  *     (the memory discipline is part of the method).  The only device memory the library
- *     owns is the per-Hamiltonian term table (a few KB for sparse H, <= ~8 MB for dense N=48), allocated on
- *     first device use of a handle and released by syk_free_hamiltonian.
+ *     owns belongs to a handle and is released by syk_free_hamiltonian: the term table (a few KB for sparse H,
+ *     <= ~8 MB for dense N=48) and, for the dense-table kernel on vectors with fewer tiles than SMs, a scratch
+ *     buffer of partial sums (<= 64 vectors of <= 2^19 amplitudes).  syk_ham_prepare allocates and uploads all
+ *     of it; after that no compute call allocates.  A handle that was not prepared does the same lazily inside
+ *     its first compute call (one synchronous cudaMalloc + copy).
+ *   - A handle is not thread-safe and must not be used by two launches that are in flight at the same time
+ *     (different streams or threads): the lazily built table caches, the split scratch and the pacing counters
+ *     of the tile kernels belong to the handle.  Different handles are independent.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and return, except
  *     where they hand back host scalars (syk_krylov_evolve, syk_otoc, syk_lanczos_run, *_host): those
  *     synchronise that stream only.
@@ -82,6 +88,12 @@ int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, 
  * z[n_terms], c_re_im[n_terms][2], quartet_of_term[n_terms][4], J_of_term[n_terms]. */
 int syk_ham_tables(const syk_ham* h, uint64_t* x, uint32_t* group_off, uint64_t* z, double* c_re_im,
                    int32_t* quartet_of_term, double* J_of_term);
+
+/* Creates the device copy of the term tables of `h` on the current device for `dtype` (and, for the dense-table
+ * kernel, its entry stream and split scratch): after this call syk_apply_H / syk_lanczos_run / syk_krylov_evolve /
+ * syk_otoc / syk_green on this handle and dtype allocate nothing (few allocation calls).  Synchronous
+ * (cudaMalloc + cudaMemcpy).  Call again after syk_set_apply_H_kernel or after switching devices. */
+int syk_ham_prepare(const syk_ham* h, int dtype);
 
 /* ------------------------------------------------------------------------------------------------------------
  * a-2  apply_H (device).  Algorithm 1, in gather form:
@@ -238,6 +250,11 @@ int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
 /* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 / 4 as above
  * (a kind the handle cannot use falls back to the next lower one). */
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
+/* Shape of the dense-table kernel's (kind 4) device table for this handle: n_loads source tiles per output tile,
+ * n_chunks table chunks of <= 512 entries streamed per output tile, split = CTAs that share one output tile (1 = the
+ * persistent one-CTA-per-tile form; > 1 = the split form for vectors with fewer tiles than SMs).  Builds the table if
+ * needed.  Any output pointer may be NULL.  SYK_EINVAL if the handle cannot use kind 4. */
+int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split);
 /* Tile layout the scatter-tile kernel (kind 3) chose for this Hamiltonian: n_loads = source tiles fetched per
  * output tile (L2 -> SM transfers of the whole vector per product), n_passes = distinct X-masks outside tile and
  * L2-window bits (DRAM reads of the whole vector per product, if L2 reuse were perfect), tile_mask / window_mask =
@@ -259,6 +276,26 @@ int64_t syk_launch_count(int reset);
  * and, when `reset` is non-zero, forgets them.  Any output pointer may be NULL. */
 int syk_profile_enable(int on);
 int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * On-chip peak measurements (denominators of the benchmark's roofline; SURVEY section 7 "hard parts": the HBM copy
+ * peak is known, the L2 -> SM, shared-memory and ALU-issue peaks of this box are not).  One launch of 1 CTA per SM:
+ *   kind 0: every CTA streams arg0 chunks of 64 KiB from d_buf (walked pseudo-randomly; a buffer of <= 32 MB stays in
+ *           L2, a multi-GB one streams from DRAM) into the 3-chunk shared-memory ring of the scatter-tile kernel with
+ *           cp.async.bulk, no arithmetic;
+ *   kind 1: no copies; the 8 consumer warps make arg1 passes over each of arg0 staged chunks with the kernel's
+ *           XOR-permuted LDS.128 + 2 FP64 FMA per element;
+ *   kind 2: both at once (arg1 passes over every chunk that arrives);
+ *   kind 3: arg0 x 64 FP64 adds per thread in 8 independent chains, 512 threads per SM;
+ *   kind 4: arg0 x 64 times the per-term sequence of the dense-table kernel (broadcast LDS of a table entry, AND, POPC,
+ *           shift, XOR into the sign bit, FP64 add into one of 8 bin registers), 512 threads per SM.
+ * result[0] = device time in ms (CUDA events), result[1] = SM cycles of the slowest CTA (clock64), result[2] = bytes
+ * copied into shared memory (kinds 0, 2) or thread-level adds (kinds 3, 4), result[3] = bytes read by LDS (kinds 1, 2).
+ * d_work: >= syk_microbench_workspace_bytes() of device memory; d_buf (kinds 0, 2): 128-byte aligned, buf_bytes >= 128 KiB
+ * (rounded down to a power of two).  Synchronises. */
+size_t syk_microbench_workspace_bytes(void);
+int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_bytes, void* d_work, size_t work_bytes,
+                   double* result, void* stream);
 
 #ifdef __cplusplus
 }

@@ -58,6 +58,8 @@ _SIGNATURES = {
     "syk_free_hamiltonian": (None, [_vp]),
     "syk_ham_info": (_i, [_vp, _P(_i), _P(_i64), _P(_i64), _P(_i64)]),
     "syk_ham_tables": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "syk_ham_prepare": (_i, [_vp, _i]),
+    "syk_apply_H_dense_info": (_i, [_vp, _i, _P(_i), _P(_i), _P(_i)]),
     "syk_apply_H": (_i, [_vp, _i, _vp, _vp, _vp]),
     "syk_apply_H_batched": (_i, [_P(_vp), _i, _i, _vp, _vp, _i64, _vp]),
     "syk_apply_H_host": (_i, [_vp, _i, _vp, _vp, _vp, _sz, _vp]),
@@ -89,6 +91,8 @@ _SIGNATURES = {
     "syk_set_lockstep": (_i, [_i, _i]),
     "syk_apply_H_layout": (_i, [_vp, _i, _P(_i), _P(_i), _P(_u32), _P(_u32)]),
     "syk_launch_count": (_i64, [_i]),
+    "syk_microbench_workspace_bytes": (_sz, []),
+    "syk_microbench": (_i, [_i, _i, _i, _vp, _sz, _vp, _sz, _P(_d), _vp]),
     "syk_profile_enable": (_i, [_i]),
     "syk_profile_read": (_i, [_P(_d), _P(_i64), _i]),
 }
@@ -224,6 +228,17 @@ def syk_ham_tables(h):
     _check(_lib.syk_ham_tables(_h(h), x.ctypes.data, off.ctypes.data, z.ctypes.data, c.ctypes.data,
                                quart.ctypes.data, J.ctypes.data), "syk_ham_tables")
     return {"x": x, "group_off": off, "z": z, "c": c[:, 0] + 1j * c[:, 1], "quartet_of_term": quart, "J": J}
+
+
+def syk_ham_prepare(h, dtype):
+    _check(_lib.syk_ham_prepare(_h(h), int(dtype)), "syk_ham_prepare")
+
+
+def syk_apply_H_dense_info(h, dtype):
+    nl, nc, sp = _i(), _i(), _i()
+    _check(_lib.syk_apply_H_dense_info(_h(h), int(dtype), ctypes.byref(nl), ctypes.byref(nc), ctypes.byref(sp)),
+           "syk_apply_H_dense_info")
+    return {"n_loads": nl.value, "n_chunks": nc.value, "split": sp.value}
 
 
 # ---- a-2 ---------------------------------------------------------------------------------------------------
@@ -462,6 +477,19 @@ def syk_profile_read(reset=True):
     ms, n = ctypes.c_double(), ctypes.c_int64()
     _check(_lib.syk_profile_read(ctypes.byref(ms), ctypes.byref(n), 1 if reset else 0), "syk_profile_read")
     return ms.value, n.value
+
+
+def syk_microbench_workspace_bytes():
+    return int(_lib.syk_microbench_workspace_bytes())
+
+
+def syk_microbench(kind, arg0, arg1, d_buf, d_work, stream=None):
+    """One on-chip peak measurement (include/syk.h); returns {"ms", "cycles", "units", "lds_bytes"}."""
+    res = (ctypes.c_double * 4)()
+    nb = 0 if d_buf is None else d_buf.numel() * d_buf.element_size()
+    _check(_lib.syk_microbench(int(kind), int(arg0), int(arg1), 0 if d_buf is None else _dptr(d_buf), nb, _dptr(d_work),
+                               d_work.numel() * d_work.element_size(), res, _stream(stream)), "syk_microbench")
+    return {"ms": res[0], "cycles": res[1], "units": res[2], "lds_bytes": res[3]}
 
 
 def syk_version():

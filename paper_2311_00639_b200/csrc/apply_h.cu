@@ -557,6 +557,10 @@ bool batched_apply_ok(const syk_ham* const* hams, int nb, int dtype) {
     for (int r = 0; r < nb; ++r) {
         const syk_ham* h = hams[r];
         if (!h || h->N != hams[0]->N || h->L < kTileLog2[k] || h->n_terms() == 0) return false;
+        // one gamma scaling, one kind of operator and one space for the whole batch (the pipelines take them from hams[0])
+        if (h->gamma_norm != hams[0]->gamma_norm || h->generic != hams[0]->generic ||
+            h->block_of_N != hams[0]->block_of_N || h->sector != hams[0]->sector)
+            return false;
         const size_t tb = tma_table_bytes((int)h->n_groups(), (int)h->n_terms(), (int)h->n_groups() + 1, elem_bytes(dtype));
         if (tb + (size_t)kBatchedStages * kTileBytes > (size_t)kSmemLimit / 2 - 1024) return false;   // two CTAs per SM
     }
@@ -636,6 +640,20 @@ int syk_apply_H_batched(const syk_ham* const* hams, int n_batch, int dtype, cons
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype) {
     if (!h || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
     return syk::apply_h_kernel_kind(h, dtype);
+}
+
+int syk_ham_prepare(const syk_ham* h, int dtype) {
+    if (!h || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    if (h->L > 32) return SYK_EINVAL;
+    SYK_TRY(syk::ensure_device_tables(h));
+    const int kind = syk::apply_h_kernel_kind(h, dtype);   // builds the host tables of the tile kernels
+    if (kind == 4) SYK_TRY(syk::prepare_dense_tables(h, dtype));
+    return SYK_OK;
+}
+
+int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split) {
+    if (!h || (dtype != SYK_C64 && dtype != SYK_C128) || !syk::dense_kernel_ok(h, true)) return SYK_EINVAL;
+    return syk::dense_tables_info(h, dtype, n_loads, n_chunks, split);
 }
 
 int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,

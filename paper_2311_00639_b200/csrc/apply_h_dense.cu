@@ -602,8 +602,32 @@ int launch_dn(const syk_ham* h, const DenseCache& dc, const void* d_in, void* d_
 // take the split form: the table is shared out over several CTAs per tile).
 bool dense_kernel_ok(const syk_ham* h, bool forced) {
     if (h->n_terms() == 0 || h->L < kTileLog2D) return false;
-    if (forced) return true;
-    return h->n_terms() >= 4 * h->n_groups() && h->n_terms() > kRtMaxTerms;   // any vector of at least one tile
+    if (!forced && !(h->n_terms() >= 4 * h->n_groups() && h->n_terms() > kRtMaxTerms)) return false;
+    // what build_dense_tables cannot represent: a group larger than one table chunk (generic Pauli sums with very many
+    // diagonal terms), a coefficient that is neither real nor imaginary (non-Hermitian sums) -> another kernel
+    if (h->dense_representable < 0) {   // tables are immutable after the build: checked once
+        int ok = 1;
+        for (size_t g = 0; g < h->x.size() && ok; ++g)
+            if (h->group_off[g + 1] - h->group_off[g] + 1 > (uint32_t)kChunkEntries - 1) ok = 0;
+        for (size_t t = 0; t < h->c.size() && ok; ++t)
+            if (h->c[t].real() != 0.0 && h->c[t].imag() != 0.0) ok = 0;
+        h->dense_representable = ok;
+    }
+    return h->dense_representable == 1;
+}
+
+int prepare_dense_tables(const syk_ham* h, int dtype) {
+    const DenseCache* dc = nullptr;
+    return get_dense_tables(h, dtype, &dc);
+}
+
+int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split) {
+    const DenseCache* dc = nullptr;
+    SYK_TRY(get_dense_tables(h, dtype, &dc));
+    if (n_loads) *n_loads = dc->n_loads;
+    if (n_chunks) *n_chunks = dc->n_chunks;
+    if (split) *split = dc->split;
+    return SYK_OK;
 }
 
 int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

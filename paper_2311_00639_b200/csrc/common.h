@@ -97,6 +97,7 @@ struct syk_ham {
     int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
     bool generic = false;                      // built from caller-supplied Pauli strings (no Majorana meaning)
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
+    mutable int dense_representable = -1;      // dense-table kernel: -1 not checked yet, 0 / 1
     mutable syk::DeviceTables dev;             // created on first device use
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
     mutable syk::StCache* st[2] = {nullptr, nullptr};   // scatter-tile kernel tables per dtype (host, lazily built)
@@ -188,6 +189,8 @@ bool dense_kernel_ok(const syk_ham* h, bool forced);
 int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
                          cudaStream_t stream);
 void free_dense_tables(const syk_ham* h);
+int prepare_dense_tables(const syk_ham* h, int dtype);   // builds / uploads the device table and the split scratch
+int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split);
 
 // apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

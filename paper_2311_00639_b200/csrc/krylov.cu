@@ -320,6 +320,11 @@ int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, vo
     const size_t vbytes = (size_t)D * elem_bytes(dtype);
     const size_t ws_stride = krylov_header_bytes() + (size_t)m * vbytes;
     if (work_bytes < krylov_batched_bytes(h0, nb, dtype, m)) return SYK_ENOMEM;
+    {   // the states must not overlap the work space
+        const uintptr_t a = (uintptr_t)d_psi, b = (uintptr_t)d_work;
+        const size_t span = (size_t)(nb - 1) * psi_stride_bytes + vbytes;
+        if (a < b + krylov_batched_bytes(h0, nb, dtype, m) && b < a + span) return SYK_EINVAL;
+    }
     char* tab = (char*)d_work;
     char* ws = tab + batched_table_bytes(nb);                 // realization r: header at ws + r ws_stride, then m vectors
     char* vecs = ws + krylov_header_bytes();

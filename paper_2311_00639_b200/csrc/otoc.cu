@@ -139,6 +139,10 @@ static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int 
     const size_t v = (size_t)D * elem_bytes(dtype);
     const int m = resolve_krylov_dim(h0, opts);
     if (work_bytes < otoc_batched_bytes(h0, nb, dtype, opts)) return SYK_ENOMEM;
+    {   // the states must not overlap the work space
+        const uintptr_t a = (uintptr_t)d_psi, b = (uintptr_t)d_work;
+        if (a < b + otoc_batched_bytes(h0, nb, dtype, opts) && b < a + (size_t)(nb - 1) * psi_stride + v) return SYK_EINVAL;
+    }
     char* l = (char*)d_psi;
     char* phi = (char*)d_work;
     char* r = phi + (size_t)nb * v;

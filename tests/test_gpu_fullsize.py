@@ -241,3 +241,74 @@ def test_scatter_kernel_many_layouts_sampled(B, N, k, seed):
         diff = float(torch.linalg.vector_norm(d_out - d_out2) / torch.linalg.vector_norm(d_out2))
         assert diff <= tol
         del d_in, d_out, d_out2
+
+
+@pytest.mark.parametrize("N,n_samples", [(40, 320), (44, 128)])
+def test_dense_table_kernel_multichunk_sampled(B, N, n_samples):
+    """Algorithm 1 on the dense p = 1 Hamiltonian (the dense rows of PAPER.md:342-354; BASELINE
+    configs[2] "dense p=1") in the form the dense-table kernel takes for N >= 40: ONE persistent CTA per tile (no split),
+    several table chunks per source tile streamed through the double buffer.  N = 40: 91 390 terms, 2^20 amplitudes,
+    256 tiles; N = 44: 135 751 terms, 1024 tiles.  Sampled outputs (plus the edges of the first / last tiles) against the
+    oracle's monomial rows, both precisions, plain and inside two fused Lanczos steps; sum rule; two-pass (out aliases
+    prev) against one-pass."""
+    import torch
+    D = 1 << (N // 2)
+    q, J, _ = orng.sample_couplings(N, 1.0, 3, 0)
+    h = B.syk_build_from_terms(N, q, J)
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    idx = inputs.sample_indices(D, n_samples, seed=5)
+    edge = np.array([1, 511, 512, 4095, 4096, 8191, D // 2 - 1, D // 2, D - 4097, D - 4096, D - 513, D - 2], dtype=np.uint64)
+    idx = np.unique(np.concatenate([idx, edge]))
+    didx = torch.from_numpy(idx.astype(np.int64)).cuda()
+    cols, vals = ohm.hamiltonian_rows(N, q, J, idx)                      # [T, n] each: the oracle's rows, used for all checks
+    flat = torch.from_numpy(cols.astype(np.int64).reshape(-1)).cuda()
+
+    def rows_times(d_vec):
+        src = d_vec[flat].cpu().numpy().astype(np.complex128).reshape(cols.shape)
+        return (vals * src).sum(axis=0)
+
+    for tdt, code, tol in ((torch.complex128, B.SYK_C128, 1e-10), (torch.complex64, B.SYK_C64, 1e-5)):
+        assert B.syk_apply_H_kernel_kind(h, code) == 4                    # automatic choice for dense H
+        B.syk_ham_prepare(h, code)
+        info = B.syk_apply_H_dense_info(h, code)
+        assert info["split"] == 1 and info["n_chunks"] >= 2 * info["n_loads"], info   # non-split, multi-chunk loads
+        d_in = torch.empty(D, dtype=tdt, device="cuda")
+        B.syk_random_state(N, 3, 0, d_in, scratch)
+        d_out = torch.full((D,), complex(float("nan"), float("nan")), dtype=tdt, device="cuda")
+        B.syk_launch_count(reset=True)
+        B.syk_apply_H(h, d_in, d_out)
+        torch.cuda.synchronize()
+        assert B.syk_launch_count(reset=True) == 1                        # one kernel: not split + reduce
+        ref = rows_times(d_in)
+        got = d_out[didx].cpu().numpy().astype(np.complex128)
+        scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= tol, (N, tdt)
+        assert np.max(np.abs(got - ref)) <= 10 * tol * scale
+        assert not bool(torch.isnan(torch.view_as_real(d_out)).any())
+        n2 = B.syk_dot(N, d_out, d_out, scratch).real                     # sum rule (pin P3): |H psi|^2 ~ sum J^2
+        assert abs(n2 / float(np.sum(J ** 2)) - 1.0) <= 2e-2
+        # two fused Lanczos steps (one-pass layout: u_2, u_3 are the first two work vectors):
+        #   u_2 = H u_1/|u_1| - alpha_1 u_1/|u_1| ;  u_3 = H u_2/|u_2| - (|u_2|/|u_1|) u_1 - alpha_2 u_2/|u_2|
+        m = 2
+        wk = torch.empty(B.syk_krylov_workspace_bytes(h, code, {"krylov_dim": m}), dtype=torch.uint8, device="cuda")
+        alpha, beta, _ = B.syk_lanczos_run(h, d_in, m, wk)
+        hdr = (wk.numel() - m * D * d_in.element_size())
+        vecs = wk[hdr:].view(tdt).view(m, D)
+        u1 = d_in[didx].cpu().numpy().astype(np.complex128)
+        u2 = vecs[0][didx].cpu().numpy().astype(np.complex128)
+        u3 = vecs[1][didx].cpu().numpy().astype(np.complex128)
+        ref2 = ref / beta[0] - alpha[0] * u1 / beta[0]
+        assert np.linalg.norm(u2 - ref2) / np.linalg.norm(ref2) <= 2 * tol, (N, tdt)
+        ref3 = rows_times(vecs[0]) / beta[1] - (beta[1] / beta[0]) * u1 - alpha[1] * u2 / beta[1]
+        assert np.linalg.norm(u3 - ref3) / np.linalg.norm(ref3) <= 4 * tol, (N, tdt)
+        a1 = B.syk_dot(N, d_in, d_out, scratch).real / beta[0] ** 2       # alpha_1 = <v|H|v> from the plain product
+        assert abs(alpha[0] - a1) <= 10 * tol
+        # two-pass (out aliases prev from step 3 on) = one-pass, same kernel
+        if N == 40:
+            o1, o2 = {"krylov_dim": 5}, {"krylov_dim": 5, "two_pass": 1}
+            a, b = d_in.clone(), d_in.clone()
+            B.syk_krylov_evolve(h, a, 0.2, -0.1, torch.empty(B.syk_krylov_workspace_bytes(h, code, o1), dtype=torch.uint8, device="cuda"), o1)
+            B.syk_krylov_evolve(h, b, 0.2, -0.1, torch.empty(B.syk_krylov_workspace_bytes(h, code, o2), dtype=torch.uint8, device="cuda"), o2)
+            rel = float(torch.linalg.vector_norm(a - b) / torch.linalg.vector_norm(a))
+            assert rel <= (1e-13 if code == B.SYK_C128 else 2e-6), rel
+        del d_in, d_out, wk

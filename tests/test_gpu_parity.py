@@ -379,6 +379,37 @@ def test_krylov_evolve_vs_exact(B, torch, propagators, N, k, tau, opts, dt):
     assert st["err_est"] <= TOL[dt] and st["n_substeps"] >= 1 and st["n_matvec"] >= 2
 
 
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_two_pass_every_tile_kernel_vs_chebyshev(B, torch, dt):
+    """Two-pass Lanczos (bounded vector count) makes `out` alias `prev` in the fused epilogue from step 3
+    on.  The register-tile, scatter-tile and dense-table kernels -- the ones that run the N = 64 two-pass workload --
+    are forced at N = 28 (2..4 tiles, several ring chunks per tile) and compared with the oracle's Chebyshev propagator
+    (O8: shares nothing with Lanczos), for real and complex tau, and with the one-pass result of the same kernel."""
+    N = 28
+    q, J = couplings(N, 4, seed=9)
+    D = 1 << (N // 2)
+    psi = inputs.gaussian_state(D, 41, npdtype(dt))
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    h = B.syk_build_from_terms(N, q, J)
+    o2 = {"krylov_dim": 6, "two_pass": 1}
+    o1 = {"krylov_dim": 6}
+    w2 = work(torch, B.syk_krylov_workspace_bytes(h, code, o2))
+    w1 = work(torch, B.syk_krylov_workspace_bytes(h, code, o1))
+    for tau in ((1.2, 0.0), (-0.7, -1.25)):
+        ref = oev.chebyshev_propagate(N, q, J, complex(*tau), psi.astype(np.complex128))
+        for kind in (1, 2, 3, 4):
+            B.syk_set_apply_H_kernel(h, kind)
+            assert B.syk_apply_H_kernel_kind(h, code) == kind
+            d2 = to_dev(torch, psi)
+            st2 = B.syk_krylov_evolve(h, d2, tau[0], tau[1], w2, o2)
+            assert relerr(d2.cpu().numpy(), ref) <= TOL[dt], (kind, tau, st2)
+            assert st2["n_substeps"] >= 2                              # several rounds: u_1 is rebuilt from psi each time
+            d1 = to_dev(torch, psi)
+            st1 = B.syk_krylov_evolve(h, d1, tau[0], tau[1], w1, o1)
+            assert st1["n_substeps"] == st2["n_substeps"]              # the recurrence is repeated bit-identically
+            assert relerr(d2.cpu().numpy(), d1.cpu().numpy()) <= (1e-13 if dt == "c128" else 2e-6), (kind, tau)
+
+
 def test_krylov_dim2_two_pass(B, torch, propagators):
     """The paper's N >= 62 setting, Krylov dimension 2: a first-order scheme, so the sub-step
     count grows like 1/tol; checked at tol = 1e-6 against the exact exponential."""
@@ -502,7 +533,7 @@ def test_otoc_config0_vs_oracle(B, torch):
     B.syk_random_state(N, cfg["seed"], 0, d_psi, scratch)
     F, st = B.syk_otoc(h, cfg["i_W"], cfg["j_V"], cfg["beta"], t_grid, d_psi, wk, o)
     assert np.max(np.abs(F - ref)) / abs(ref[0]) <= 1e-10
-    assert abs(F[0].imag) <= 1e-12 * abs(F[0]) + 1e-15 or True
+    # (the same-psi F(0) is complex: conjugation exchanges W and V; only the exact trace is real -- pin P11)
     # two-pass and complex64 variants
     o2 = {"krylov_dim": cfg["krylov_dim"], "two_pass": 1}
     B.syk_random_state(N, cfg["seed"], 0, d_psi, scratch)
@@ -625,7 +656,7 @@ def test_parity_block_apply_H_and_gamma(B, torch, dt):
                 gref = opar.restrict(ohm.apply_gamma(N, n, full), L, 1 - sector)
                 d_g = torch.empty_like(d_out)
                 B.syk_apply_gamma_block(N, n, 1 - sector, to_dev(torch, vs), d_g)
-                assert relerr(d_g.cpu().numpy(), gref) <= 1e-15 if dt == "c128" else 1e-7, (N, n, sector)
+                assert relerr(d_g.cpu().numpy(), gref) <= (1e-15 if dt == "c128" else 1e-7), (N, n, sector)
                 d_ip = to_dev(torch, vs)
                 B.syk_apply_gamma_block(N, n, 1 - sector, d_ip, d_ip)           # in place
                 assert torch.equal(torch.view_as_real(d_ip), torch.view_as_real(d_g))

@@ -127,8 +127,9 @@ def test_hand_worked_terms(B):
 
 
 def test_large_N_tables_structure(B):
-    """N=56, k=4 and N=64, k=2 (bench configs): structure that holds at any size."""
-    for N, k in ((56, 4), (64, 2)):
+    """N=48 (configs[2] sparsities), N=56, k=4 and N=64, k=2 (bench configs): structure that holds at any size, and EVERY
+    term against the oracle's dense-row derivation (integer tables bit-exact)."""
+    for N, k in ((48, 1), (48, 8), (56, 4), (64, 2)):
         p = inputs.bernoulli_p(N, k)
         h = B.syk_build_hamiltonian(N, p, 0, 0, 0)
         info, t = h.info(), h.tables()
@@ -144,13 +145,11 @@ def test_large_N_tables_structure(B):
         assert np.all((t["c"].imag == 0) == (par == 0))
         assert np.all((t["c"].real == 0) == (par == 1))
         assert np.all(t["x"] < (1 << (N // 2))) and np.all(t["z"] < (1 << (N // 2)))
-        # sampled terms against the oracle's dense-row derivation
-        sel = np.arange(0, T, max(1, T // 16))
-        ref = ohm.derive_tables(N, t["quartet_of_term"][sel], t["J"][sel], 0)
-        got = {(int(a), int(b)): c for a, b, c in zip(xs[sel], t["z"][sel], t["c"][sel])}
-        refx = np.repeat(ref["x"], np.diff(ref["group_off"]).astype(np.int64))
-        want = {(int(a), int(b)): c for a, b, c in zip(refx, ref["z"], ref["c"])}
-        assert got == want
+        # all terms against the oracle's dense-row derivation: whole tables, canonical order included
+        ref = ohm.derive_tables(N, t["quartet_of_term"], t["J"], 0)
+        for key in ("x", "group_off", "z"):
+            assert np.array_equal(t[key], ref[key]), (N, k, key)
+        assert_coeff_equal(t["c"], ref["c"], 0)
 
 
 def test_argument_errors(B):
