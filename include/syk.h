@@ -89,6 +89,41 @@ int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, 
 int syk_ham_tables(const syk_ham* h, uint64_t* x, uint32_t* group_off, uint64_t* z, double* c_re_im,
                    int32_t* quartet_of_term, double* J_of_term);
 
+/* ------------------------------------------------------------------------------------------------------------
+ * Qubit layout of a handle (the fewer and the more local the terms, the cheaper
+ * Algorithm 1).  Which qubit sits on which bit of the basis index is physically free -- a relabelling of the Jordan-
+ * Wigner qubits is a permutation of the basis -- but it decides how often the tile kernels of apply_H move the vector:
+ * once from L2 into the SMs per distinct X-mask outside the low "tile" bits, once from DRAM per distinct X-mask outside
+ * tile + "window" bits.  A handle therefore carries a layout perm[q] = index bit of qubit q (identity after a build).
+ *   syk_ham_optimize_layout : chooses perm for the tile geometry of `dtype` (deterministic hill climbing on
+ *                             loads + 2 passes over the partition of the qubits into tile / window / rest) and sets it;
+ *                             Hamiltonians with more than 1024 terms keep the identity.
+ *   syk_ham_set_layout      : sets a caller-chosen permutation (NULL = identity).  SYK_EINVAL if perm is not one.
+ *   syk_ham_layout          : exports perm[N/2] and whether it is the identity.
+ * Setting a layout rewrites the handle's kernel tables (every string c Z^z X^x becomes c Z^{Pz} X^{Px}) and drops its
+ * device copies: do it before syk_ham_prepare and before any vector exists.  The CANONICAL tables exported by
+ * syk_ham_tables never change.  From then on every DEVICE vector passed with this handle (syk_apply_H, syk_lanczos_run,
+ * syk_krylov_evolve, syk_otoc, syk_green, ...) is stored in the handle's layout: amplitude of basis state b at index
+ * sum_q bit_q(b) 2^perm[q].  The calls below produce / convert such vectors; the *_host entry points take canonical host
+ * vectors and convert on the device; results that do not depend on the basis (F(t), G(t), Lanczos coefficients, dots)
+ * are the same in every layout up to rounding order.  The two parity blocks of a Hamiltonian must share one layout.
+ */
+int syk_ham_optimize_layout(syk_ham* h, int dtype);
+int syk_ham_set_layout(syk_ham* h, const int32_t* perm /* [N/2] or NULL */);
+int syk_ham_layout(const syk_ham* h, int32_t* perm /* [N/2], may be NULL */, int* is_identity /* may be NULL */);
+/* d_out = the vector d_in converted from the canonical basis to the handle's layout (to_layout != 0) or back; d_in and
+ * d_out must not overlap. */
+int syk_permute_vector(const syk_ham* h, int dtype, int to_layout, const void* d_in, void* d_out, void* stream);
+/* syk_random_state / syk_apply_gamma / syk_apply_gamma_block for vectors in the layout of a handle: the same physical
+ * state / operator (the Haar-random amplitude of canonical basis state b lands on its stored index; the Jordan-Wigner
+ * string of gamma_n has its masks mapped through perm).  syk_random_state_h and syk_permute_vector accept any handle,
+ * syk_apply_gamma_h a full-space Majorana handle, syk_apply_gamma_block_h a parity block (N, gamma_norm taken from it). */
+int syk_random_state_h(const syk_ham* h, uint64_t seed, uint32_t realization, int dtype, void* d_psi, void* d_scratch,
+                       void* stream);
+int syk_apply_gamma_h(const syk_ham* h, int n, int dtype, const void* d_in, void* d_out, void* stream);
+int syk_apply_gamma_block_h(const syk_ham* h_block, int n, int sector_out, int dtype, const void* d_in, void* d_out,
+                            void* stream);
+
 /* Creates the device copy of the term tables of `h` on the current device for `dtype` (and, for the dense-table
  * kernel, its entry stream and split scratch): after this call syk_apply_H / syk_lanczos_run / syk_krylov_evolve /
  * syk_otoc / syk_green on this handle and dtype allocate nothing (few allocation calls).  Synchronous
@@ -255,7 +290,7 @@ int syk_set_apply_H_kernel(syk_ham* h, int kind);
  * persistent one-CTA-per-tile form; > 1 = the split form for vectors with fewer tiles than SMs).  Builds the table if
  * needed.  Any output pointer may be NULL.  SYK_EINVAL if the handle cannot use kind 4. */
 int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split);
-/* Tile layout the scatter-tile kernel (kind 3) chose for this Hamiltonian: n_loads = source tiles fetched per
+/* Tile layout the scatter-tile kernel (kind 3) uses for this Hamiltonian in its current qubit layout: n_loads = source tiles fetched per
  * output tile (L2 -> SM transfers of the whole vector per product), n_passes = distinct X-masks outside tile and
  * L2-window bits (DRAM reads of the whole vector per product, if L2 reuse were perfect), tile_mask / window_mask =
  * the index bits of a tile / of tile + window.  Any output pointer may be NULL.  SYK_EINVAL if kind 3 cannot be used. */

@@ -59,6 +59,13 @@ _SIGNATURES = {
     "syk_ham_info": (_i, [_vp, _P(_i), _P(_i64), _P(_i64), _P(_i64)]),
     "syk_ham_tables": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "syk_ham_prepare": (_i, [_vp, _i]),
+    "syk_ham_optimize_layout": (_i, [_vp, _i]),
+    "syk_ham_set_layout": (_i, [_vp, _vp]),
+    "syk_ham_layout": (_i, [_vp, _vp, _P(_i)]),
+    "syk_permute_vector": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
+    "syk_random_state_h": (_i, [_vp, _u64, _u32, _i, _vp, _vp, _vp]),
+    "syk_apply_gamma_h": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
+    "syk_apply_gamma_block_h": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp]),
     "syk_apply_H_dense_info": (_i, [_vp, _i, _P(_i), _P(_i), _P(_i)]),
     "syk_apply_H": (_i, [_vp, _i, _vp, _vp, _vp]),
     "syk_apply_H_batched": (_i, [_P(_vp), _i, _i, _vp, _vp, _i64, _vp]),
@@ -228,6 +235,54 @@ def syk_ham_tables(h):
     _check(_lib.syk_ham_tables(_h(h), x.ctypes.data, off.ctypes.data, z.ctypes.data, c.ctypes.data,
                                quart.ctypes.data, J.ctypes.data), "syk_ham_tables")
     return {"x": x, "group_off": off, "z": z, "c": c[:, 0] + 1j * c[:, 1], "quartet_of_term": quart, "J": J}
+
+
+def syk_ham_optimize_layout(h, dtype):
+    _check(_lib.syk_ham_optimize_layout(_h(h), int(dtype)), "syk_ham_optimize_layout")
+    return syk_ham_layout(h)
+
+
+def syk_ham_set_layout(h, perm):
+    """perm[q] = index bit of qubit q (None = identity)."""
+    if perm is None:
+        _check(_lib.syk_ham_set_layout(_h(h), None), "syk_ham_set_layout")
+        return
+    p = np.ascontiguousarray(perm, dtype=np.int32)
+    if len(p) != syk_ham_info(h)["N"] // 2:
+        raise SykError(SYK_EINVAL, "syk_ham_set_layout: perm must have N/2 entries")
+    _check(_lib.syk_ham_set_layout(_h(h), p.ctypes.data), "syk_ham_set_layout")
+
+
+def syk_ham_layout(h):
+    L = syk_ham_info(h)["N"] // 2
+    p = np.zeros(L, dtype=np.int32)
+    ident = _i()
+    _check(_lib.syk_ham_layout(_h(h), p.ctypes.data, ctypes.byref(ident)), "syk_ham_layout")
+    return {"perm": p, "identity": bool(ident.value)}
+
+
+def syk_permute_vector(h, to_layout, d_in, d_out, stream=None):
+    _check(_lib.syk_permute_vector(_h(h), dtype_code(d_in), 1 if to_layout else 0, _dptr(d_in), _dptr(d_out),
+                                   _stream(stream)), "syk_permute_vector")
+    return d_out
+
+
+def syk_random_state_h(h, seed, realization, d_psi, d_scratch, stream=None):
+    _check(_lib.syk_random_state_h(_h(h), int(seed), int(realization), dtype_code(d_psi), _dptr(d_psi), _dptr(d_scratch),
+                                   _stream(stream)), "syk_random_state_h")
+    return d_psi
+
+
+def syk_apply_gamma_h(h, n, d_in, d_out, stream=None):
+    _check(_lib.syk_apply_gamma_h(_h(h), int(n), dtype_code(d_in), _dptr(d_in), _dptr(d_out), _stream(stream)),
+           "syk_apply_gamma_h")
+    return d_out
+
+
+def syk_apply_gamma_block_h(h_block, n, sector_out, d_in, d_out, stream=None):
+    _check(_lib.syk_apply_gamma_block_h(_h(h_block), int(n), int(sector_out), dtype_code(d_in), _dptr(d_in), _dptr(d_out),
+                                        _stream(stream)), "syk_apply_gamma_block_h")
+    return d_out
 
 
 def syk_ham_prepare(h, dtype):

@@ -559,7 +559,7 @@ bool batched_apply_ok(const syk_ham* const* hams, int nb, int dtype) {
         if (!h || h->N != hams[0]->N || h->L < kTileLog2[k] || h->n_terms() == 0) return false;
         // one gamma scaling, one kind of operator and one space for the whole batch (the pipelines take them from hams[0])
         if (h->gamma_norm != hams[0]->gamma_norm || h->generic != hams[0]->generic ||
-            h->block_of_N != hams[0]->block_of_N || h->sector != hams[0]->sector)
+            h->block_of_N != hams[0]->block_of_N || h->sector != hams[0]->sector || h->perm != hams[0]->perm)
             return false;
         const size_t tb = tma_table_bytes((int)h->n_groups(), (int)h->n_terms(), (int)h->n_groups() + 1, elem_bytes(dtype));
         if (tb + (size_t)kBatchedStages * kTileBytes > (size_t)kSmemLimit / 2 - 1024) return false;   // two CTAs per SM

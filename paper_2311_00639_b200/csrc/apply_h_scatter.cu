@@ -7,7 +7,8 @@
 // distinct value of (x restricted to the bits above the L2 window), once from L2 into an SM per distinct value of
 // (x restricted to the bits outside a tile).  Both counts depend on WHICH qubits are the tile / window bits, and
 // the X-masks of a sparse SYK Hamiltonian are random 2- and 4-subsets of the qubits, so the host picks the bits
-// (choose_layout: hill climbing on  #loads + 2 #passes):
+// (choose_layout: hill climbing on  #loads + 2 #passes; on top of it syk_ham_optimize_layout relabels the qubits so that
+// all 13 / 14 tile bits and the 7 window bits are chosen, term_compiler.cpp):
 //   * slice bits   : index bits 0..TB-1: a slice = 256 consecutive 16-byte ELEMENTS, one per consumer thread; an
 //                    element is one complex128 amplitude (TB = 8) or a pair of adjacent complex64 amplitudes
 //                    (TB = 9: both precisions move 16 bytes per LDS and per store);
@@ -26,17 +27,23 @@
 // output chunk oc = c ^ (xr >> LRC): the consumers take the chunks of a load in arrival order and branch
 // (uniformly) to the code that owns the accumulator registers of chunk oc.
 //
-// Per (amplitude, term): one LDS, two FMAs (the coefficient is exactly real or exactly imaginary: c = J s^4 times
-// 1, -1, i, -i); the sign is popcount((base | element) & z) once per (term, chunk) and thread plus a Gray-code walk
-// over the slices of a chunk (one XOR each).  Per-term data comes from the __grid_constant__ table (constant
-// bank).  No atomics on data, one write per output: bitwise reproducible.
+// Per (amplitude, term): one LDS.128 at [thread register + warp-uniform offset] and two FMAs (the coefficient is exactly
+// real or exactly imaginary: c = J s^4 times 1, -1, i, -i).  The sign is popcount((base | element) & z) once per
+// (term, chunk) and thread; over the 16 slices of a chunk it is a Walsh function of the slice number, walked in groups of
+// four: one XOR per group, and inside a group the signs are compile-time FMA operand negations of a kernel variant chosen
+// by a uniform branch on the two low slice bits of z (accumulate_chunk).  Per-term data comes from the __grid_constant__
+// table (constant bank), the next entry fetched one term ahead.  No atomics on data, one write per output: bitwise
+// reproducible.  ~100 warp instructions per (term, chunk of 16 slices) instead of ~150 with a per-slice sign walk; what
+// the launch is bound by is the supply of tiles (DRAM phases and L2 phases of the lock-stepped CTAs do not overlap; L2
+// prefetching by the TMA unit or by prefetch.global.L2, of every load or only of the loads that must miss, 1..12 loads
+// ahead, made every configuration slower: profiles/r2_apply_h_experiments.md).
 //
 // Fused Lanczos epilogue (a-3 part 1) as in apply_h.cu: out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, per-CTA fp64
 // partial sums of Re<in|out>.  The tile of `in` and of `prev` are staged through the same ring after the last
 // source tile (their DRAM latency would otherwise be exposed once per tile: measured 50 ms of 385 ms at N = 64).
 //
-// Measured (profiles/r1e_*.md): both headline workloads sit at the L2 -> SM throughput ceiling (~6000-6600 B/clk
-// chip-wide): #loads x V / time = 12.1 TB/s (N = 56 complex128) and 10.1 TB/s (N = 64 complex64).
+// Measured peaks of this box (syk_microbench, profiles/r2_measured_onchip_peaks.md): L2 -> SM 88 B/clk/SM (25 TB/s),
+// DRAM -> SM 7.2-7.5 TB/s, LDS 125 B/clk/SM; the headline launches run at 12-13 TB/s of L2 -> SM traffic.
 #include <algorithm>
 #include <atomic>
 #include <cstring>
@@ -61,6 +68,7 @@ constexpr int kRun = 8;                            // consecutive slices per bul
 constexpr int kMaxRing = 16;
 constexpr int kSmemLimit = 232448;                 // 227 KiB opt-in maximum per CTA on sm_100
 constexpr int kMiscBytes = 2 * kMaxRing * 8 + 40 * 8 + 128;
+constexpr uint32_t kRingAlign = 4096;              // alignment of the ring inside the shared window
 constexpr int kWindowBits = 7;                     // ~log2(148 tiles in flight)
 constexpr int kFixedR = 3;                         // r bits 0..2 sit at index bits 8..10: a chunk is one contiguous run
 
@@ -101,59 +109,103 @@ template <> struct El<double> { static constexpr int PAIR = 1, TB = 8; };
 template <> struct El<float> { static constexpr int PAIR = 2, TB = 9; };
 constexpr uint32_t kSliceBytes = kConsumerThreads * 16;
 
-// One term applied to the RC slices of output chunk OC.  `pb` = the thread's element inside the staged source chunk;
-// `w` = sign-carrying word of the coefficient times the sign of (thread, tile, chunk); the slices of the chunk are
-// walked in Gray-code order so that consecutive signs differ by one uniform XOR.  complex64: `aux` = (z & 1) << 31, the
-// relative sign of the second amplitude of the pair; SWAP = the mask flips index bit 0 (the pair arrives swapped).
-template <typename T, int R, int RC, int OC, bool IMAG, bool SWAP>
-__device__ __forceinline__ void accumulate_chunk(const unsigned char* __restrict__ pb, uint32_t xr_lo, uint32_t zr_lo,
-                                                 uint32_t aux, uint32_t w, T (&ar)[R * El<T>::PAIR],
-                                                 T (&ai)[R * El<T>::PAIR]) {
+__device__ __forceinline__ double2 lds_el(uint32_t addr, double) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float4 lds_el(uint32_t addr, float) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+// One term applied to the RC slices of output chunk OC.  `pb` = shared-memory address of the thread's element in slice 0
+// of the staged source chunk; `w` = sign-carrying word of the coefficient times the sign of (thread, tile, chunk, term).
+// The slices are taken in groups of four, rl = 4 g + j: the sign of slice rl relative to `w` is
+// (-1)^(popcount(g & zg) + popcount(j & ZJ)) with zg / ZJ the upper / lower two bits of the term's Z-mask on the slice
+// bits of a chunk.  ZJ is a template parameter -- the caller branches on it (uniformly) -- so inside a group the four
+// signs are compile-time negations of one coefficient register pair (FMA operand modifiers: no instruction), and only the
+// group sign costs an XOR.  Source addresses are pb + a warp-uniform offset ((rl ^ xr_lo) slices).  complex64: `aux` =
+// (z & 1) << 31, the relative sign of the second amplitude of the pair; SWAP = the mask flips index bit 0 (the pair arrives
+// swapped).  Per slice: one LDS.128 and two FP64 (four FP32) FMAs.
+template <typename T, int R, int RC, int OC, bool IMAG, bool SWAP, int ZJ>
+__device__ __forceinline__ void accumulate_chunk(uint32_t pb, uint32_t xr_lo, uint32_t zg, uint32_t aux, uint32_t w,
+                                                 T (&ar)[R * El<T>::PAIR], T (&ai)[R * El<T>::PAIR]) {
+    static_assert(RC % 4 == 0, "slices of a chunk are walked in groups of four");
+    constexpr int r0 = OC * RC;
 #pragma unroll
-    for (int i = 0; i < RC; ++i) {
-        const int rl = i ^ (i >> 1);
-        if (i > 0) w ^= (zr_lo * (0x80000000u / (uint32_t)(i & -i))) & 0x80000000u;   // z bit ctz(i) -> bit 31; a shift after unrolling
-        const unsigned char* src = pb + (((uint32_t)rl ^ xr_lo) * kSliceBytes);
-        constexpr int r0 = OC * RC;
+    for (int g = 0; g < RC / 4; ++g) {
+        // sign of the group: parity of (g & zg); g is a compile-time constant of the unrolled loop
+        uint32_t wg = w;
+        if (g & 1) wg ^= zg << 31;                  // bit 0 of zg -> bit 31
+        if (g & 2) wg ^= (zg << 30) & 0x80000000u;  // bit 1 of zg -> bit 31
         if constexpr (sizeof(T) == 8) {
-            const double a = __hiloint2double((int)w, (int)aux);   // aux = low word of the coefficient
-            const double2 v = *reinterpret_cast<const double2*>(src);
-            if constexpr (IMAG) {   // (i a)(vx + i vy) = -a vy + i a vx
-                ar[r0 + rl] = st_fma(-a, v.y, ar[r0 + rl]);
-                ai[r0 + rl] = st_fma(a, v.x, ai[r0 + rl]);
-            } else {
-                ar[r0 + rl] = st_fma(a, v.x, ar[r0 + rl]);
-                ai[r0 + rl] = st_fma(a, v.y, ai[r0 + rl]);
+            const double a = __hiloint2double((int)wg, (int)aux);   // aux = low word of the coefficient
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                constexpr int dummy = 0;
+                (void)dummy;
+                const int rl = 4 * g + j;
+                const bool neg = (__builtin_popcount(j & ZJ) & 1) != 0;
+                const double2 v = lds_el(pb + (((uint32_t)rl ^ xr_lo) * kSliceBytes), double());
+                const double aj = neg ? -a : a;
+                if constexpr (IMAG) {   // (i a)(vx + i vy) = -a vy + i a vx
+                    ar[r0 + rl] = st_fma(-aj, v.y, ar[r0 + rl]);
+                    ai[r0 + rl] = st_fma(aj, v.x, ai[r0 + rl]);
+                } else {
+                    ar[r0 + rl] = st_fma(aj, v.x, ar[r0 + rl]);
+                    ai[r0 + rl] = st_fma(aj, v.y, ai[r0 + rl]);
+                }
             }
         } else {
-            const float a0 = __uint_as_float(w), a1 = __uint_as_float(w ^ aux);
-            const float4 v = *reinterpret_cast<const float4*>(src);
-            const float s0x = SWAP ? v.z : v.x, s0y = SWAP ? v.w : v.y, s1x = SWAP ? v.x : v.z, s1y = SWAP ? v.y : v.w;
-            const int k0 = 2 * (r0 + rl), k1 = k0 + 1;
-            if constexpr (IMAG) {
-                ar[k0] = st_fma(-a0, s0y, ar[k0]);
-                ai[k0] = st_fma(a0, s0x, ai[k0]);
-                ar[k1] = st_fma(-a1, s1y, ar[k1]);
-                ai[k1] = st_fma(a1, s1x, ai[k1]);
-            } else {
-                ar[k0] = st_fma(a0, s0x, ar[k0]);
-                ai[k0] = st_fma(a0, s0y, ai[k0]);
-                ar[k1] = st_fma(a1, s1x, ar[k1]);
-                ai[k1] = st_fma(a1, s1y, ai[k1]);
+            const float a0 = __uint_as_float(wg), a1 = __uint_as_float(wg ^ aux);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int rl = 4 * g + j;
+                const bool neg = (__builtin_popcount(j & ZJ) & 1) != 0;
+                const float4 v = lds_el(pb + (((uint32_t)rl ^ xr_lo) * kSliceBytes), float());
+                const float b0 = neg ? -a0 : a0, b1 = neg ? -a1 : a1;
+                const float s0x = SWAP ? v.z : v.x, s0y = SWAP ? v.w : v.y, s1x = SWAP ? v.x : v.z, s1y = SWAP ? v.y : v.w;
+                const int k0 = 2 * (r0 + rl), k1 = k0 + 1;
+                if constexpr (IMAG) {
+                    ar[k0] = st_fma(-b0, s0y, ar[k0]);
+                    ai[k0] = st_fma(b0, s0x, ai[k0]);
+                    ar[k1] = st_fma(-b1, s1y, ar[k1]);
+                    ai[k1] = st_fma(b1, s1x, ai[k1]);
+                } else {
+                    ar[k0] = st_fma(b0, s0x, ar[k0]);
+                    ai[k0] = st_fma(b0, s0y, ai[k0]);
+                    ar[k1] = st_fma(b1, s1x, ar[k1]);
+                    ai[k1] = st_fma(b1, s1y, ai[k1]);
+                }
             }
         }
     }
 }
 
-template <typename T, int R, int RC, int OC, bool IMAG, bool SWAP>
-__device__ __forceinline__ void dispatch_chunk(uint32_t oc, const unsigned char* pb, uint32_t xr_lo, uint32_t zr_lo,
+// Uniform branch to the instantiation for (variant, output chunk): variant = ZJ | IMAG << 2 | SWAP << 3.
+template <typename T, int R, int RC, int OC, int V>
+__device__ __forceinline__ void dispatch_variant(uint32_t variant, uint32_t pb, uint32_t xr_lo, uint32_t zg, uint32_t aux,
+                                                 uint32_t w, T (&ar)[R * El<T>::PAIR], T (&ai)[R * El<T>::PAIR]) {
+    constexpr int NV = sizeof(T) == 8 ? 8 : 16;
+    if constexpr (V + 1 == NV) {
+        accumulate_chunk<T, R, RC, OC, (V & 4) != 0, (V & 8) != 0, V & 3>(pb, xr_lo, zg, aux, w, ar, ai);
+    } else {
+        if (variant == (uint32_t)V) accumulate_chunk<T, R, RC, OC, (V & 4) != 0, (V & 8) != 0, V & 3>(pb, xr_lo, zg, aux, w, ar, ai);
+        else dispatch_variant<T, R, RC, OC, V + 1>(variant, pb, xr_lo, zg, aux, w, ar, ai);
+    }
+}
+
+template <typename T, int R, int RC, int OC>
+__device__ __forceinline__ void dispatch_chunk(uint32_t oc, uint32_t variant, uint32_t pb, uint32_t xr_lo, uint32_t zg,
                                                uint32_t aux, uint32_t w, T (&ar)[R * El<T>::PAIR],
                                                T (&ai)[R * El<T>::PAIR]) {
     if constexpr (OC + 1 == R / RC) {
-        accumulate_chunk<T, R, RC, OC, IMAG, SWAP>(pb, xr_lo, zr_lo, aux, w, ar, ai);
+        dispatch_variant<T, R, RC, OC, 0>(variant, pb, xr_lo, zg, aux, w, ar, ai);
     } else {
-        if (oc == (uint32_t)OC) accumulate_chunk<T, R, RC, OC, IMAG, SWAP>(pb, xr_lo, zr_lo, aux, w, ar, ai);
-        else dispatch_chunk<T, R, RC, OC + 1, IMAG, SWAP>(oc, pb, xr_lo, zr_lo, aux, w, ar, ai);
+        if (oc == (uint32_t)OC) dispatch_variant<T, R, RC, OC, 0>(variant, pb, xr_lo, zg, aux, w, ar, ai);
+        else dispatch_chunk<T, R, RC, OC + 1>(oc, variant, pb, xr_lo, zg, aux, w, ar, ai);
     }
 }
 
@@ -170,7 +222,10 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
     constexpr uint32_t CHUNK_BYTES = RC * SLICE_BYTES;
     static_assert(R % RC == 0 && RC % kRun == 0 && LRC >= kFixedR, "tile = whole chunks = whole runs");
 
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    // the ring starts on a 4 KiB boundary of the shared window: a consumer's element address inside a staged slice is then
+    // chunk address | (tid ^ xt) * 16 -- one XOR with a warp-uniform value, no carry into the slice bits
+    unsigned char* smem = smem_raw + ((kRingAlign - (smem_u32(smem_raw) & (kRingAlign - 1u))) & (kRingAlign - 1u));
     unsigned char* q = smem + (size_t)p.nring * CHUNK_BYTES;
     uint64_t* bars = reinterpret_cast<uint64_t*>(q);
     q += 2 * kMaxRing * 8;
@@ -267,6 +322,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
             uint32_t base = 0;
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
             const uint32_t bt = base | ((uint32_t)tid << (TB - 8));   // index of the element's first amplitude, r bits 0
+            const uint32_t stage_base = smem_u32(smem), tid16 = (uint32_t)tid << 4;
             T ar[R * PAIR], ai[R * PAIR];
 #pragma unroll
             for (int r = 0; r < R * PAIR; ++r) {
@@ -277,28 +333,25 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 const int t0 = tab.load_t0[l], t1 = tab.load_t0[l + 1];
                 for (uint32_t c = 0; c < (uint32_t)NC; ++c) {
                     mbar_wait(bar_full + 8 * pos, phase);
-                    const unsigned char* cp = smem + (size_t)pos * CHUNK_BYTES;
+                    const uint32_t cp = stage_base + (uint32_t)pos * CHUNK_BYTES + tid16;
+                    uint4 e = tab.term[t0];
                     for (int t = t0; t < t1; ++t) {
-                        const uint4 e = tab.term[t];
-                        const uint32_t xt = e.x & 511u, xr = (e.x >> 9) & 63u, zr = (e.x >> 16) & 63u;
+                        const uint4 en = tab.term[t + 1 < t1 ? t + 1 : t];   // next entry: its constant-bank latency is hidden
+                        // e.x: bits 0..8 in-slice bits of x | 9..13 r bits of x | 16..20 r bits of z | 31 imaginary coefficient
+                        const uint32_t xr = (e.x >> 9) & 31u, zr = (e.x >> 16) & 31u;
                         const uint32_t oc = c ^ (xr >> LRC);
-                        const unsigned char* pb = cp + (((uint32_t)tid ^ (xt >> (TB - 8))) * 16u);
-                        const uint32_t sgn = (uint32_t)(__popc(bt & e.y) + __popc((oc << LRC) & zr)) << 31;
+                        const uint32_t pb = cp ^ (((e.x & 511u) >> (TB - 8)) << 4);   // (tid ^ xt) * 16: bits 4..11 only
+                        const uint32_t sgn = ((uint32_t)__popc(bt & e.y) + (uint32_t)__popc((oc << LRC) & zr)) << 31;
                         const uint32_t w = (sizeof(T) == 8 ? e.w : e.z) ^ sgn;
                         constexpr uint32_t lo = (uint32_t)RC - 1u;
-                        if constexpr (sizeof(T) == 8) {
-                            if (e.x >> 31) dispatch_chunk<T, R, RC, 0, true, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
-                            else dispatch_chunk<T, R, RC, 0, false, false>(oc, pb, xr & lo, zr & lo, e.z, w, ar, ai);
-                        } else {
-                            const uint32_t aux = (e.y & 1u) << 31;   // second amplitude of the pair: index bit 0 set
-                            if (e.x >> 31) {
-                                if (xt & 1u) dispatch_chunk<T, R, RC, 0, true, true>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
-                                else dispatch_chunk<T, R, RC, 0, true, false>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
-                            } else {
-                                if (xt & 1u) dispatch_chunk<T, R, RC, 0, false, true>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
-                                else dispatch_chunk<T, R, RC, 0, false, false>(oc, pb, xr & lo, zr & lo, aux, w, ar, ai);
-                            }
+                        uint32_t variant = (zr & 3u) | ((e.x >> 31) << 2);
+                        uint32_t aux = e.z;
+                        if constexpr (sizeof(T) == 4) {
+                            variant |= (e.x & 1u) << 3;            // the mask flips index bit 0: the pair arrives swapped
+                            aux = (e.y & 1u) << 31;                // second amplitude of the pair: index bit 0 set
                         }
+                        dispatch_chunk<T, R, RC, 0>(oc, variant, pb, xr & lo, (zr & lo) >> 2, aux, w, ar, ai);
+                        e = en;
                     }
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_empty + 8 * pos);
@@ -579,9 +632,9 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
     p.prev = (const C*)fa.prev;
     p.sc = fa.sc;
     p.j = fa.j;
-    p.nring = (int)((kSmemLimit - kMiscBytes) / kChunkBytes);
+    p.nring = (int)((kSmemLimit - kMiscBytes - kRingAlign) / kChunkBytes);
     if (p.nring > kMaxRing) p.nring = kMaxRing;
-    const size_t smem = (size_t)p.nring * kChunkBytes + kMiscBytes;
+    const size_t smem = (size_t)p.nring * kChunkBytes + kMiscBytes + kRingAlign;
     const int sms = num_sms();
     if (sms <= 0) return SYK_ECUDA;
     const uint64_t n_tiles = 1ull << tab.n_outer;
@@ -644,6 +697,12 @@ int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes
     if (window_mask) *window_mask = win;
     return SYK_OK;
 }
+
+int scatter_tile_bits(int dtype) {
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    return kStTB[k] + kStNR[k];
+}
+int scatter_window_bits() { return kWindowBits; }
 
 void free_scatter_tables(const syk_ham* h) {
     for (int k = 0; k < 2; ++k) {

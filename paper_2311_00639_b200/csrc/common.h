@@ -87,12 +87,20 @@ struct syk_ham {
     int N = 0;
     int L = 0;
     int gamma_norm = 0;
+    // Tables in the STORAGE basis: what every kernel table is built from.  Index bit perm[q] of a stored vector is qubit q
+    // (qubit relabelling); with the identity layout they equal the canonical tables below.
     std::vector<uint64_t> x;                   // [n_groups]
     std::vector<uint32_t> group_off;           // [n_groups+1]
     std::vector<uint64_t> z;                   // [n_terms]
     std::vector<std::complex<double>> c;       // [n_terms]
-    std::vector<int32_t> quartet;              // [n_terms*4]
-    std::vector<double> J;                     // [n_terms]
+    // Canonical tables (a-1, qubit q = index bit q): what syk_ham_tables exports; fixed at build time.
+    std::vector<uint64_t> can_x;               // [n_groups]
+    std::vector<uint32_t> can_group_off;       // [n_groups+1]
+    std::vector<uint64_t> can_z;               // [n_terms]
+    std::vector<std::complex<double>> can_c;   // [n_terms]
+    std::vector<int32_t> quartet;              // [n_terms*4]  canonical term order
+    std::vector<double> J;                     // [n_terms]    canonical term order
+    std::vector<uint8_t> perm;                 // [L] qubit -> index bit of stored vectors; empty = identity
     int block_of_N = 0;                        // parity block (syk_build_parity_block): N of the full Hamiltonian, else 0
     int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
     bool generic = false;                      // built from caller-supplied Pauli strings (no Majorana meaning)
@@ -102,6 +110,14 @@ struct syk_ham {
     mutable syk::RtCache* rt[2] = {nullptr, nullptr};   // register-tile kernel tables per dtype (host, lazily built)
     mutable syk::StCache* st[2] = {nullptr, nullptr};   // scatter-tile kernel tables per dtype (host, lazily built)
     mutable syk::DenseCache* dn[2] = {nullptr, nullptr};   // dense-table kernel tables per dtype (device, lazily built)
+    bool identity_layout() const { return perm.empty(); }
+    int bit_of_qubit(int q) const { return perm.empty() ? q : (int)perm[(size_t)q]; }
+    uint64_t to_storage(uint64_t mask) const {   // a mask over qubits -> the same mask over index bits
+        if (perm.empty()) return mask;
+        uint64_t r = 0;
+        for (int q = 0; q < L; ++q) r |= ((mask >> q) & 1ull) << perm[(size_t)q];
+        return r;
+    }
     int64_t n_terms() const { return (int64_t)z.size(); }
     int64_t n_groups() const { return (int64_t)x.size(); }
 };
@@ -183,6 +199,8 @@ int launch_apply_h_scatter(const syk_ham* h, int dtype, const void* d_in, void* 
 int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
                         uint32_t* window_mask);
 void free_scatter_tables(const syk_ham* h);
+int scatter_tile_bits(int dtype);      // index bits of one tile (13 complex128 / 14 complex64)
+int scatter_window_bits();             // ~log2(tiles in flight)
 
 // dense-table kernel (apply_h_dense.cu)
 bool dense_kernel_ok(const syk_ham* h, bool forced);
@@ -235,11 +253,21 @@ int cdot_batched(int dtype, uint64_t D, const void* d_a, const void* d_b, Lanczo
 int launch_normalise(int dtype, uint64_t D, void* d_v, LanczosScalars* sc, cudaStream_t stream);
 int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, void* d_out, cudaStream_t stream,
                  const Batch& bt = Batch());
+// gamma_n in the storage basis of `h` (a full-space handle, or a parity block for n < N_full - 2): the Jordan-Wigner string
+// with its masks mapped through the handle's qubit layout
+int launch_gamma_h(const syk_ham* h, int n, int dtype, const void* d_in, void* d_out, cudaStream_t stream,
+                   const Batch& bt = Batch());
+// out[i] = in[sigma(i)], sigma = the bit permutation that moves index bit j to bit src_bit[j]
+int launch_bit_permute(int L, const uint8_t* src_bit, int dtype, const void* d_in, void* d_out, cudaStream_t stream);
+// canonical -> storage basis of h (to_layout) or back; in != out
+int permute_vector(const syk_ham* h, int dtype, bool to_layout, const void* d_in, void* d_out, cudaStream_t stream);
+// drops every cached kernel table of the handle (after a change of layout)
+void invalidate_kernel_tables(const syk_ham* h);
 // gamma_n of the FULL space (N Majoranas) between parity blocks on N/2-1 qubits; the result lies in sector_out
 int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* d_in, void* d_out,
-                       cudaStream_t stream);
+                       cudaStream_t stream, const syk_ham* layout_of = nullptr);
 int launch_random_fill(int N, uint64_t seed, uint32_t realization, int dtype, void* d_psi, LanczosScalars* sc,
-                       cudaStream_t stream);
+                       cudaStream_t stream, const syk_ham* layout_of = nullptr);
 int apply_h_kernel_kind(const syk_ham* h, int dtype);
 
 // Krylov driver internals shared with the OTOC pipeline (krylov.cu)

@@ -164,6 +164,14 @@ void free_device_tables(const syk_ham* h) {
     d = DeviceTables();
 }
 
+void invalidate_kernel_tables(const syk_ham* h) {
+    free_device_tables(h);
+    free_regtile_tables(h);
+    free_scatter_tables(h);
+    free_dense_tables(h);
+    h->dense_representable = -1;
+}
+
 }  // namespace syk
 
 extern "C" {

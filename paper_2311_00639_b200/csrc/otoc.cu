@@ -25,9 +25,10 @@ struct Space {
     int N;         // Majoranas of the FULL Hamiltonian
     int gamma_norm;
     const syk_ham* ham(int sec) const { return sector < 0 ? hs[0] : hs[sec]; }
+    // vectors live in the qubit layout of the handles (both blocks share one layout: a gamma maps between them)
     int gamma(int n, int sec_out, int dtype, const void* in, void* out, cudaStream_t st) const {
-        return sector < 0 ? launch_gamma(N, n, gamma_norm, dtype, in, out, st)
-                          : launch_gamma_block(N, n, gamma_norm, sec_out, dtype, in, out, st);
+        return sector < 0 ? launch_gamma_h(hs[0], n, dtype, in, out, st)
+                          : launch_gamma_block(N, n, gamma_norm, sec_out, dtype, in, out, st, hs[0]);
     }
 };
 
@@ -150,7 +151,6 @@ static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int 
     const size_t kbytes = krylov_batched_bytes(h0, nb, dtype, m);
     const size_t ws_stride = krylov_header_bytes() + (size_t)m * v;
     LanczosScalars* sc = (LanczosScalars*)(kwork + batched_table_bytes(nb));   // realization 0's header
-    const int N = h0->N, gn = h0->gamma_norm;
     bool uploaded = false;
     int rc_soft = SYK_OK;
     auto evolve = [&](void* vec, size_t stride, double tre, double tim) -> int {
@@ -167,7 +167,7 @@ static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int 
         b.n = nb;
         b.s.a = s_in;
         b.s.b = s_out;
-        return launch_gamma(N, n, gn, dtype, in, out, st, b);
+        return launch_gamma_h(h0, n, dtype, in, out, st, b);   // one layout for the whole batch (batched_apply_ok)
     };
     std::vector<double> dots((size_t)2 * nb);
     SYK_TRY(evolve(l, psi_stride, 0.0, -beta / 8.0));
@@ -205,7 +205,7 @@ static Space full_space(const syk_ham* h) { return Space{{h, h}, -1, h->N, h->ga
 // the two blocks of one Hamiltonian: same N, same normalisation, sectors 0 and 1
 static bool blocks_ok(const syk_ham* he, const syk_ham* ho, int sector) {
     return he && ho && (sector == 0 || sector == 1) && he->block_of_N >= 6 && he->block_of_N == ho->block_of_N &&
-           he->sector == 0 && ho->sector == 1 && he->gamma_norm == ho->gamma_norm;
+           he->sector == 0 && ho->sector == 1 && he->gamma_norm == ho->gamma_norm && he->perm == ho->perm;
 }
 
 static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
@@ -329,9 +329,17 @@ int syk_apply_H_host(const syk_ham* h, int dtype, const void* h_in, void* h_out,
     cudaStream_t st = (cudaStream_t)stream;
     char* din = (char*)d_work;
     char* dout = din + v;
-    SYK_CUDA(cudaMemcpyAsync(din, h_in, v, cudaMemcpyHostToDevice, st));
-    SYK_TRY(syk_apply_H(h, dtype, din, dout, stream));
-    SYK_CUDA(cudaMemcpyAsync(h_out, dout, v, cudaMemcpyDeviceToHost, st));
+    if (h->identity_layout()) {
+        SYK_CUDA(cudaMemcpyAsync(din, h_in, v, cudaMemcpyHostToDevice, st));
+        SYK_TRY(syk_apply_H(h, dtype, din, dout, stream));
+        SYK_CUDA(cudaMemcpyAsync(h_out, dout, v, cudaMemcpyDeviceToHost, st));
+    } else {   // host vectors are canonical: one gather pass into / out of the handle's qubit layout
+        SYK_CUDA(cudaMemcpyAsync(dout, h_in, v, cudaMemcpyHostToDevice, st));
+        SYK_TRY(syk::permute_vector(h, dtype, true, dout, din, st));
+        SYK_TRY(syk_apply_H(h, dtype, din, dout, stream));
+        SYK_TRY(syk::permute_vector(h, dtype, false, dout, din, st));
+        SYK_CUDA(cudaMemcpyAsync(h_out, din, v, cudaMemcpyDeviceToHost, st));
+    }
     SYK_CUDA(cudaStreamSynchronize(st));
     return SYK_OK;
 }
@@ -343,10 +351,17 @@ int syk_krylov_evolve_host(const syk_ham* h, int dtype, void* h_psi, double tau_
     const size_t v = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
     if (work_bytes < v) return SYK_ENOMEM;
     cudaStream_t st = (cudaStream_t)stream;
-    SYK_CUDA(cudaMemcpyAsync(d_work, h_psi, v, cudaMemcpyHostToDevice, st));
+    // host vectors are canonical; with a relabelled handle the first Krylov work vector stages the copy (one gather pass
+    // into / out of the handle's qubit layout on either side)
+    char* stage = (char*)d_work + v + syk::krylov_header_bytes();
+    const bool relabelled = !h->identity_layout();
+    if (relabelled && work_bytes < 2 * v + syk::krylov_header_bytes()) return SYK_ENOMEM;
+    SYK_CUDA(cudaMemcpyAsync(relabelled ? (void*)stage : d_work, h_psi, v, cudaMemcpyHostToDevice, st));
+    if (relabelled) SYK_TRY(syk::permute_vector(h, dtype, true, stage, d_work, st));
     int rc = syk_krylov_evolve(h, dtype, d_work, tau_re, tau_im, opts, (char*)d_work + v, work_bytes - v, stats, stream);
     if (rc != SYK_OK && rc != SYK_ENOCONV) return rc;
-    SYK_CUDA(cudaMemcpyAsync(h_psi, d_work, v, cudaMemcpyDeviceToHost, st));
+    if (relabelled) SYK_TRY(syk::permute_vector(h, dtype, false, d_work, stage, st));
+    SYK_CUDA(cudaMemcpyAsync(h_psi, relabelled ? (const void*)stage : (const void*)d_work, v, cudaMemcpyDeviceToHost, st));
     SYK_CUDA(cudaStreamSynchronize(st));
     return rc;
 }

@@ -79,12 +79,153 @@ int compile(int N, int gamma_norm, std::vector<RawTerm>& raw, syk_ham** out) {
             h->quartet.insert(h->quartet.end(), r.q, r.q + 4);
         }
         h->group_off.push_back((uint32_t)h->z.size());
+        // the canonical tables are what syk_ham_tables exports; the storage-basis tables start out equal to them
+        h->can_x = h->x;
+        h->can_group_off = h->group_off;
+        h->can_z = h->z;
+        h->can_c = h->c;
     } catch (const std::bad_alloc&) {
         delete h;
         return SYK_ENOMEM;
     }
     *out = h;
     return SYK_OK;
+}
+
+// Storage-basis tables of a handle for the qubit layout `perm` (qubit q = index bit perm[q]): every canonical string
+// c Z^z X^x becomes c Z^{P z} X^{P x}; groups by ascending P x, terms by ascending P z.  Drops all cached kernel tables.
+int apply_layout(syk_ham* h, const std::vector<uint8_t>& perm) {
+    const int L = h->L;
+    auto map = [&](uint64_t m) {
+        uint64_t r = 0;
+        for (int q = 0; q < L; ++q) r |= ((m >> q) & 1ull) << perm[(size_t)q];
+        return r;
+    };
+    struct T3 { uint64_t x, z; std::complex<double> c; };
+    try {
+        std::vector<T3> t;
+        t.reserve(h->can_z.size());
+        for (size_t g = 0; g < h->can_x.size(); ++g)
+            for (uint32_t k = h->can_group_off[g]; k < h->can_group_off[g + 1]; ++k)
+                t.push_back(T3{map(h->can_x[g]), map(h->can_z[k]), h->can_c[k]});
+        std::sort(t.begin(), t.end(), [](const T3& a, const T3& b) { return a.x != b.x ? a.x < b.x : a.z < b.z; });
+        std::vector<uint64_t> x, z;
+        std::vector<uint32_t> off;
+        std::vector<std::complex<double>> c;
+        for (const T3& e : t) {
+            if (x.empty() || x.back() != e.x) {
+                x.push_back(e.x);
+                off.push_back((uint32_t)z.size());
+            }
+            z.push_back(e.z);
+            c.push_back(e.c);
+        }
+        off.push_back((uint32_t)z.size());
+        bool identity = true;
+        for (int q = 0; q < L; ++q) identity &= perm[(size_t)q] == q;
+        syk::invalidate_kernel_tables(h);
+        h->x.swap(x);
+        h->group_off.swap(off);
+        h->z.swap(z);
+        h->c.swap(c);
+        h->perm = identity ? std::vector<uint8_t>() : perm;
+    } catch (const std::bad_alloc&) {
+        return SYK_ENOMEM;
+    }
+    return SYK_OK;
+}
+
+// ---- choice of the layout -------------------------------------------------------------------
+// The tile kernels move the vector once from L2 into the SMs per distinct value of (x outside the TILE bits) and once
+// from DRAM per distinct value of (x outside TILE + WINDOW bits) (apply_h_scatter.cu).  The X-masks of a sparse SYK
+// Hamiltonian are random 2- and 4-subsets of the qubits, so WHICH qubits sit on the low index bits decides both counts:
+// minimise  loads + 2 passes  over the partition of the qubits into tile / window / rest by deterministic hill climbing
+// from a few starting points.
+struct DistinctCounter {
+    std::vector<uint32_t> key, stamp;
+    uint32_t gen = 0, mask = 0;
+    explicit DistinctCounter(size_t n) {
+        size_t cap = 64;
+        while (cap < 4 * n) cap <<= 1;
+        key.assign(cap, 0);
+        stamp.assign(cap, 0);
+        mask = (uint32_t)cap - 1;
+    }
+    int count(const std::vector<uint32_t>& xs, uint32_t keep) {
+        ++gen;
+        int n = 0;
+        for (uint32_t x : xs) {
+            const uint32_t v = x & keep;
+            uint32_t slot = (v * 0x9E3779B1u) >> 7 & mask;
+            for (;;) {
+                if (stamp[slot] != gen) {
+                    stamp[slot] = gen;
+                    key[slot] = v;
+                    ++n;
+                    break;
+                }
+                if (key[slot] == v) break;
+                slot = (slot + 1) & mask;
+            }
+        }
+        return n;
+    }
+};
+
+void choose_permutation(const syk_ham* h, int n_tile, int n_window, std::vector<uint8_t>& perm) {
+    const int L = h->L;
+    std::vector<uint32_t> xs;
+    for (uint64_t x : h->can_x) xs.push_back((uint32_t)x);
+    DistinctCounter dc(xs.size());
+    const int nt = std::min(n_tile, L), nw = std::min(n_window, L - nt);
+    // seq[0..nt) = qubits of the tile, seq[nt..nt+nw) = window qubits, the rest above
+    auto cost = [&](const std::vector<int>& seq) {
+        uint32_t tile = 0, win = 0;
+        for (int i = 0; i < nt; ++i) tile |= 1u << seq[(size_t)i];
+        win = tile;
+        for (int i = nt; i < nt + nw; ++i) win |= 1u << seq[(size_t)i];
+        return dc.count(xs, ~tile) + 2 * dc.count(xs, ~win);
+    };
+    auto cls = [&](int i) { return i < nt ? 0 : (i < nt + nw ? 1 : 2); };
+    std::vector<int> best;
+    int best_cost = 0;
+    uint64_t rng = 0x243F6A8885A308D3ull;   // fixed: the choice is a deterministic function of the tables
+    for (int start = 0; start < 4; ++start) {
+        std::vector<int> seq((size_t)L);
+        std::iota(seq.begin(), seq.end(), 0);
+        if (start > 0)
+            for (int i = L - 1; i > 0; --i) {   // Fisher-Yates with a 64-bit LCG
+                rng = rng * 6364136223846793005ull + 1442695040888963407ull;
+                std::swap(seq[(size_t)i], seq[(size_t)((rng >> 33) % (uint64_t)(i + 1))]);
+            }
+        int cur = cost(seq);
+        for (int sweep = 0; sweep < 32; ++sweep) {
+            bool improved = false;
+            for (int i = 0; i < nt + nw; ++i)
+                for (int j = i + 1; j < L; ++j) {
+                    if (cls(i) == cls(j)) continue;
+                    std::swap(seq[(size_t)i], seq[(size_t)j]);
+                    const int c = cost(seq);
+                    if (c < cur) {
+                        cur = c;
+                        improved = true;
+                    } else {
+                        std::swap(seq[(size_t)i], seq[(size_t)j]);
+                    }
+                }
+            if (!improved) break;
+        }
+        if (best.empty() || cur < best_cost) {
+            best = seq;
+            best_cost = cur;
+        }
+    }
+    // canonical order inside each class (the cost does not depend on it): ascending qubit numbers
+    std::sort(best.begin(), best.begin() + nt);
+    std::sort(best.begin() + nt, best.begin() + nt + nw);
+    std::sort(best.begin() + nt + nw, best.end());
+    perm.assign((size_t)L, 0);
+    for (int i = 0; i < L; ++i) perm[(size_t)best[(size_t)i]] = (uint8_t)i;
 }
 
 bool make_term(int N, int gamma_norm, const int32_t* q, double J, RawTerm* t) {
@@ -197,16 +338,17 @@ int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out) {
     const uint64_t low = (1ull << (L - 1)) - 1;
     std::vector<RawTerm> raw;
     try {
-        raw.reserve(h->z.size());
-        for (size_t g = 0; g < h->x.size(); ++g)
-            for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1]; ++t) {
+        raw.reserve(h->can_z.size());
+        for (size_t g = 0; g < h->can_x.size(); ++g)
+            for (uint32_t t = h->can_group_off[g]; t < h->can_group_off[g + 1]; ++t) {
                 // c Z^z X^x restricted to the sector (R-BLOCK): the dropped top bit of the output index is
                 // parity(b') xor sector, so a Z on it contributes (-1)^sector and complements the low Z-mask
-                const bool z_top = (h->z[t] >> (L - 1)) & 1ull;
+                // (canonical tables: a block is cut from the canonical Hamiltonian and starts with the identity layout)
+                const bool z_top = (h->can_z[t] >> (L - 1)) & 1ull;
                 RawTerm r;
-                r.x = h->x[g] & low;
-                r.z = z_top ? (~h->z[t]) & low : h->z[t] & low;
-                r.c = (z_top && sector) ? -h->c[t] : h->c[t];
+                r.x = h->can_x[g] & low;
+                r.z = z_top ? (~h->can_z[t]) & low : h->can_z[t] & low;
+                r.c = (z_top && sector) ? -h->can_c[t] : h->can_c[t];
                 for (int k = 0; k < 4; ++k) r.q[k] = h->quartet[4 * (size_t)t + k];
                 r.J = h->J[t];
                 raw.push_back(r);
@@ -224,11 +366,42 @@ int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out) {
 
 void syk_free_hamiltonian(syk_ham* h) {
     if (!h) return;
-    syk::free_device_tables(h);
-    syk::free_regtile_tables(h);
-    syk::free_scatter_tables(h);
-    syk::free_dense_tables(h);
+    syk::invalidate_kernel_tables(h);
     delete h;
+}
+
+int syk_ham_set_layout(syk_ham* h, const int32_t* perm) {
+    if (!h || h->L > 32) return SYK_EINVAL;
+    std::vector<uint8_t> p((size_t)h->L);
+    uint64_t seen = 0;
+    for (int q = 0; q < h->L; ++q) {
+        const int32_t b = perm ? perm[q] : q;
+        if (b < 0 || b >= h->L || ((seen >> b) & 1ull)) return SYK_EINVAL;
+        seen |= 1ull << b;
+        p[(size_t)q] = (uint8_t)b;
+    }
+    return apply_layout(h, p);
+}
+
+int syk_ham_optimize_layout(syk_ham* h, int dtype) {
+    if (!h || h->L > 32 || (dtype != SYK_C64 && dtype != SYK_C128)) return SYK_EINVAL;
+    // only the tile kernels for sparse H gain (<= 1024 terms); anything else keeps the identity layout
+    if (h->n_terms() == 0 || h->n_terms() > syk::kStMaxTerms) return syk_ham_set_layout(h, nullptr);
+    std::vector<uint8_t> p;
+    try {
+        choose_permutation(h, syk::scatter_tile_bits(dtype), syk::scatter_window_bits(), p);
+    } catch (const std::bad_alloc&) {
+        return SYK_ENOMEM;
+    }
+    return apply_layout(h, p);
+}
+
+int syk_ham_layout(const syk_ham* h, int32_t* perm, int* is_identity) {
+    if (!h) return SYK_EINVAL;
+    if (perm)
+        for (int q = 0; q < h->L; ++q) perm[q] = h->bit_of_qubit(q);
+    if (is_identity) *is_identity = h->identity_layout() ? 1 : 0;
+    return SYK_OK;
 }
 
 int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, int64_t* dim) {
@@ -243,13 +416,13 @@ int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, 
 int syk_ham_tables(const syk_ham* h, uint64_t* x, uint32_t* group_off, uint64_t* z, double* c_re_im,
                    int32_t* quartet_of_term, double* J_of_term) {
     if (!h) return SYK_EINVAL;
-    if (x) std::copy(h->x.begin(), h->x.end(), x);
-    if (group_off) std::copy(h->group_off.begin(), h->group_off.end(), group_off);
-    if (z) std::copy(h->z.begin(), h->z.end(), z);
+    if (x) std::copy(h->can_x.begin(), h->can_x.end(), x);
+    if (group_off) std::copy(h->can_group_off.begin(), h->can_group_off.end(), group_off);
+    if (z) std::copy(h->can_z.begin(), h->can_z.end(), z);
     if (c_re_im)
-        for (size_t t = 0; t < h->c.size(); ++t) {
-            c_re_im[2 * t] = h->c[t].real();
-            c_re_im[2 * t + 1] = h->c[t].imag();
+        for (size_t t = 0; t < h->can_c.size(); ++t) {
+            c_re_im[2 * t] = h->can_c[t].real();
+            c_re_im[2 * t + 1] = h->can_c[t].imag();
         }
     if (quartet_of_term) std::copy(h->quartet.begin(), h->quartet.end(), quartet_of_term);
     if (J_of_term) std::copy(h->J.begin(), h->J.end(), J_of_term);

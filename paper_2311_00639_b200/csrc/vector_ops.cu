@@ -278,12 +278,27 @@ __global__ void __launch_bounds__(kThreads) normalise_kernel(typename Unit<T>::V
 }
 
 // R-PSI: amplitude b = rho (cos, sin)(2 pi u2), rho = sqrt(-2 ln u1), from stream 2 of R-RNG; partial |.|^2
+// A bit permutation of basis indices: index bit j moves to bit src_bit[j] (n_bits = 0: identity).
+struct BitPerm {
+    uint8_t src_bit[32];
+    int n_bits;
+};
+__device__ __forceinline__ uint64_t bit_permute(const BitPerm& bp, uint64_t i) {
+    if (bp.n_bits == 0) return i;
+    uint64_t r = 0;
+    for (int j = 0; j < bp.n_bits; ++j) r |= ((i >> j) & 1ull) << bp.src_bit[j];
+    return r;
+}
+
+// The stored amplitude i is the amplitude of the canonical basis state bit_permute(to_canonical, i) (qubit layout of
+// a handle), so a state is the same physical state in every layout.
 template <typename T>
 __global__ void __launch_bounds__(kThreads) random_fill_kernel(typename Cx<T>::type* psi, uint64_t D, uint64_t key,
-                                                               LanczosScalars* sc) {
+                                                               LanczosScalars* sc, const BitPerm to_canonical) {
     __shared__ double red[40];
     double s = 0.0;
-    GRID_STRIDE(b, D) {
+    GRID_STRIDE(i, D) {
+        const uint64_t b = bit_permute(to_canonical, i);
         const double u1 = (double)(rng_draw(key, b, 0) + 1) * 0x1.0p-53;
         const double u2 = (double)rng_draw(key, b, 1) * 0x1.0p-53;
         const double rho = sqrt(-2.0 * log(u1));
@@ -292,7 +307,7 @@ __global__ void __launch_bounds__(kThreads) random_fill_kernel(typename Cx<T>::t
         typename Cx<T>::type o;
         o.x = (T)(rho * cs);
         o.y = (T)(rho * sn);
-        psi[b] = o;
+        psi[i] = o;
         s += (double)o.x * (double)o.x + (double)o.y * (double)o.y;
     }
     s = block_sum(s, red);
@@ -304,14 +319,14 @@ __global__ void __launch_bounds__(kThreads) random_fill_kernel(typename Cx<T>::t
 
 // out = gamma_n in, one thread per pair (b0, b0 | bit); works in place.
 //   gamma_{2q}   = s Z^{bit-1} X^{bit};  gamma_{2q+1} = -i s Z^{2 bit - 1} X^{bit}   (R-JW, R-SIGN)
+// given as the index bit q that is flipped and the Z-mask over index bits (both already mapped through the qubit layout).
 template <typename T>
 __global__ void __launch_bounds__(kThreads) gamma_kernel(const typename Cx<T>::type* in, typename Cx<T>::type* out,
-                                                         uint64_t half, int q, int odd, T s, BatchStride bs) {
+                                                         uint64_t half, int q, uint32_t zmask, int odd, T s, BatchStride bs) {
     using C = typename Cx<T>::type;
     in = at_batch(in, bs.a);
     out = at_batch(out, bs.b);
     const uint64_t bit = 1ull << q;
-    const uint32_t zmask = (uint32_t)(odd ? ((bit << 1) - 1) : (bit - 1));
     GRID_STRIDE(pidx, half) {
         const uint64_t b0 = ((pidx >> q) << (q + 1)) | (pidx & (bit - 1));
         const uint64_t b1 = b0 | bit;
@@ -350,6 +365,13 @@ __global__ void __launch_bounds__(kThreads) gamma_top_kernel(const typename Cx<T
         }
         out[b] = o;
     }
+}
+
+// out[i] = in[bit_permute(bp, i)]: change of qubit layout of a whole vector (writes coalesced, reads gathered)
+template <typename T>
+__global__ void __launch_bounds__(kThreads) bit_permute_kernel(const typename Cx<T>::type* in, typename Cx<T>::type* out,
+                                                               uint64_t D, const BitPerm bp) {
+    GRID_STRIDE(i, D) { out[i] = in[bit_permute(bp, i)]; }
 }
 
 #define DISPATCH(dtype, CALL_D, CALL_F) \
@@ -438,31 +460,89 @@ int launch_normalise(int dtype, uint64_t D, void* v, LanczosScalars* sc, cudaStr
     return SYK_OK;
 }
 
+// index bit j of a vector stored in the layout of `h` is qubit inv[j]: stored index -> canonical index
+static BitPerm to_canonical_perm(const syk_ham* h) {
+    BitPerm bp;
+    bp.n_bits = 0;
+    for (int j = 0; j < 32; ++j) bp.src_bit[j] = (uint8_t)j;
+    if (h && !h->identity_layout()) {
+        bp.n_bits = h->L;
+        for (int q = 0; q < h->L; ++q) bp.src_bit[h->perm[(size_t)q]] = (uint8_t)q;
+    }
+    return bp;
+}
+
 int launch_random_fill(int N, uint64_t seed, uint32_t realization, int dtype, void* psi, LanczosScalars* sc,
-                       cudaStream_t st) {
+                       cudaStream_t st, const syk_ham* layout_of) {
     const uint64_t D = 1ull << (N / 2);
     const uint64_t key = rng_key(seed, realization, kStreamState);
     const int g = grid_for(D);
-    DISPATCH(dtype, (random_fill_kernel<double><<<g, kThreads, 0, st>>>((double2*)psi, D, key, sc)),
-             (random_fill_kernel<float><<<g, kThreads, 0, st>>>((float2*)psi, D, key, sc)));
+    const BitPerm bp = to_canonical_perm(layout_of);
+    DISPATCH(dtype, (random_fill_kernel<double><<<g, kThreads, 0, st>>>((double2*)psi, D, key, sc, bp)),
+             (random_fill_kernel<float><<<g, kThreads, 0, st>>>((float2*)psi, D, key, sc, bp)));
     return SYK_OK;
 }
 
-int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* in, void* out, cudaStream_t st, const Batch& bt) {
-    const uint64_t half = 1ull << (N / 2 - 1);
+static int launch_gamma_masks(int L, int qbit, uint32_t zmask, int odd, int gamma_norm, int dtype, const void* in, void* out,
+                              cudaStream_t st, const Batch& bt) {
+    const uint64_t half = 1ull << (L - 1);
     const dim3 g(grid_for(half), bt.n);
     const double s = gamma_norm == SYK_GAMMA_HALF ? 0.70710678118654752440 : 1.0;
     DISPATCH(dtype,
-             (gamma_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, half, n >> 1, n & 1, s,
+             (gamma_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, half, qbit, zmask, odd, s,
                                                           bt.s)),
-             (gamma_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, half, n >> 1, n & 1,
+             (gamma_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, half, qbit, zmask, odd,
                                                          (float)s, bt.s)));
     return SYK_OK;
 }
 
+int launch_gamma(int N, int n, int gamma_norm, int dtype, const void* in, void* out, cudaStream_t st, const Batch& bt) {
+    const int q = n >> 1, odd = n & 1;
+    const uint64_t bit = 1ull << q;
+    return launch_gamma_masks(N / 2, q, (uint32_t)(odd ? ((bit << 1) - 1) : (bit - 1)), odd, gamma_norm, dtype, in, out, st, bt);
+}
+
+// gamma_n on vectors stored in the qubit layout of `h` (h spans the vector: L qubits): the same string with the flipped
+// qubit and the Z-mask mapped to index bits
+int launch_gamma_h(const syk_ham* h, int n, int dtype, const void* in, void* out, cudaStream_t st, const Batch& bt) {
+    const int q = n >> 1, odd = n & 1;
+    if (q >= h->L) return SYK_EINVAL;
+    const uint64_t bit = 1ull << q;
+    const uint64_t zq = odd ? ((bit << 1) - 1) : (bit - 1);
+    return launch_gamma_masks(h->L, h->bit_of_qubit(q), (uint32_t)h->to_storage(zq), odd, h->gamma_norm, dtype, in, out, st, bt);
+}
+
+int launch_bit_permute(int L, const uint8_t* src_bit, int dtype, const void* in, void* out, cudaStream_t st) {
+    BitPerm bp;
+    bp.n_bits = L;
+    for (int j = 0; j < 32; ++j) bp.src_bit[j] = j < L ? src_bit[j] : (uint8_t)j;
+    const uint64_t D = 1ull << L;
+    const int g = grid_for(D);
+    DISPATCH(dtype, (bit_permute_kernel<double><<<g, kThreads, 0, st>>>((const double2*)in, (double2*)out, D, bp)),
+             (bit_permute_kernel<float><<<g, kThreads, 0, st>>>((const float2*)in, (float2*)out, D, bp)));
+    return SYK_OK;
+}
+
+int permute_vector(const syk_ham* h, int dtype, bool to_layout, const void* in, void* out, cudaStream_t st) {
+    uint8_t src[32];
+    for (int j = 0; j < 32; ++j) src[j] = (uint8_t)j;
+    if (!h->identity_layout()) {
+        // to_layout: out[i] = in[canonical(i)], index bit perm[q] <- qubit q;  back: out[b] = in[storage(b)], bit q <- perm[q]
+        for (int q = 0; q < h->L; ++q) {
+            if (to_layout) src[h->perm[(size_t)q]] = (uint8_t)q;
+            else src[q] = h->perm[(size_t)q];
+        }
+    }
+    return launch_bit_permute(h->L, src, dtype, in, out, st);
+}
+
 int launch_gamma_block(int N, int n, int gamma_norm, int sector_out, int dtype, const void* in, void* out,
-                       cudaStream_t st) {
-    if (n < N - 2) return launch_gamma(N - 2, n, gamma_norm, dtype, in, out, st);   // string lives on the kept qubits
+                       cudaStream_t st, const syk_ham* layout_of) {
+    if (n < N - 2) {   // string lives on the kept qubits
+        if (layout_of) return launch_gamma_h(layout_of, n, dtype, in, out, st);
+        return launch_gamma(N - 2, n, gamma_norm, dtype, in, out, st);
+    }
+    // gamma_{N-2}: (-1)^popcount(b') and gamma_{N-1}: a constant -- both invariant under a relabelling of the kept qubits
     const uint64_t Dr = 1ull << (N / 2 - 1);
     const int g = grid_for(Dr);
     double s = gamma_norm == SYK_GAMMA_HALF ? 0.70710678118654752440 : 1.0;
@@ -536,6 +616,42 @@ int syk_apply_gamma(int N, int n, int gamma_norm, int dtype, const void* d_in, v
         if (a < b + bytes && b < a + bytes) return SYK_EINVAL;
     }
     return syk::launch_gamma(N, n, gamma_norm, dtype, d_in, d_out, (cudaStream_t)stream);
+}
+
+int syk_apply_gamma_h(const syk_ham* h, int n, int dtype, const void* d_in, void* d_out, void* stream) {
+    if (!h || h->generic || h->block_of_N || !ok_vec(h->N, dtype, d_in) || !ok_vec(h->N, dtype, d_out) || n < 0 || n >= h->N)
+        return SYK_EINVAL;
+    if (d_in != d_out) {
+        const size_t bytes = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+        const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+        if (a < b + bytes && b < a + bytes) return SYK_EINVAL;
+    }
+    return syk::launch_gamma_h(h, n, dtype, d_in, d_out, (cudaStream_t)stream);
+}
+
+int syk_apply_gamma_block_h(const syk_ham* h_block, int n, int sector_out, int dtype, const void* d_in, void* d_out,
+                            void* stream) {
+    if (!h_block || h_block->block_of_N < 6 || n < 0 || n >= h_block->block_of_N || (dtype != SYK_C64 && dtype != SYK_C128) ||
+        !d_in || !d_out || (sector_out != 0 && sector_out != 1) || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15))
+        return SYK_EINVAL;
+    return syk::launch_gamma_block(h_block->block_of_N, n, h_block->gamma_norm, sector_out, dtype, d_in, d_out,
+                                   (cudaStream_t)stream, h_block);
+}
+
+int syk_random_state_h(const syk_ham* h, uint64_t seed, uint32_t realization, int dtype, void* d_psi, void* d_scratch,
+                       void* stream) {
+    if (!h || h->L > 32 || !ok_vec(2 * h->L, dtype, d_psi) || !d_scratch || ((uintptr_t)d_scratch & 15)) return SYK_EINVAL;
+    auto* sc = (syk::LanczosScalars*)d_scratch;
+    SYK_TRY(syk::launch_random_fill(2 * h->L, seed, realization, dtype, d_psi, sc, (cudaStream_t)stream, h));
+    return syk::launch_normalise(dtype, 1ull << h->L, d_psi, sc, (cudaStream_t)stream);
+}
+
+int syk_permute_vector(const syk_ham* h, int dtype, int to_layout, const void* d_in, void* d_out, void* stream) {
+    if (!h || h->L > 32 || !ok_vec(2 * h->L, dtype, d_in) || !ok_vec(2 * h->L, dtype, d_out)) return SYK_EINVAL;
+    const size_t bytes = ((size_t)1 << h->L) * syk::elem_bytes(dtype);
+    const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+    if (a < b + bytes && b < a + bytes) return SYK_EINVAL;
+    return syk::permute_vector(h, dtype, to_layout != 0, d_in, d_out, (cudaStream_t)stream);
 }
 
 int syk_random_state(int N, uint64_t seed, uint32_t realization, int dtype, void* d_psi, void* d_scratch,

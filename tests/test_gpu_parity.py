@@ -869,3 +869,145 @@ def test_otoc_run_and_sweep_scripts(B, torch):
     sw = subprocess.run([sys.executable, "-m", "paper_2311_00639_b200.sweep", "--quick"], cwd=root, capture_output=True,
                         text=True, check=True)
     assert "| (i) k=4 |" in sw.stdout and "Affine fit" in sw.stdout
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-3 qubit relabelling (include/syk.h "Qubit layout of a handle")
+# ------------------------------------------------------------------------------------------------------------
+def _to_storage_index(idx, perm):
+    """canonical basis index -> index in a vector stored in the layout perm (qubit q = index bit perm[q])"""
+    idx = np.asarray(idx, dtype=np.uint64)
+    out = np.zeros_like(idx)
+    for q, b in enumerate(perm):
+        out |= ((idx >> np.uint64(q)) & np.uint64(1)) << np.uint64(int(b))
+    return out
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_qubit_layout_apply_gamma_state(B, torch, dt):
+    """A relabelled handle computes the SAME operator on vectors stored in its layout: canonical vector -> device ->
+    syk_permute_vector -> apply_H (every kernel kind) -> back = oracle H.v; likewise gamma_n (all n), the random state,
+    the Lanczos coefficients and the host entry points.  Layouts: the optimiser's choice and a random permutation."""
+    N = 28
+    L = N // 2
+    D = 1 << L
+    q, J = couplings(N, 4, seed=11)
+    v = inputs.gaussian_state(D, 61, npdtype(dt))
+    ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    h = B.syk_build_from_terms(N, q, J)
+    canon = h.tables()
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, code, {"krylov_dim": 5}))
+    a0, b0, _ = B.syk_lanczos_run(h, to_dev(torch, v), 5, wk)
+    rng = np.random.default_rng(5)
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    for which in ("optimised", "random", "random2"):
+        if which == "optimised":                       # (at L = 14 the tile spans almost all qubits: may be the identity)
+            perm = [int(x) for x in B.syk_ham_optimize_layout(h, code)["perm"]]
+        else:
+            perm = [int(x) for x in rng.permutation(L)]
+            B.syk_ham_set_layout(h, perm)
+            assert perm != list(range(L))
+        assert all(np.array_equal(canon[k], h.tables()[k]) for k in ("x", "z", "group_off"))
+        d_can = to_dev(torch, v)
+        d_lay = torch.empty_like(d_can)
+        B.syk_permute_vector(h, True, d_can, d_lay)
+        # the permutation itself: stored[P(b)] = canonical[b]
+        sidx = _to_storage_index(np.arange(D), perm).astype(np.int64)
+        assert np.array_equal(d_lay.cpu().numpy()[sidx], v)
+        for kind in (0, 1, 2, 3):
+            B.syk_set_apply_H_kernel(h, kind)
+            assert B.syk_apply_H_kernel_kind(h, code) == kind
+            d_out = torch.full((D,), complex(float("nan"), float("nan")), dtype=tdtype(torch, dt), device="cuda")
+            B.syk_apply_H(h, d_lay, d_out)
+            d_back = torch.empty_like(d_out)
+            B.syk_permute_vector(h, False, d_out, d_back)
+            assert relerr(d_back.cpu().numpy(), ref) <= TOL[dt], (which, kind)
+        B.syk_set_apply_H_kernel(h, -1)
+        # gamma_n in the layout
+        for n in (0, 1, 2, 9, N - 2, N - 1):
+            d_g = torch.empty_like(d_lay)
+            B.syk_apply_gamma_h(h, n, d_lay, d_g)
+            d_back = torch.empty_like(d_g)
+            B.syk_permute_vector(h, False, d_g, d_back)
+            assert relerr(d_back.cpu().numpy(), ohm.apply_gamma(N, n, v.astype(np.complex128))) <= (1e-15 if dt == "c128" else 1e-7), n
+        # the random state is the same physical state
+        d_psi = torch.empty(D, dtype=tdtype(torch, dt), device="cuda")
+        B.syk_random_state_h(h, 3, 1, d_psi, scratch)
+        d_back = torch.empty_like(d_psi)
+        B.syk_permute_vector(h, False, d_psi, d_back)
+        assert relerr(d_back.cpu().numpy(), orng.random_state(N, 3, 1)) <= (1e-13 if dt == "c128" else 1e-7)
+        # Lanczos coefficients do not depend on the basis
+        a1, b1, _ = B.syk_lanczos_run(h, d_lay, 5, wk)
+        tol = 1e-12 if dt == "c128" else 2e-5
+        assert np.max(np.abs(a1 - a0)) <= tol and np.max(np.abs(b1 - b0)) <= tol
+        # host entry points take canonical vectors
+        out_h = np.zeros(D, dtype=npdtype(dt))
+        B.syk_apply_H_host(h, v, out_h, work(torch, 2 * D * v.itemsize))
+        assert relerr(out_h, ref) <= TOL[dt]
+        o = {"krylov_dim": 8}
+        hp = v.copy()
+        B.syk_krylov_evolve_host(h, hp, 0.7, -0.2, work(torch, B.syk_krylov_workspace_bytes(h, code, o) + D * v.itemsize), o)
+        ref_ev = oev.chebyshev_propagate(N, q, J, 0.7 - 0.2j, v.astype(np.complex128))
+        assert relerr(hp, ref_ev) <= TOL[dt], which
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_qubit_layout_otoc_green_blocks(B, torch, dt):
+    """OTOC and Green function through relabelled handles (full space and parity blocks that share one layout) against the
+    oracle: F(t), G(t) do not depend on the basis when the state is the same physical state."""
+    from oracle import parity as opar
+    N, L = 20, 10
+    p = inputs.bernoulli_p(N, 4)
+    q, J, _ = orng.sample_couplings(N, p, 2, 0)
+    prop = oev.ExactPropagator(N, q, J)
+    psi = orng.random_state(N, 2, 0).astype(npdtype(dt))
+    t_grid = np.array([0.0, 0.8, 2.0])
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    o = {"krylov_dim": 16}
+    scratch = work(torch, B.syk_reduce_scratch_bytes())
+    h = B.syk_build_hamiltonian(N, p, 2, 0)
+    perm = [3, 7, 0, 9, 1, 8, 2, 6, 5, 4]
+    B.syk_ham_set_layout(h, perm)
+    wk = work(torch, B.syk_otoc_workspace_bytes(h, code, o))
+    d_psi = torch.empty(1 << L, dtype=tdtype(torch, dt), device="cuda")
+    for (iW, jV) in ((N - 1, N - 2), (4, 13)):
+        B.syk_random_state_h(h, 2, 0, d_psi, scratch)
+        F, _ = B.syk_otoc(h, iW, jV, 5.0, t_grid, d_psi, wk, o)
+        ref = ootoc.otoc_same_psi(prop, N, iW, jV, 5.0, t_grid, psi.astype(np.complex128))
+        assert np.max(np.abs(F - ref)) / abs(ref[0]) <= TOL[dt], (iW, jV)
+    B.syk_random_state_h(h, 2, 0, d_psi, scratch)
+    G, _ = B.syk_green(h, 7, 2.0, t_grid, d_psi, wk, o)
+    refG = ogreen.green_same_psi(prop, N, 7, 2.0, t_grid, psi.astype(np.complex128))
+    assert np.max(np.abs(G - refG)) / abs(refG[0]) <= TOL[dt]
+    # parity blocks: cut from the canonical Hamiltonian, then both blocks get the same layout on the L-1 kept qubits
+    B.syk_ham_set_layout(h, None)
+    he, ho = B.syk_build_parity_block(h, 0), B.syk_build_parity_block(h, 1)
+    permb = [4, 0, 8, 2, 6, 1, 7, 3, 5]
+    B.syk_ham_set_layout(he, permb)
+    with pytest.raises(B.SykError):                      # blocks with different layouts are rejected
+        B.syk_otoc_block(he, ho, 0, 1, 2, 1.0, [0.0], to_dev(torch, opar.restrict(psi, L, 0)), wk, o)
+    B.syk_ham_set_layout(ho, permb)
+    props = [opar.BlockPropagator(N, q, J, s) for s in (0, 1)]
+    for s in (0, 1):
+        ps = opar.restrict(psi, L, s)
+        hb = he if s == 0 else ho
+        d_can = to_dev(torch, ps)
+        d_lay = torch.empty_like(d_can)
+        B.syk_permute_vector(hb, True, d_can, d_lay)
+        for (iW, jV) in ((N - 1, N - 2), (3, N - 1), (5, 8)):
+            ref = opar.otoc_block_same_psi(props, N, iW, jV, 5.0, t_grid, ps.astype(np.complex128), s)
+            F, _ = B.syk_otoc_block(he, ho, s, iW, jV, 5.0, t_grid, d_lay.clone(), wk, o)
+            assert np.max(np.abs(F - ref)) <= TOL[dt] * max(abs(ref[0]), 1e-3), (s, iW, jV)
+        refG = opar.green_block_same_psi(props, N, 6, 2.0, t_grid, ps.astype(np.complex128), s)
+        G, _ = B.syk_green_block(he, ho, s, 6, 2.0, t_grid, d_lay.clone(), wk, o)
+        assert np.max(np.abs(G - refG)) <= TOL[dt] * abs(refG[0])
+        # gamma between blocks in the layout = oracle block of gamma
+        full = opar.embed(ps.astype(np.complex128), L, s)
+        for n in (0, 5, N - 3, N - 2, N - 1):
+            gref = opar.restrict(ohm.apply_gamma(N, n, full), L, 1 - s)
+            d_g = torch.empty_like(d_lay)
+            B.syk_apply_gamma_block_h(hb, n, 1 - s, d_lay, d_g)
+            d_back = torch.empty_like(d_g)
+            B.syk_permute_vector(hb, False, d_g, d_back)
+            assert relerr(d_back.cpu().numpy(), gref) <= (1e-15 if dt == "c128" else 1e-7), (s, n)

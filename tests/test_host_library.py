@@ -323,3 +323,47 @@ def test_scatter_layout_choice_on_host(B):
         assert lay["n_loads"] + 2 * lay["n_passes"] <= len({v & ~ident_tile for v in x}) + 2 * len({v & ~ident_win for v in x})
         if N >= 56:
             assert lay["n_loads"] < len({v & ~ident_tile for v in x}) and lay["n_passes"] < len({v & ~ident_win for v in x})
+
+
+def _permute_mask(m, perm):
+    return sum(((int(m) >> q) & 1) << int(perm[q]) for q in range(len(perm)))
+
+
+def test_qubit_layout_api_on_host(B):
+    """NEXT-3: the exported qubit relabelling.  syk_ham_optimize_layout returns a permutation, is
+    deterministic, never changes the canonical tables, and cuts the loads / passes of the tile kernel below what the
+    canonical layout (with the kernel's own choice of 2 free tile bits) reaches; the counts the library reports equal a
+    direct count from the permuted X-masks; set_layout validates its argument and NULL restores the identity."""
+    for N, k, code in ((56, 4, B.SYK_C128), (64, 2, B.SYK_C64)):
+        L = N // 2
+        p = inputs.bernoulli_p(N, k)
+        h = B.syk_build_hamiltonian(N, p, 0, 0)
+        t0 = h.tables()
+        lay0 = B.syk_apply_H_layout(h, code)
+        assert B.syk_ham_layout(h)["identity"] and list(B.syk_ham_layout(h)["perm"]) == list(range(L))
+        res = B.syk_ham_optimize_layout(h, code)
+        perm = res["perm"]
+        assert sorted(perm) == list(range(L)) and not res["identity"]
+        h2 = B.syk_build_hamiltonian(N, p, 0, 0)
+        assert list(B.syk_ham_optimize_layout(h2, code)["perm"]) == list(perm)          # deterministic
+        t1 = h.tables()
+        for key in ("x", "group_off", "z", "c", "quartet_of_term", "J"):
+            assert np.array_equal(t0[key], t1[key]), key                                 # canonical tables untouched
+        lay1 = B.syk_apply_H_layout(h, code)
+        xs = [_permute_mask(v, perm) for v in t0["x"]]
+        assert lay1["n_loads"] == len({v & ~lay1["tile_mask"] for v in xs})
+        assert lay1["n_passes"] == len({v & ~lay1["window_mask"] for v in xs})
+        assert lay1["n_loads"] < lay0["n_loads"] and lay1["n_passes"] <= lay0["n_passes"], (lay0, lay1)
+        assert lay1["n_loads"] <= 0.93 * lay0["n_loads"]                                 # N=56: 137 -> ~124, N=64: 100 -> ~92
+        # explicit layouts
+        B.syk_ham_set_layout(h, None)
+        assert B.syk_ham_layout(h)["identity"] and B.syk_apply_H_layout(h, code) == lay0
+        rev = list(range(L - 1, -1, -1))
+        B.syk_ham_set_layout(h, rev)
+        assert list(B.syk_ham_layout(h)["perm"]) == rev
+        for bad in ([0] * L, list(range(1, L + 1)), list(range(L - 1))):
+            with pytest.raises(B.SykError):
+                B.syk_ham_set_layout(h, bad)
+    # dense Hamiltonians (more than 1024 terms) keep the identity
+    hd = B.syk_build_hamiltonian(24, 1.0, 0, 0)
+    assert B.syk_ham_optimize_layout(hd, B.SYK_C128)["identity"]
