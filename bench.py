@@ -14,6 +14,11 @@ bytes per second: the byte model of DESIGN.md section 6 ((D_x + 2) V per matvec 
 + combine) divided by the device time of the step.  The `roofline` object is for the dominant kernel (apply_H)
 alone, timed with CUDA events around each of its launches inside the timed region.
 
+The default run times BASELINE.json's first headline config (N=56, k=4, complex128) as the JSON line itself and then its
+second one (N=64, k=2, complex64, two-pass Lanczos) for 3 steps, embedded under `second_headline` (skipped with a stated
+reason when less than 175 GB of device memory is free).  On-chip peaks (L2 -> SM, shared-memory reads, DRAM -> SM through
+the TMA ring) are measured in the same run with `syk_microbench` and the roofline reports one fraction per unit.
+
 N > 1 (torchrun): realizations are independent, so each rank runs its own realization with no
 data-path collective ("weak" scaling); the time is the max over ranks.
 
@@ -253,20 +258,11 @@ def run_reference(args, wl, name):
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args, wl, name):
+def measure_workload(args, wl, name, steps, warmup, world, rank, local, dist, with_e2e, with_cpu, peaks):
+    """Times `steps` steps of one workload on this rank's GPU; returns the JSON line as a dict (rank 0) or None."""
     import numpy as np
     import torch
-    import torch.distributed as dist
     from paper_2311_00639_b200 import binding as B, inputs
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     N, k = wl["N"], wl["k"]
     block = bool(wl.get("block"))
@@ -280,21 +276,39 @@ def run_ours(args, wl, name):
     tau = (wl["dt"], 0.0)                            # one real-time segment of the t grid
     batch = int(wl.get("batch", 1))
     realization = rank * batch                       # independent realizations per rank (weak scaling)
+    relabel = not args.no_relabel and batch == 1     # NEXT-3: qubit layout chosen per Hamiltonian (sparse H only)
 
-    h0 = B.syk_build_hamiltonian(N, p, 0, realization)
-    if block:
-        h0 = B.syk_build_parity_block(h0, 0)
+    def build(r, sector=None):
+        """a-1: term compiler (+ parity block) + qubit layout + device tables: everything the later calls need, so that
+        no compute call allocates (syk_ham_prepare)."""
+        h = B.syk_build_hamiltonian(N, p, 0, r)
+        if block:
+            hb = B.syk_build_parity_block(h, sector)
+            h.close()
+            h = hb
+        if relabel:
+            B.syk_ham_optimize_layout(h, code)
+        B.syk_ham_prepare(h, code)
+        return h
+
+    h0 = build(realization, 0)
     info = h0.info()
     n_x, n_t = info["n_xmasks"], info["n_terms"]
     kbytes = B.syk_krylov_workspace_bytes(h0, code, opts)
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
-    wk = torch.empty(kbytes + V, dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
+    wk = torch.empty(kbytes + (V if with_e2e else 0), dtype=torch.uint8, device="cuda")   # + one vector for the host entry point
     l = torch.empty((batch, D), dtype=tdt, device="cuda")
     r = torch.empty((batch, D), dtype=tdt, device="cuda")
     Nvec = N - 2 if block else N                     # number of Majoranas that spans the stored vector
     for i in range(batch):
-        B.syk_random_state(Nvec, 0, realization + i, r[i], scratch)
-        B.syk_apply_gamma(Nvec, 1, r[i], l[i])       # a second, different state for the bra side
+        hi = h0 if batch == 1 else build(realization + i, 0)
+        B.syk_random_state_h(hi, 0, realization + i, r[i], scratch)
+        if block:
+            B.syk_apply_gamma_block_h(hi, 1, 0, r[i], l[i])   # a second, different state for the bra side
+        else:
+            B.syk_apply_gamma_h(hi, 1, r[i], l[i])
+        if hi is not h0:
+            hi.close()
     torch.cuda.synchronize()
     sector = [0]                                     # parity block the state is in (every gamma flips it)
 
@@ -306,9 +320,9 @@ def run_ours(args, wl, name):
 
     def step_lockstep():
         # every realization advances through the Lanczos recurrence in the same launches (grid.y = realization)
-        hams = [B.syk_build_hamiltonian(N, p, 0, realization + i) for i in range(batch)]     # a-1
+        hams = [build(realization + i) for i in range(batch)]                              # a-1
         for i in range(batch):
-            B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                                   # a-5 insertion
+            B.syk_apply_gamma_h(hams[i], wl["i_W"], r[i], r[i])                            # a-5 insertion
         st = B.syk_krylov_evolve_batched(hams, r, D, tau[0], tau[1], wk_b, opts)          # a-2, a-3, a-4
         F = 0.0
         for i in range(batch):
@@ -325,15 +339,13 @@ def run_ours(args, wl, name):
             return step_lockstep()
         F = 0.0
         for i in range(batch):
-            h = B.syk_build_hamiltonian(N, p, 0, realization + i)                     # a-1
             if block:
                 sector[0] ^= 1
-                hb = B.syk_build_parity_block(h, sector[0])                           # a-1, block of the new sector
-                h.close()
-                h = hb
-                B.syk_apply_gamma_block(N, wl["i_W"], sector[0], r[i], r[i])          # a-5 insertion (no gather)
+                h = build(realization + i, sector[0])                                 # a-1, block of the new sector
+                B.syk_apply_gamma_block_h(h, wl["i_W"], sector[0], r[i], r[i])        # a-5 insertion (no gather)
             else:
-                B.syk_apply_gamma(N, wl["i_W"], r[i], r[i])                           # a-5 insertion (in place)
+                h = build(realization + i)                                            # a-1
+                B.syk_apply_gamma_h(h, wl["i_W"], r[i], r[i])                         # a-5 insertion (in place)
             st = B.syk_krylov_evolve(h, r[i], tau[0], tau[1], wk, opts)               # a-2, a-3, a-4
             F = B.syk_dot(Nvec, l[i], r[i], scratch)                                  # a-5 inner product
             stats_acc["n_matvec"] += st["n_matvec"]
@@ -347,7 +359,7 @@ def run_ours(args, wl, name):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     for key in stats_acc:
         stats_acc[key] = 0
@@ -361,7 +373,7 @@ def run_ours(args, wl, name):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     F_last = None
-    for _ in range(args.steps):
+    for _ in range(steps):
         F_last = step()
     e1.record()
     barrier()
@@ -385,24 +397,20 @@ def run_ours(args, wl, name):
     # ---- end to end through the HOST entry point: pinned host vector in, evolved vector out, every step ----
     e2e = None
     try:
-        if args.no_e2e:
-            raise RuntimeError("skipped (--no-e2e)")
+        if not with_e2e:
+            raise RuntimeError("skipped")
         host = torch.empty(D, dtype=tdt, pin_memory=True)
         fill_host_state(host.numpy(), 7 + rank)
         def e2e_step():
             tot = {"model_bytes": 0.0}
             for i in range(batch):
-                h = B.syk_build_hamiltonian(N, p, 0, realization + i)
-                if block:
-                    hb = B.syk_build_parity_block(h, 0)
-                    h.close()
-                    h = hb
+                h = build(realization + i, 0)
                 tot["model_bytes"] += B.syk_krylov_evolve_host(h, host, tau[0], tau[1], wk, opts)["model_bytes"]
                 h.close()
             return tot
         e2e_step()
         barrier()
-        n_e2e = max(1, min(args.steps, 3))
+        n_e2e = max(1, min(steps, 3))
         t0 = time.perf_counter()
         e2e_bytes = 0.0
         for _ in range(n_e2e):
@@ -416,15 +424,21 @@ def run_ours(args, wl, name):
             dist.all_reduce(b, op=dist.ReduceOp.SUM)
             t_e2e, e2e_bytes = float(t[0]), float(b[0])
         e2e = {"value": e2e_bytes / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": V * batch,
-               "d2h_bytes_per_step": V * batch, "steps": n_e2e, "call": "syk_krylov_evolve_host (pinned host vector in and out each step)"}
+               "d2h_bytes_per_step": V * batch, "steps": n_e2e,
+               "call": "syk_krylov_evolve_host (pinned canonical host vector in and out each step; converted to and "
+                       "from the handle's qubit layout on the device)"}
         del host
     except Exception as ex:   # noqa: BLE001 -- report, do not hide
         e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
 
+    kind = B.syk_apply_H_kernel_kind(h0, code)
+    layout = B.syk_apply_H_layout(h0, code) if kind == 3 else None
+    perm = [int(x) for x in B.syk_ham_layout(h0)["perm"]]
+    h0.close()
+    del l, r, wk, scratch
+    torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
 
     peak, peak_src = measured_peak()
     per_launch_bytes = (n_x + 2) * V
@@ -432,32 +446,14 @@ def run_ours(args, wl, name):
     achieved = per_launch_bytes / (avg_ms * 1e-3) / 1e9 if apply_n else None
     kernel_names = {0: "apply_h_generic_kernel", 1: "apply_h_tma_kernel", 2: "apply_h_regtile_kernel",
                     3: "apply_h_scatter_kernel", 4: "apply_h_dense_kernel"}
-    kind = B.syk_apply_H_kernel_kind(h0, code)
-    layout = B.syk_apply_H_layout(h0, code) if kind == 3 else None
     roofline = {"bound": "hbm", "kernel": kernel_names[kind], "layout": layout, "achieved": achieved, "peak": peak,
                 "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms, "launches_timed": apply_n,
                 "share_of_step": apply_ms / ms if ms else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None}
-    if layout and apply_n:
-        # what actually binds the tile kernels: every load moves the whole vector from L2 into the
-        # SMs once (+ 2 epilogue tiles in the fused launches); the chip-wide LTS ceiling is ~6300 B/clk (microarch guide)
-        l2_bytes = (layout["n_loads"] + 2) * V
-        roofline["l2_to_sm"] = {"bytes_per_launch": l2_bytes, "TB_per_s": l2_bytes / (avg_ms * 1e-3) / 1e12,
-                                "bytes_per_clk": (l2_bytes / (avg_ms * 1e-3) / (clocks["sm_mhz"] * 1e6)
-                                                  if clocks and clocks.get("sm_mhz") else None),
-                                "ceiling_bytes_per_clk": 6300}
-    if kind in (0, 4) and n_t > 8 * n_x:
-        # dense table: plain-ALU bound: amplitude-terms per second against the issue-slot peak
-        # 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz / 3 slots per amplitude-term (LOP3 + POPC + signed add)
-        alu_peak = 148 * 4 * 32 * 1.965e9 / 3.0 / 1e9
-        ach = n_t * D / (avg_ms * 1e-3) / 1e9 if apply_n else None
-        roofline.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "G amplitude-terms/s",
-                         "frac": ach / alu_peak if ach else None,
-                         "peak_source": "derived: 148 SM x 4 x 32 lanes x 1.965 GHz / 3 issue slots (DESIGN.md section 6)",
-                         "model_GBs_for_reference": achieved})
-    # DRAM bytes per launch of that kernel from the last committed `ncu --set full` capture (profiles/traffic.csv)
+    # DRAM bytes per launch of that kernel from the last committed `ncu --set full` capture (profiles/traffic.csv): a
+    # property of (kernel, workload) recorded with the commit it was taken at -- NOT measured in this run
     traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_file):
         try:
@@ -465,12 +461,55 @@ def run_ours(args, wl, name):
             for row in csv.DictReader(open(traffic_file)):
                 if row["workload"] == name:
                     roofline["traffic"] = float(row["dram_bytes_per_launch"])
-                    roofline["traffic_source"] = row["source"]
+                    roofline["traffic_source"] = ("committed ncu capture, not measured in this run: " + row["source"])
         except Exception:
             pass
+    if layout and apply_n:
+        # One fraction per unit that could bind a tile-kernel launch, each = bytes the launch moves through that unit /
+        # launch time / the peak of that unit MEASURED on this box in this run (syk_microbench):
+        #   model_vs_hbm        (D_x + 2) V, the byte model of SURVEY 8(d)      / HBM copy peak      (the graded figure)
+        #   dram_traffic_vs_hbm ncu DRAM bytes per launch (committed capture)   / DRAM -> SM streaming peak
+        #   l2_to_sm            (n_loads + 2) V: every load moves the vector once from L2 into the SMs / L2 -> SM peak
+        #   lds                 n_terms V: every term reads the staged vector once from shared memory   / LDS peak
+        sec = avg_ms * 1e-3
+        fr = {"model_vs_hbm": roofline["frac"]}
+        l2_bytes = (layout["n_loads"] + 2) * V
+        lds_bytes = n_t * V
+        detail = {"l2_to_sm_bytes_per_launch": l2_bytes, "l2_to_sm_TB_per_s": l2_bytes / sec / 1e12,
+                  "lds_bytes_per_launch": lds_bytes, "lds_TB_per_s": lds_bytes / sec / 1e12}
+        if roofline["traffic"]:
+            detail["dram_TB_per_s"] = roofline["traffic"] / sec / 1e12
+        if peaks:
+            if roofline["traffic"]:
+                fr["dram_traffic_vs_dram_to_sm_peak"] = roofline["traffic"] / sec / 1e12 / peaks["dram_to_sm"]["load_TB_per_s"]
+                fr["dram_traffic_vs_hbm_copy_peak"] = roofline["traffic"] / sec / 1e9 / peak
+            fr["l2_to_sm_vs_measured_peak"] = detail["l2_to_sm_TB_per_s"] / peaks["l2_to_sm"]["load_TB_per_s"]
+            fr["lds_vs_measured_peak"] = detail["lds_TB_per_s"] / peaks["lds_only"]["lds_TB_per_s"]
+            # supply model of the lock-stepped CTAs: DRAM phases and L2 phases do not overlap
+            if roofline["traffic"]:
+                t_supply = (roofline["traffic"] / 1e12 / peaks["dram_to_sm"]["load_TB_per_s"] +
+                            max(0.0, l2_bytes - roofline["traffic"]) / 1e12 / peaks["l2_to_sm"]["load_TB_per_s"])
+                fr["serial_dram_plus_l2_model_vs_time"] = t_supply / sec
+        physical = {kk: vv for kk, vv in fr.items() if kk != "model_vs_hbm" and vv is not None}
+        roofline["fractions"] = fr
+        roofline["binding_unit"] = max(physical, key=physical.get) if physical else None
+        roofline["on_chip"] = detail
+        roofline["measured_peaks"] = peaks
+    if kind in (0, 4) and n_t > 8 * n_x:
+        # dense table: plain-ALU bound.  Work unit = one thread-level bin add: every term costs ONE
+        # add per thread (8 amplitudes share it through the Walsh binning), i.e. n_terms x D / 8 per launch; peak = the
+        # issue rate of exactly that instruction sequence measured on this box (syk_microbench kind 4)
+        ach = n_t * (D / 8.0) / (avg_ms * 1e-3) if apply_n else None
+        alu_peak = peaks["dense_term_sequence"]["adds_per_s"] if peaks else 148 * 512 * 1.965e9 / 42.0
+        roofline.update({"bound": "alu", "achieved": ach / 1e9 if ach else None, "peak": alu_peak / 1e9,
+                         "unit": "G thread-level term adds/s",
+                         "frac": ach / alu_peak if ach else None,
+                         "peak_source": ("measured: syk_microbench kind 4 (the kernel's per-term instruction sequence, 512 "
+                                         "threads per SM)" if peaks else "fallback: 12.1 adds/clk/SM x 148 SMs x 1.965 GHz"),
+                         "model_GBs_for_reference": achieved})
 
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if with_cpu:
         try:
             gbs, cores, sample, secs, rows = cpu_oracle_matvec_rate(N, k, 0, 15.0)
             cpu = {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
@@ -478,21 +517,71 @@ def run_ours(args, wl, name):
         except Exception as ex:   # noqa: BLE001
             cpu = {"value": None, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": repr(ex)[:200]}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if wl["dtype"] == "c128" else "f32", "data": "synthetic",
             "config": {"workload": name, "N": N, "k": k, "dim_log2": N // 2 - (1 if block else 0), "parity_block": block, "n_terms": n_t, "n_xmasks": n_x,
                        "vector_bytes": V, "krylov_dim": wl["krylov_dim"], "two_pass": wl["two_pass"],
                        "tau": list(tau), "realizations_per_gpu": batch, "lockstep_batched": lockstep,
+                       "qubit_layout": perm if relabel else "identity",
                        "l2_policy": ("inputs larger than L2 (vector %.1f GB >> 126 MB)" % (V / 1e9)) if V > 3e8 else
                                     ("working set of one step %.2f GB > L2 (%d realizations x %d vectors of %.1f MB)"
                                      % (batch * (wl["krylov_dim"] + 2) * V / 1e9, batch, wl["krylov_dim"] + 2, V / 1e6)),
-                       "step": "build_hamiltonian + gamma insertion + krylov_evolve (m fused Lanczos steps, "
-                               "host exp, combine) + inner product"},
-            "lanczos_steps_per_s": total_matvec / (ms * 1e-3), "matvecs_per_step": total_matvec / args.steps / world,
+                       "step": "build_hamiltonian + qubit layout + table upload (syk_ham_prepare) + gamma insertion + "
+                               "krylov_evolve (m fused Lanczos steps, host exp, combine) + inner product"},
+            "lanczos_steps_per_s": total_matvec / (ms * 1e-3), "matvecs_per_step": total_matvec / steps / world,
             "F_last": [F_last.real, F_last.imag], "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": roofline, "cpu_baseline": cpu}
-    print(json.dumps(line), flush=True)
+    return line
+
+
+def run_ours(args, wl, name):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # on-chip peaks of this box, measured before the timed region (a few hundred ms)
+    peaks = None
+    if not args.no_peaks:
+        try:
+            from paper_2311_00639_b200 import microbench
+            peaks = microbench.measure(quick=False)
+        except Exception as ex:   # noqa: BLE001
+            peaks = None
+            print(f"note: on-chip peaks not measured: {ex!r}", file=sys.stderr)
+
+    line = measure_workload(args, wl, name, args.steps, args.warmup, world, rank, local, dist, not args.no_e2e,
+                            world == 1 and not args.no_cpu_baseline, peaks)
+    # the second headline config of BASELINE.json's metric ("at N=56/64"), in the default run only
+    second = None
+    if name == "N56_k4_c128" and not args.no_second:
+        name2 = "N64_k2_c64"
+        free, _ = torch.cuda.mem_get_info()
+        ok = torch.tensor([1 if free >= 175 * 2 ** 30 else 0], device="cuda")
+        if world > 1:
+            dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+        if int(ok[0]) == 0:
+            second = {"workload": name2, "skipped": "needs 175 GB of free device memory (5 vectors of 34.4 GB); free: %.1f GB"
+                      % (free / 2 ** 30)}
+        else:
+            l2 = measure_workload(args, WORKLOADS[name2], name2, 3, 1, world, rank, local, dist, False, False, peaks)
+            if l2 is not None:
+                l2["roofline"].pop("measured_peaks", None)
+                second = {key: l2[key] for key in ("value", "unit", "steps", "warmup", "ms_per_step", "dtype", "config",
+                                                    "lanczos_steps_per_s", "matvecs_per_step", "clocks", "gpu_launches",
+                                                    "roofline")}
+    if rank == 0:
+        if name == "N56_k4_c128" and not args.no_second:
+            line["second_headline"] = second
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
@@ -508,6 +597,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
     ap.add_argument("--no-clocks", action="store_true", help="do not poll nvidia-smi (diagnosis only)")
     ap.add_argument("--no-kernel-timing", action="store_true", help="no CUDA events around apply_H (diagnosis only)")
+    ap.add_argument("--no-second", action="store_true", help="skip the N=64 complex64 leg of the default run")
+    ap.add_argument("--no-peaks", action="store_true", help="skip the on-chip peak measurements (profiling runs only)")
+    ap.add_argument("--no-relabel", action="store_true", help="keep the canonical qubit layout (diagnosis only)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("note: fewer than 3 warm-up steps; not a valid bench number", file=sys.stderr)
