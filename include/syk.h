@@ -70,15 +70,26 @@ int syk_version(void);
 int syk_build_hamiltonian(int N, double p, uint64_t seed, uint32_t realization, int gamma_norm, syk_ham** out);
 int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets /* [n_terms][4] */,
                          const double* J /* [n_terms] */, int gamma_norm, syk_ham** out);
-/* Generic Hermitian sum of Pauli strings on L qubits (2 <= L <= 32; spin chains, Ising-type
- * models through the same operator action).  String t is c_t Z^{z_t} X^{x_t} acting as
- * (O v)[b] = c_t (-1)^popcount(b & z_t) v[b xor x_t] (R-SIGN; Y = -i Z X).  Strings must be Hermitian one by one:
- * c_t real when popcount(x_t & z_t) is even, imaginary when odd; otherwise SYK_EINVAL (non-Hermitian operators
- * need Arnoldi: out of scope).  Equal (x, z) are combined.  The handle works with syk_apply_H, syk_lanczos_run,
- * syk_krylov_evolve and the work-space queries (dim = 2^L; syk_ham_info reports N = 2L); the Majorana calls
+/* Generic sum of Pauli strings on L qubits (2 <= L <= 32; spin chains, Ising-type models and
+ * non-Hermitian operators through the same operator action).  String t is c_t Z^{z_t} X^{x_t} acting as
+ * (O v)[b] = c_t (-1)^popcount(b & z_t) v[b xor x_t] (R-SIGN; Y = -i Z X), c_t any finite complex number.  Equal (x, z)
+ * are combined.  A string is Hermitian iff c_t is real when popcount(x_t & z_t) is even and imaginary when it is odd; if
+ * every string is, the handle is Hermitian and evolves by Lanczos, otherwise it is NON-HERMITIAN: syk_apply_H works as
+ * for any handle (strings whose coefficient is neither real nor imaginary use the generic / 16 KiB-tile kernels),
+ * syk_krylov_evolve runs the Arnoldi process with the exponential of the m x m Hessenberg matrix on the host (one-pass
+ * only: two_pass -> SYK_EINVAL), syk_lanczos_run and the batched lock-step calls return SYK_EINVAL.  The handle works with
+ * syk_apply_H, syk_krylov_evolve and the work-space queries (dim = 2^L; syk_ham_info reports N = 2L); the Majorana calls
  * (syk_otoc, syk_green, syk_build_parity_block) reject it. */
 int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, const uint64_t* z, const double* c_re_im,
                                  syk_ham** out);
+/* syk_build_from_terms with COMPLEX couplings J_t = J_re_im[t][0] + i J_re_im[t][1]: the non-Hermitian SYK model named in
+ * PAPER.md:108.  It is Hermitian iff all imaginary parts are zero; a non-Hermitian handle works with syk_apply_H,
+ * syk_krylov_evolve (Arnoldi), syk_build_parity_block and the layout calls, while syk_otoc / syk_green (defined through
+ * thermal factors of a Hermitian H) return SYK_EINVAL.  syk_ham_tables reports Re J in J_of_term; the coefficients c carry the full coupling. */
+int syk_build_from_terms_complex(int N, int64_t n_terms, const int32_t* quartets /* [n_terms][4] */,
+                                 const double* J_re_im /* [n_terms][2] */, int gamma_norm, syk_ham** out);
+/* 1 if the handle is Hermitian (Lanczos), 0 if not (Arnoldi). */
+int syk_ham_is_hermitian(const syk_ham* h);
 void syk_free_hamiltonian(syk_ham* h);
 
 /* Sizes: any output pointer may be NULL. dim = 2^(N/2). */

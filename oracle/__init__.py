@@ -17,11 +17,12 @@ Modules
   green        same-psi and exact-trace retarded Green function
   pauli        generic sums of Pauli strings / spin chains by Kronecker products
   parity       parity blocks H_UU / H_DD, gamma blocks, block OTOC / Green function
+  nonhermitian complex-coupling SYK Hamiltonian; exp(-i tau H) v by the dense matrix exponential
   alg1         literal transcription of the paper's Algorithm 1 (Python + C)    (P6)
 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): Clifford algebra, Hermiticity/trace/parity,
 Tr H^2 closed form, hand-worked Pauli products (tests/golden/), two representations with one
 spectrum, literal Algorithm 1 vs dense, exactly solvable exponentials, group properties,
-OTOC and Green-function closed forms.  Parity unpinned: none of the functions here; what stays unpinned is
+OTOC and Green-function closed forms, nilpotent / diagonal / anti-Hermitian exponentials.  Parity unpinned: none of the functions here; what stays unpinned is
 agreement with the paper's Fig. 1 curves and its iteration counts (no data in PAPER.md).
 """

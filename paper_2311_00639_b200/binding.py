@@ -55,6 +55,8 @@ _SIGNATURES = {
     "syk_build_hamiltonian": (_i, [_i, _d, _u64, _u32, _i, _P(_vp)]),
     "syk_build_from_terms": (_i, [_i, _i64, _vp, _vp, _i, _P(_vp)]),
     "syk_build_from_pauli_strings": (_i, [_i, _i64, _vp, _vp, _vp, _P(_vp)]),
+    "syk_build_from_terms_complex": (_i, [_i, _i64, _vp, _vp, _i, _P(_vp)]),
+    "syk_ham_is_hermitian": (_i, [_vp]),
     "syk_free_hamiltonian": (None, [_vp]),
     "syk_ham_info": (_i, [_vp, _P(_i), _P(_i64), _P(_i64), _P(_i64)]),
     "syk_ham_tables": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -204,8 +206,25 @@ def syk_build_from_terms(N, quartets, J, gamma_norm=SYK_GAMMA_PAULI):
     return Hamiltonian(out.value)
 
 
+def syk_build_from_terms_complex(N, quartets, J, gamma_norm=SYK_GAMMA_PAULI):
+    """Complex couplings: the non-Hermitian SYK model."""
+    q = np.ascontiguousarray(quartets, dtype=np.int32).reshape(-1, 4)
+    Jc = np.asarray(J, dtype=np.complex128).reshape(-1)
+    if len(q) != len(Jc):
+        raise SykError(SYK_EINVAL, "syk_build_from_terms_complex: quartets and J differ in length")
+    Jri = np.ascontiguousarray(np.stack([Jc.real, Jc.imag], axis=1), dtype=np.float64)
+    out = ctypes.c_void_p()
+    _check(_lib.syk_build_from_terms_complex(int(N), len(Jc), q.ctypes.data, Jri.ctypes.data, int(gamma_norm),
+                                             ctypes.byref(out)), "syk_build_from_terms_complex")
+    return Hamiltonian(out.value)
+
+
+def syk_ham_is_hermitian(h):
+    return bool(_check(_lib.syk_ham_is_hermitian(_h(h)), "syk_ham_is_hermitian", soft=(0, 1)))
+
+
 def syk_build_from_pauli_strings(L, terms):
-    """terms: iterable of (x, z, c) with c real or imaginary as Hermiticity demands (see include/syk.h)."""
+    """terms: iterable of (x, z, c), c any complex number (see include/syk.h for when the sum is Hermitian)."""
     terms = list(terms)
     x = np.array([int(t[0]) for t in terms], dtype=np.uint64)
     z = np.array([int(t[1]) for t in terms], dtype=np.uint64)

@@ -556,7 +556,7 @@ bool batched_apply_ok(const syk_ham* const* hams, int nb, int dtype) {
     const int k = dtype == SYK_C128 ? 1 : 0;
     for (int r = 0; r < nb; ++r) {
         const syk_ham* h = hams[r];
-        if (!h || h->N != hams[0]->N || h->L < kTileLog2[k] || h->n_terms() == 0) return false;
+        if (!h || h->N != hams[0]->N || h->L < kTileLog2[k] || h->n_terms() == 0 || !h->hermitian) return false;
         // one gamma scaling, one kind of operator and one space for the whole batch (the pipelines take them from hams[0])
         if (h->gamma_norm != hams[0]->gamma_norm || h->generic != hams[0]->generic ||
             h->block_of_N != hams[0]->block_of_N || h->sector != hams[0]->sector || h->perm != hams[0]->perm)

@@ -104,6 +104,7 @@ struct syk_ham {
     int block_of_N = 0;                        // parity block (syk_build_parity_block): N of the full Hamiltonian, else 0
     int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
     bool generic = false;                      // built from caller-supplied Pauli strings (no Majorana meaning)
+    bool hermitian = true;                     // false: complex couplings / strings with a non-Hermitian coefficient (Arnoldi)
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable int dense_representable = -1;      // dense-table kernel: -1 not checked yet, 0 / 1
     mutable syk::DeviceTables dev;             // created on first device use
@@ -280,6 +281,9 @@ int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, vo
                                double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work,
                                size_t work_bytes, syk_stats* stats, bool* tables_uploaded, cudaStream_t stream);
 int resolve_krylov_dim(const syk_ham* h, const syk_krylov_opts* o);
+// the same call for a non-Hermitian operator: Arnoldi + host exponential of the Hessenberg matrix (arnoldi.cu)
+int arnoldi_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im, const syk_krylov_opts* opts,
+                        void* d_work, size_t work_bytes, syk_stats* stats, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------------------------------
 // The counter-based generator R-RNG, host and device.

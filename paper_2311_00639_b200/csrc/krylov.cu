@@ -227,6 +227,8 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
     if (!valid_args(h, dtype, d_psi, d_work) || !std::isfinite(tau_re) || !std::isfinite(tau_im)) return SYK_EINVAL;
     if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->tol < 0 || opts->max_substeps < 0))
         return SYK_EINVAL;
+    if (!h->hermitian)   // no three-term recurrence without H = H^+: Arnoldi (NEXT-4)
+        return arnoldi_evolve_impl(h, dtype, d_psi, tau_re, tau_im, opts, d_work, work_bytes, stats, st);
     const int m = resolve_dim(h, opts);
     const bool two_pass = opts && opts->two_pass;
     const double tol = (opts && opts->tol > 0) ? opts->tol : (dtype == SYK_C128 ? 1e-12 : 1e-6);
@@ -502,7 +504,7 @@ int syk_krylov_evolve(const syk_ham* h, int dtype, void* d_psi, double tau_re, d
 
 int syk_lanczos_run(const syk_ham* h, int dtype, const void* d_psi, int m, double* alpha, double* beta,
                     void* d_work, size_t work_bytes, syk_stats* stats, void* stream) {
-    if (!syk::valid_args(h, dtype, d_psi, d_work) || !alpha || !beta || m < 1 || m > syk::kMaxKrylov)
+    if (!syk::valid_args(h, dtype, d_psi, d_work) || !alpha || !beta || m < 1 || m > syk::kMaxKrylov || !h->hermitian)
         return SYK_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     syk::Ctx c;

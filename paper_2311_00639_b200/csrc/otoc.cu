@@ -214,6 +214,7 @@ static bool otoc_args_ok(const syk_ham* h, int dtype, int i_W, int j_V, double b
         return false;
     if (((uintptr_t)d_psi & 15) || ((uintptr_t)d_work & 15)) return false;
     if (h->generic) return false;                         // gamma insertions mean nothing for a spin-chain operator
+    if (!h->hermitian) return false;                      // the regularised OTOC / Green function are defined for H = H^+
     const int N = h->block_of_N ? h->block_of_N : h->N;   // operator indices refer to the full Hamiltonian
     if (i_W < 0 || i_W >= N || j_V < 0 || j_V >= N || i_W == j_V || !(beta >= 0.0)) return false;
     double prev = 0.0;

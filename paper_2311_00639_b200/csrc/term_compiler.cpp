@@ -228,18 +228,22 @@ void choose_permutation(const syk_ham* h, int n_tile, int n_window, std::vector<
     for (int i = 0; i < L; ++i) perm[(size_t)best[(size_t)i]] = (uint8_t)i;
 }
 
-bool make_term(int N, int gamma_norm, const int32_t* q, double J, RawTerm* t) {
+bool make_term(int N, int gamma_norm, const int32_t* q, double J, RawTerm* t, double J_im = 0.0) {
     if (!(0 <= q[0] && q[0] < q[1] && q[1] < q[2] && q[2] < q[3] && q[3] < N)) return false;
     PauliString s = mul(mul(mul(jw_gamma(q[0]), jw_gamma(q[1])), jw_gamma(q[2])), jw_gamma(q[3]));
     t->x = s.x;
     t->z = s.z;
     double s4 = (gamma_norm == SYK_GAMMA_HALF) ? 0.25 : 1.0;   // (1/sqrt 2)^4, exact
-    double a = J * s4;
+    double a = J * s4, b = J_im * s4;   // (a + i b) i^ipow, exactly: multiplication by i is a swap and a sign
     switch (s.ipow) {
-        case 0: t->c = {a, 0.0}; break;
-        case 1: t->c = {0.0, a}; break;
-        case 2: t->c = {-a, 0.0}; break;
-        default: t->c = {0.0, -a}; break;
+        case 0: t->c = {a, b}; break;
+        case 1: t->c = {-b, a}; break;
+        case 2: t->c = {-a, -b}; break;
+        default: t->c = {b, -a}; break;
+    }
+    if (J_im == 0.0) {   // keep exact zeros (not -0.0 + 0.0 artefacts): the tile kernels test c for real / imaginary
+        if (s.ipow & 1) t->c = {0.0, t->c.imag()};
+        else t->c = {t->c.real(), 0.0};
     }
     for (int k = 0; k < 4; ++k) t->q[k] = q[k];
     t->J = J;
@@ -300,6 +304,29 @@ int syk_build_from_terms(int N, int64_t n_terms, const int32_t* quartets, const 
     return compile(N, gamma_norm, raw, out);
 }
 
+int syk_build_from_terms_complex(int N, int64_t n_terms, const int32_t* quartets, const double* J_re_im, int gamma_norm,
+                                 syk_ham** out) {
+    if (!valid_common(N, gamma_norm, out) || n_terms < 0 || (n_terms > 0 && (!quartets || !J_re_im))) return SYK_EINVAL;
+    if (n_terms > 0xFFFFFFF0ll) return SYK_EINVAL;
+    *out = nullptr;
+    std::vector<RawTerm> raw;
+    try {
+        raw.resize((size_t)n_terms);
+    } catch (const std::bad_alloc&) {
+        return SYK_ENOMEM;
+    }
+    bool hermitian = true;
+    for (int64_t t = 0; t < n_terms; ++t) {
+        const double re = J_re_im[2 * t], im = J_re_im[2 * t + 1];
+        if (!std::isfinite(re) || !std::isfinite(im)) return SYK_EINVAL;
+        if (!make_term(N, gamma_norm, quartets + 4 * t, re, &raw[(size_t)t], im)) return SYK_EINVAL;
+        hermitian &= im == 0.0;   // a product of four distinct Majoranas is Hermitian: H = H^+ iff every J is real
+    }
+    int rc = compile(N, gamma_norm, raw, out);
+    if (rc == SYK_OK) (*out)->hermitian = hermitian;
+    return rc;
+}
+
 int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, const uint64_t* z, const double* c_re_im,
                                  syk_ham** out) {
     if (!out || L < 2 || L > 32 || n_terms < 0 || (n_terms > 0 && (!x || !z || !c_re_im))) return SYK_EINVAL;
@@ -312,13 +339,16 @@ int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, cons
     } catch (const std::bad_alloc&) {
         return SYK_ENOMEM;
     }
+    bool hermitian = true;
     for (int64_t t = 0; t < n_terms; ++t) {
         if ((x[t] | z[t]) & ~mask) return SYK_EINVAL;
         const double re = c_re_im[2 * t], im = c_re_im[2 * t + 1];
-        // Hermitian sum of independent strings: (c Z^z X^x)^+ = conj(c) (-1)^popcount(x & z) Z^z X^x, so c must be
-        // real when popcount(x & z) is even and imaginary when it is odd (the Lanczos driver needs H = H^+)
+        // (c Z^z X^x)^+ = conj(c) (-1)^popcount(x & z) Z^z X^x: a string is Hermitian iff c is real when
+        // popcount(x & z) is even and imaginary when it is odd.  Any other coefficient makes the sum non-Hermitian
+        // (checked string by string): such a handle is evolved by Arnoldi instead of Lanczos.
         const bool odd = __builtin_popcountll(x[t] & z[t]) & 1;
-        if (!std::isfinite(re) || !std::isfinite(im) || (odd ? re != 0.0 : im != 0.0)) return SYK_EINVAL;
+        if (!std::isfinite(re) || !std::isfinite(im)) return SYK_EINVAL;
+        hermitian &= odd ? re == 0.0 : im == 0.0;
         RawTerm& r = raw[(size_t)t];
         r.x = x[t];
         r.z = z[t];
@@ -327,7 +357,10 @@ int syk_build_from_pauli_strings(int L, int64_t n_terms, const uint64_t* x, cons
         r.J = 0.0;
     }
     int rc = compile(2 * L, SYK_GAMMA_PAULI, raw, out);
-    if (rc == SYK_OK) (*out)->generic = true;
+    if (rc == SYK_OK) {
+        (*out)->generic = true;
+        (*out)->hermitian = hermitian;
+    }
     return rc;
 }
 
@@ -360,6 +393,7 @@ int syk_build_parity_block(const syk_ham* h, int sector, syk_ham** out) {
     if (rc == SYK_OK) {
         (*out)->block_of_N = h->N;
         (*out)->sector = sector;
+        (*out)->hermitian = h->hermitian;
     }
     return rc;
 }
@@ -403,6 +437,8 @@ int syk_ham_layout(const syk_ham* h, int32_t* perm, int* is_identity) {
     if (is_identity) *is_identity = h->identity_layout() ? 1 : 0;
     return SYK_OK;
 }
+
+int syk_ham_is_hermitian(const syk_ham* h) { return h ? (h->hermitian ? 1 : 0) : SYK_EINVAL; }
 
 int syk_ham_info(const syk_ham* h, int* N, int64_t* n_terms, int64_t* n_xmasks, int64_t* dim) {
     if (!h) return SYK_EINVAL;

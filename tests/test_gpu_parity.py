@@ -1011,3 +1011,130 @@ def test_qubit_layout_otoc_green_blocks(B, torch, dt):
             d_back = torch.empty_like(d_g)
             B.syk_permute_vector(hb, False, d_g, d_back)
             assert relerr(d_back.cpu().numpy(), gref) <= (1e-15 if dt == "c128" else 1e-7), (s, n)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-4: non-Hermitian operators through Arnoldi (oracle/nonhermitian.py)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_nonhermitian_syk_complex_couplings(B, torch, dt):
+    """Non-Hermitian SYK (complex J) at N = 20: H.v with every kernel the handle can use against the dense matrix, and
+    exp(-i tau H) psi by Arnoldi against the dense matrix exponential for real, imaginary and complex tau."""
+    from oracle import nonhermitian as onh
+    N = 20
+    D = 1 << (N // 2)
+    q, J = couplings(N, 4, seed=13)
+    Jc = J * np.exp(1j * np.random.default_rng(2).uniform(0, 2 * np.pi, len(J)))
+    H = onh.complex_syk_hamiltonian(N, q, Jc)
+    assert np.linalg.norm(H - H.conj().T) > 0.1 * np.linalg.norm(H)
+    h = B.syk_build_from_terms_complex(N, q, Jc)
+    assert not B.syk_ham_is_hermitian(h)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    v = inputs.gaussian_state(D, 91, npdtype(dt))
+    ref = H @ v.astype(np.complex128)
+    seen = set()
+    for kind in (0, 1, 2, 3, 4):
+        B.syk_set_apply_H_kernel(h, kind)
+        seen.add(B.syk_apply_H_kernel_kind(h, code))
+        d_out = torch.full((D,), complex(float("nan"), float("nan")), dtype=tdtype(torch, dt), device="cuda")
+        B.syk_apply_H(h, to_dev(torch, v), d_out)
+        assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt], kind
+    # general complex coefficients: only the generic and the 16 KiB-tile kernels (the latter needs D >= one tile)
+    assert seen == ({0, 1} if dt == "c128" else {0})
+    B.syk_set_apply_H_kernel(h, -1)
+    o = {"krylov_dim": 20}
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, code, o))
+    for tau in (1.5 + 0j, -0.8j, 1.0 - 0.5j, -2.0 + 0.3j):
+        d = to_dev(torch, v)
+        st = B.syk_krylov_evolve(h, d, tau.real, tau.imag, wk, o)
+        exact = onh.expm_propagate(H, tau, v)
+        assert relerr(d.cpu().numpy(), exact) <= TOL[dt], (tau, st)
+        assert st["n_matvec"] >= 2 and st["err_est"] <= TOL[dt]
+    # group law through the library itself
+    a, b = to_dev(torch, v), to_dev(torch, v)
+    B.syk_krylov_evolve(h, a, 0.4, -0.1, wk, o)
+    B.syk_krylov_evolve(h, a, 0.6, 0.0, wk, o)
+    B.syk_krylov_evolve(h, b, 1.0, -0.1, wk, o)
+    assert relerr(a.cpu().numpy(), b.cpu().numpy()) <= 10 * TOL[dt]
+    # what needs H = H^+ is refused
+    with pytest.raises(B.SykError):
+        B.syk_krylov_evolve(h, to_dev(torch, v), 1.0, 0.0, wk, {"krylov_dim": 20, "two_pass": 1})
+    with pytest.raises(B.SykError):
+        B.syk_lanczos_run(h, to_dev(torch, v), 4, wk)
+    with pytest.raises(B.SykError):
+        B.syk_otoc(h, 0, 1, 1.0, [0.0], to_dev(torch, v), work(torch, B.syk_otoc_workspace_bytes(h, code, o)), o)
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_nonhermitian_closed_form_and_spin_chain(B, torch, dt):
+    """(i) one term with a complex coupling, H = J P, P^2 = 1: exp(-i tau H) = cos(tau J) - i sin(tau J) P with complex
+    tau J; Arnoldi breaks down after two steps (exact).  (ii) a non-Hermitian spin chain (asymmetric hopping a la
+    Hatano-Nelson + an imaginary field; every coefficient purely real or imaginary, so the tile kernels apply) on 10 and
+    14 spins: H.v with every kernel against the string-by-string Kronecker action, exp(-i tau H) psi against expm."""
+    import cmath
+    from oracle import nonhermitian as onh
+    from oracle import pauli as opauli
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    N, D = 16, 256
+    psi = inputs.gaussian_state(D, 5, npdtype(dt))
+    qd, Jd = np.array([[1, 4, 6, 11]], dtype=np.int32), np.array([0.7 - 0.4j])
+    h = B.syk_build_from_terms_complex(N, qd, Jd)
+    P = ohm.matvec_sequential(N, qd, np.array([1.0]), psi.astype(np.complex128))
+    o = {"krylov_dim": 8}
+    wk = work(torch, B.syk_krylov_workspace_bytes(h, code, o))
+    d = to_dev(torch, psi)
+    st = B.syk_krylov_evolve(h, d, 2.5, -0.3, wk, o)
+    zz = (2.5 - 0.3j) * Jd[0]
+    ref = cmath.cos(zz) * psi.astype(np.complex128) - 1j * cmath.sin(zz) * P
+    assert relerr(d.cpu().numpy(), ref) <= (1e-12 if dt == "c128" else 1e-5)
+    assert st["krylov_dim_used"] == 2
+
+    def chain(L, g):
+        terms = []
+        for i in range(L - 1):
+            pair = (1 << i) | (1 << (i + 1))
+            # (1+g) s+_i s-_{i+1} + (1-g) s-_i s+_{i+1} = (XX + YY)/2 + i g (YX - XY)/2 ... written as Z^z X^x strings:
+            terms.append((pair, 0, 0.5))                     # X X / 2
+            terms.append((pair, pair, -0.5))                 # Y Y / 2 = -(ZX)(ZX) / 2
+            terms.append((pair, 1 << i, 0.5 * g))            # i g (Y_i X_j)/2 = i g (-i Z_i X_i) X_j / 2 = g/2 Z_i X_i X_j
+            terms.append((pair, 1 << (i + 1), -0.5 * g))     # -i g (X_i Y_j)/2 = -g/2 X_i Z_j X_j
+        for i in range(L):
+            terms.append((0, 1 << i, 0.3j * (i % 3 - 1)))    # imaginary longitudinal field
+        return terms
+
+    L2 = 10
+    t2 = chain(L2, 0.35)
+    H2 = opauli.sum_matrix(L2, t2)
+    assert np.linalg.norm(H2 - H2.conj().T) > 0.1
+    h2 = B.syk_build_from_pauli_strings(L2, t2)
+    assert not B.syk_ham_is_hermitian(h2)
+    v2 = inputs.gaussian_state(1 << L2, 6, npdtype(dt))
+    o2 = {"krylov_dim": 24}
+    wk2 = work(torch, B.syk_krylov_workspace_bytes(h2, code, o2))
+    for tau in (1.2 + 0j, 0.7 - 0.4j):
+        d = to_dev(torch, v2)
+        B.syk_krylov_evolve(h2, d, tau.real, tau.imag, wk2, o2)
+        assert relerr(d.cpu().numpy(), onh.expm_propagate(H2, tau, v2)) <= TOL[dt], tau
+    L3 = 14
+    t3 = chain(L3, -0.6)
+    h3 = B.syk_build_from_pauli_strings(L3, t3)
+    v3 = inputs.gaussian_state(1 << L3, 7, npdtype(dt))
+    ref3 = np.zeros(1 << L3, dtype=np.complex128)
+    for x, z, c in t3:
+        w = v3.astype(np.complex128).reshape([2] * L3)
+        for qq in range(L3):
+            site = np.eye(2, dtype=np.complex128)
+            if (z >> qq) & 1:
+                site = site @ opauli.SZ
+            if (x >> qq) & 1:
+                site = site @ opauli.SX
+            w = np.moveaxis(np.tensordot(site, w, axes=([1], [L3 - 1 - qq])), 0, L3 - 1 - qq)
+        ref3 += c * w.reshape(-1)
+    seen = set()
+    for kind in (0, 1, 2, 3, 4):
+        B.syk_set_apply_H_kernel(h3, kind)
+        seen.add(B.syk_apply_H_kernel_kind(h3, code))
+        d_out = torch.zeros(1 << L3, dtype=tdtype(torch, dt), device="cuda")
+        B.syk_apply_H(h3, to_dev(torch, v3), d_out)
+        assert relerr(d_out.cpu().numpy(), ref3) <= TOL[dt], kind
+    assert seen == {0, 1, 2, 3, 4}

@@ -267,10 +267,20 @@ def test_pauli_string_builder(B):
     H = opauli.sum_matrix(L, terms)
     v = np.random.default_rng(1).normal(size=1 << L) + 1j * np.random.default_rng(2).normal(size=1 << L)
     assert np.allclose(ohm.matvec_from_tables(tab, v), H @ v, atol=1e-13)
-    for bad in ([(1, 1, 1.0)],            # Y-like string needs an imaginary coefficient
-                [(1, 0, 1j)],             # X needs a real one
-                [(1 << L, 0, 1.0)],       # bit outside the chain
-                [(0, 1 << L, 1.0)]):
+    assert B.syk_ham_is_hermitian(h)
+    # the Hermiticity rule, string by string: such sums are accepted and flagged non-Hermitian (Arnoldi, NEXT-4)
+    for nonherm in ([(1, 1, 1.0)],            # a Y-like string is Hermitian only with an imaginary coefficient
+                    [(1, 0, 1j)],             # X only with a real one
+                    [(1, 0, 0.3 - 0.2j), (0, 3, 1.0)]):
+        hn = B.syk_build_from_pauli_strings(L, nonherm)
+        assert not B.syk_ham_is_hermitian(hn)
+        tn = hn.tables()
+        Hn = opauli.sum_matrix(L, nonherm)
+        assert not np.allclose(Hn, Hn.conj().T)
+        assert np.allclose(ohm.matvec_from_tables(tn, v), Hn @ v, atol=1e-13)
+    for bad in ([(1 << L, 0, 1.0)],           # bit outside the chain
+                [(0, 1 << L, 1.0)],
+                [(1, 0, float("nan"))]):
         with pytest.raises(B.SykError):
             B.syk_build_from_pauli_strings(L, bad)
     with pytest.raises(B.SykError):
@@ -367,3 +377,24 @@ def test_qubit_layout_api_on_host(B):
     # dense Hamiltonians (more than 1024 terms) keep the identity
     hd = B.syk_build_hamiltonian(24, 1.0, 0, 0)
     assert B.syk_ham_optimize_layout(hd, B.SYK_C128)["identity"]
+
+
+def test_complex_coupling_builder(B):
+    """syk_build_from_terms_complex (non-Hermitian SYK): the tables are those of the real-coupling builder
+    with every coefficient multiplied by its complex J (Eq. 1 is linear in J); real J gives the identical Hermitian handle."""
+    N = 16
+    q, J, _ = orng.sample_couplings(N, inputs.bernoulli_p(N, 4), 5, 0)
+    Jc = J * np.exp(1j * np.linspace(0.1, 2.9, len(J)))
+    hc = B.syk_build_from_terms_complex(N, q, Jc)
+    h1 = B.syk_build_from_terms(N, q, np.ones(len(J)))
+    assert not B.syk_ham_is_hermitian(hc) and B.syk_ham_is_hermitian(h1)
+    tc, t1 = hc.tables(), h1.tables()
+    for key in ("x", "group_off", "z", "quartet_of_term"):
+        assert np.array_equal(tc[key], t1[key]), key
+    order = {tuple(qq): k for k, qq in enumerate(np.asarray(q).reshape(-1, 4).tolist())}
+    Jsorted = np.array([Jc[order[tuple(qq)]] for qq in tc["quartet_of_term"].tolist()])
+    assert np.allclose(tc["c"], t1["c"] * Jsorted, rtol=1e-15, atol=0)
+    hr = B.syk_build_from_terms_complex(N, q, J.astype(np.complex128))
+    h0 = B.syk_build_from_terms(N, q, J)
+    assert B.syk_ham_is_hermitian(hr)
+    assert all(np.array_equal(hr.tables()[k], h0.tables()[k]) for k in ("x", "z", "c", "group_off"))

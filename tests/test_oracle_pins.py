@@ -463,3 +463,46 @@ def test_P15_pauli_strings_and_spin_chains():
     H6 = pauli.sum_matrix(6, pauli.heisenberg_terms(6, 1.0, 1.0, 0.5, periodic=True))
     Sz = sum(pauli.string_matrix(6, 0, 1 << q) for q in range(6))
     assert np.allclose(H6 @ Sz, Sz @ H6, atol=1e-13) and np.allclose(H6, H6.conj().T, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# P16: non-Hermitian operators (oracle/nonhermitian.py)
+# ------------------------------------------------------------------------------------------------------------
+def test_P16_nonhermitian_propagator_closed_forms():
+    from oracle import nonhermitian as onh
+    v = np.array([0.3 - 0.2j, 1.1 + 0.4j])
+    # nilpotent: H^2 = 0, so exp(-i tau H) = 1 - i tau H exactly (no eigenbasis exists)
+    Hn = np.array([[0.0, 2.5], [0.0, 0.0]], dtype=np.complex128)
+    for tau in (0.7, -1.3 + 0.4j):
+        assert np.allclose(onh.expm_propagate(Hn, tau, v), v - 1j * tau * (Hn @ v), rtol=0, atol=1e-15)
+    # diagonal complex H: element-wise
+    d = np.array([0.4 + 0.3j, -1.2 - 0.7j])
+    assert np.allclose(onh.expm_propagate(np.diag(d), 0.9 - 0.2j, v), np.exp(-1j * (0.9 - 0.2j) * d) * v, atol=1e-15)
+    # Hermitian H: the eigh propagator of oracle/evolve.py
+    r = np.random.default_rng(3)
+    A = r.normal(size=(8, 8)) + 1j * r.normal(size=(8, 8))
+    Hh = A + A.conj().T
+    w = r.normal(size=8) + 1j * r.normal(size=8)
+    assert np.allclose(onh.expm_propagate(Hh, 0.6 - 0.3j, w), evolve.dense_propagator(Hh, 0.6 - 0.3j) @ w, atol=1e-12)
+    # non-normal H: group law, and exp(-i t (i K)) = exp(t K) for Hermitian K
+    assert np.linalg.norm(A @ A.conj().T - A.conj().T @ A) > 1.0
+    one = onh.expm_propagate(A, 0.5, onh.expm_propagate(A, 0.2 - 0.1j, w))
+    assert np.allclose(one, onh.expm_propagate(A, 0.7 - 0.1j, w), atol=1e-11)
+    wk, Uk = np.linalg.eigh(Hh)
+    assert np.allclose(onh.expm_propagate(1j * Hh, 0.3, w), Uk @ (np.exp(0.3 * wk) * (Uk.conj().T @ w)), atol=1e-10)
+
+
+def test_P16_complex_syk_hamiltonian():
+    """Complex couplings: linear in J (real J reproduces the dense Hermitian H of Eq. 1 built by matrix products); H - H^+ =
+    2 i H[Im J]; a purely imaginary J gives an anti-Hermitian H."""
+    from oracle import nonhermitian as onh
+    N = 10
+    q, J, _ = rng.sample_couplings(N, 0.3, 4, 0)
+    H0 = hamiltonian.dense_hamiltonian(N, q, J)
+    assert np.allclose(onh.complex_syk_hamiltonian(N, q, J.astype(np.complex128)), H0, atol=1e-15)
+    Jc = J * np.exp(1j * np.linspace(0.2, 2.5, len(J)))
+    Hc = onh.complex_syk_hamiltonian(N, q, Jc)
+    assert np.allclose(Hc - Hc.conj().T, 2j * hamiltonian.dense_hamiltonian(N, q, Jc.imag.copy()), atol=1e-14)
+    assert np.allclose(Hc, sum(Jt * M for Jt, M in zip(Jc, [hamiltonian.dense_hamiltonian(N, [qq], [1.0]) for qq in q])), atol=1e-14)
+    Hi = onh.complex_syk_hamiltonian(N, q, 1j * J)
+    assert np.allclose(Hi, -Hi.conj().T, atol=1e-15)
