@@ -188,6 +188,11 @@ typedef struct {
     double tol;         /* relative error target for the whole call; 0 = default 1e-12 (C128) / 1e-6 (C64) */
     int two_pass;       /* 0: store the m Lanczos vectors (m work vectors); 1: two-pass Lanczos (2 work vectors) */
     int max_substeps;   /* 0 = default 100000 */
+    int renormalize;    /* 1: carry the norm separately: every sub-step rescales its result to the norm
+                           of its input, so |psi| is unchanged by the call and stats->log_norm receives
+                           ln(|exp(-i tau H) psi| / |psi|); the true result is exp(log_norm) times the returned vector.
+                           Needed in complex64 for imaginary times whose growth exp(-beta E_0) leaves the fp32 range
+                           (PAPER.md:363 runs beta = 20 in single precision).  0: the result carries its norm. */
 } syk_krylov_opts;
 
 typedef struct {
@@ -197,6 +202,7 @@ typedef struct {
     double err_est;     /* accumulated a-posteriori error estimate, relative */
     double model_bytes; /* bytes the byte model of DESIGN.md section 6 attributes to the call */
     double elapsed_ms;  /* device time of the call (CUDA events on `stream`) */
+    double log_norm;    /* opts->renormalize: ln of the factor taken out of the result (summed over sub-steps); else 0 */
 } syk_stats;
 
 int syk_krylov_workspace_bytes(const syk_ham* h, int dtype, const syk_krylov_opts* opts, size_t* bytes);

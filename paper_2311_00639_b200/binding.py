@@ -26,12 +26,13 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 class syk_krylov_opts(ctypes.Structure):
     _fields_ = [("krylov_dim", ctypes.c_int), ("tol", ctypes.c_double), ("two_pass", ctypes.c_int),
-                ("max_substeps", ctypes.c_int)]
+                ("max_substeps", ctypes.c_int), ("renormalize", ctypes.c_int)]
 
 
 class syk_stats(ctypes.Structure):
     _fields_ = [("n_matvec", ctypes.c_int64), ("n_substeps", ctypes.c_int), ("krylov_dim_used", ctypes.c_int),
-                ("err_est", ctypes.c_double), ("model_bytes", ctypes.c_double), ("elapsed_ms", ctypes.c_double)]
+                ("err_est", ctypes.c_double), ("model_bytes", ctypes.c_double), ("elapsed_ms", ctypes.c_double),
+                ("log_norm", ctypes.c_double)]
 
     def as_dict(self):
         return {name: getattr(self, name) for name, _ in self._fields_}
@@ -151,7 +152,7 @@ def _opts(opts):
     if isinstance(opts, syk_krylov_opts):
         return ctypes.byref(opts)
     o = syk_krylov_opts(int(opts.get("krylov_dim", 0)), float(opts.get("tol", 0.0)), int(opts.get("two_pass", 0)),
-                        int(opts.get("max_substeps", 0)))
+                        int(opts.get("max_substeps", 0)), int(opts.get("renormalize", 0)))
     return ctypes.byref(o)
 
 

@@ -211,7 +211,16 @@ int arnoldi_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re,
             stats->n_substeps += 1;
             stats->model_bytes += me * ((Dx + 2.0) * V) + (double)me * (me + 1) * 5.0 * V + (me + 1.0) * V;
         }
-        for (int j = 1; j <= me; ++j) coef[(size_t)j] = make_double2(beta0 * y[(size_t)j - 1].real(), beta0 * y[(size_t)j - 1].imag());
+        double scale = beta0;
+        if (opts && opts->renormalize) {   // the result keeps the norm of the input, the factor goes to log_norm
+            double n2 = 0.0;
+            for (int j = 0; j < me; ++j) n2 += std::norm(y[(size_t)j]);
+            if (n2 > 0.0) {
+                scale = beta0 / std::sqrt(n2);
+                if (stats) stats->log_norm += 0.5 * std::log(n2);
+            }
+        }
+        for (int j = 1; j <= me; ++j) coef[(size_t)j] = make_double2(scale * y[(size_t)j - 1].real(), scale * y[(size_t)j - 1].imag());
         SYK_CUDA(cudaMemcpyAsync(sc->coef, coef.data(), sizeof(double2) * (size_t)(me + 1), cudaMemcpyHostToDevice, st));
         SYK_TRY(upload_unit_norms());
         SYK_TRY(launch_combine(dtype, D, vec(1), vecs, D, me, sc, st));

@@ -161,10 +161,11 @@ struct StepChoice {
     double hs;
     double err;
     bool noconv;
+    double growth;   // |exp(-i dir hs T) e_1| = |result| / |input| of the sub-step
 };
 
 StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, double tol, double len, double remaining,
-                       double eps_break, bool last_allowed, double2* coef) {
+                       double eps_break, bool last_allowed, double2* coef, bool renormalize = false) {
     StepChoice ch{};
     const int me = effective_dim(m, alpha, nrm, eps_break);
     SmallExp se;
@@ -199,8 +200,11 @@ StepChoice choose_step(int m, const double* alpha, const double* nrm, cplx dir, 
     ch.me = me;
     ch.hs = hs;
     ch.err = se.err(hs);
+    ch.growth = se.result_norm(hs);
+    // renormalize: the result keeps the norm of the input, the factor goes to log_norm
+    const double keep = (renormalize && ch.growth > 0.0) ? 1.0 / ch.growth : 1.0;
     for (int j = 1; j <= me; ++j) {
-        const cplx v = se.comp(j - 1, hs) * nrm[1];
+        const cplx v = se.comp(j - 1, hs) * (nrm[1] * keep);
         coef[j] = make_double2(v.real(), v.imag());
     }
     return ch;
@@ -233,6 +237,7 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
     const bool two_pass = opts && opts->two_pass;
     const double tol = (opts && opts->tol > 0) ? opts->tol : (dtype == SYK_C128 ? 1e-12 : 1e-6);
     const int max_sub = (opts && opts->max_substeps > 0) ? opts->max_substeps : 100000;
+    const bool renorm = opts && opts->renormalize;
 
     Ctx c;
     c.h = h;
@@ -270,7 +275,8 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
         SYK_TRY(fetch_scalars(c, m, alpha.data(), nrm.data()));
         if (!(nrm[1] > 0.0)) return SYK_OK;   // zero vector stays zero
         const StepChoice ch = choose_step(m, alpha.data(), nrm.data(), dir, tol, len, remaining, eps_break,
-                                          n_sub >= max_sub, coef.data());
+                                          n_sub >= max_sub, coef.data(), renorm);
+        if (renorm && stats && ch.growth > 0.0) stats->log_norm += std::log(ch.growth);
         const int me = ch.me;
         const double hs = ch.hs;
         if (ch.noconv) rc = SYK_ENOCONV;
@@ -458,7 +464,8 @@ int syk_krylov_evolve_batched(const syk_ham* const* hams, int n_batch, int dtype
     if (!hams || n_batch < 1 || !hams[0] || !syk::valid_args(hams[0], dtype, d_psi, d_work) || !std::isfinite(tau_re) ||
         !std::isfinite(tau_im))
         return SYK_EINVAL;
-    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->tol < 0 || opts->max_substeps < 0 || opts->two_pass))
+    if (opts && (opts->krylov_dim < 0 || opts->krylov_dim == 1 || opts->tol < 0 || opts->max_substeps < 0 || opts->two_pass ||
+                 opts->renormalize))
         return SYK_EINVAL;
     if (batch_stride < ((int64_t)1 << hams[0]->L) || ((size_t)batch_stride * syk::elem_bytes(dtype)) % 16) return SYK_EINVAL;
     if (!syk::batched_apply_ok(hams, n_batch, dtype)) return SYK_EINVAL;

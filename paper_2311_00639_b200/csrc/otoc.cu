@@ -10,6 +10,7 @@
 //   for each t_k:  l <- E(dt) l ; phi <- E(dt) phi
 //                  r <- g_W phi ; r <- E(-t - ib/4) r ; r <- g_V r ; r <- E(t - ib/4) r ; r <- g_W r ;  F_k = <l|r>
 // Resident vectors: l, phi, r + Krylov work (2 in two-pass mode: 5 in total, PAPER.md:249's v+3 with v = 2).
+#include <cmath>
 #include <vector>
 
 #include "common.h"
@@ -32,6 +33,26 @@ struct Space {
     }
 };
 
+// One evolution inside a pipeline: accumulates the call's statistics into `stats` and its log-norm (opts->renormalize:
+// the factor taken out of the vector) into the accumulator of the vector that was evolved.
+static int evolve_tracked(const syk_ham* h, int dtype, void* v, double tre, double tim, const syk_krylov_opts* opts,
+                          void* kwork, size_t kbytes, syk_stats* stats, double* log_norm, cudaStream_t st) {
+    syk_stats loc{};
+    const int rc = krylov_evolve_impl(h, dtype, v, tre, tim, opts, kwork, kbytes, &loc, st);
+    if (stats) {
+        stats->n_matvec += loc.n_matvec;
+        stats->n_substeps += loc.n_substeps;
+        stats->err_est += loc.err_est;
+        stats->model_bytes += loc.model_bytes;
+        if (loc.krylov_dim_used > 0)
+            stats->krylov_dim_used = stats->krylov_dim_used == 0 ? loc.krylov_dim_used
+                                                                 : (loc.krylov_dim_used < stats->krylov_dim_used ? loc.krylov_dim_used : stats->krylov_dim_used);
+        stats->log_norm += loc.log_norm;
+    }
+    *log_norm += loc.log_norm;
+    return rc;
+}
+
 static int otoc_one(const Space& sp, int dtype, int i_W, int j_V, double beta, const double* t_grid, int n_t,
                     void* d_psi, double* F_out, const syk_krylov_opts* opts, void* d_work, size_t work_bytes,
                     syk_stats* stats, cudaStream_t st) {
@@ -48,8 +69,10 @@ static int otoc_one(const Space& sp, int dtype, int i_W, int j_V, double beta, c
     char* kwork = r + vbytes;
     LanczosScalars* sc = (LanczosScalars*)kwork;   // the Krylov header doubles as reduction scratch between evolutions
     int rc_soft = SYK_OK;
-    auto evolve = [&](void* v, int sec, double tre, double tim) -> int {
-        int rc = krylov_evolve_impl(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+    // opts->renormalize: every vector keeps the norm it had and carries the logarithm of the factor taken out of it
+    double ln_l = 0.0, ln_phi = 0.0, ln_r = 0.0;
+    auto evolve = [&](void* v, int sec, double tre, double tim, double* ln) -> int {
+        int rc = evolve_tracked(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, ln, st);
         if (rc == SYK_ENOCONV) {
             rc_soft = rc;
             return SYK_OK;
@@ -57,24 +80,29 @@ static int otoc_one(const Space& sp, int dtype, int i_W, int j_V, double beta, c
         return rc;
     };
     // l lives in sector s0, phi in s1; r goes s0 -> s1 -> s0
-    SYK_TRY(evolve(l, s0, 0.0, -beta / 8.0));
+    SYK_TRY(evolve(l, s0, 0.0, -beta / 8.0, &ln_l));
     SYK_TRY(sp.gamma(j_V, s1, dtype, l, phi, st));
-    SYK_TRY(evolve(phi, s1, 0.0, -beta / 4.0));
+    ln_phi = ln_l;
+    SYK_TRY(evolve(phi, s1, 0.0, -beta / 4.0, &ln_phi));
     double t_prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         const double t = t_grid[k], dt = t - t_prev;
         if (dt > 0.0) {
-            SYK_TRY(evolve(l, s0, dt, 0.0));
-            SYK_TRY(evolve(phi, s1, dt, 0.0));
+            SYK_TRY(evolve(l, s0, dt, 0.0, &ln_l));
+            SYK_TRY(evolve(phi, s1, dt, 0.0, &ln_phi));
         }
         t_prev = t;
         SYK_TRY(sp.gamma(i_W, s0, dtype, phi, r, st));
-        SYK_TRY(evolve(r, s0, -t, -beta / 4.0));
+        ln_r = ln_phi;
+        SYK_TRY(evolve(r, s0, -t, -beta / 4.0, &ln_r));
         SYK_TRY(sp.gamma(j_V, s1, dtype, r, r, st));
-        SYK_TRY(evolve(r, s1, t, -beta / 4.0));
+        SYK_TRY(evolve(r, s1, t, -beta / 4.0, &ln_r));
         SYK_TRY(sp.gamma(i_W, s0, dtype, r, r, st));
         SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
         SYK_TRY(fetch_cdot(sc, F_out + 2 * k, st));
+        const double scale = std::exp(ln_l + ln_r);   // 1 unless opts->renormalize
+        F_out[2 * k] *= scale;
+        F_out[2 * k + 1] *= scale;
     }
     return rc_soft;
 }
@@ -99,27 +127,32 @@ static int green_one(const Space& sp, int dtype, int n, double beta, const doubl
     char* kwork = r + vbytes;
     LanczosScalars* sc = (LanczosScalars*)kwork;
     int rc_soft = SYK_OK;
-    auto evolve = [&](void* v, int sec, double tre, double tim) -> int {
-        int rc = krylov_evolve_impl(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, st);
+    double ln_l = 0.0, ln_phi = 0.0;
+    auto evolve = [&](void* v, int sec, double tre, double tim, double* ln) -> int {
+        int rc = evolve_tracked(sp.ham(sec), dtype, v, tre, tim, opts, kwork, kbytes, stats, ln, st);
         if (rc == SYK_ENOCONV) {
             rc_soft = rc;
             return SYK_OK;
         }
         return rc;
     };
-    SYK_TRY(evolve(l, s0, 0.0, -beta / 2.0));
+    SYK_TRY(evolve(l, s0, 0.0, -beta / 2.0, &ln_l));
     SYK_TRY(sp.gamma(n, s1, dtype, l, phi, st));
+    ln_phi = ln_l;
     double t_prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         const double dt = t_grid[k] - t_prev;
         if (dt > 0.0) {
-            SYK_TRY(evolve(l, s0, dt, 0.0));
-            SYK_TRY(evolve(phi, s1, dt, 0.0));
+            SYK_TRY(evolve(l, s0, dt, 0.0, &ln_l));
+            SYK_TRY(evolve(phi, s1, dt, 0.0, &ln_phi));
         }
         t_prev = t_grid[k];
         SYK_TRY(sp.gamma(n, s0, dtype, phi, r, st));
         SYK_TRY(launch_cdot(dtype, D, l, r, sc, st));
         SYK_TRY(fetch_cdot(sc, G_out + 2 * k, st));
+        const double scale = std::exp(ln_l + ln_phi);   // 1 unless opts->renormalize
+        G_out[2 * k] *= scale;
+        G_out[2 * k + 1] *= scale;
     }
     return rc_soft;
 }
@@ -295,7 +328,7 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
     if (stats) *stats = syk_stats{};
     // lock-step batched pipeline when the realizations qualify (small N, tables in shared memory, one-pass) and the work
     // space is large enough for it (syk_otoc_batched_workspace_bytes); else one realization after the other
-    if (n_batch >= 2 && hams[0] && !(opts && opts->two_pass) && syk::batched_apply_ok(hams, n_batch, dtype) &&
+    if (n_batch >= 2 && hams[0] && !(opts && (opts->two_pass || opts->renormalize)) && syk::batched_apply_ok(hams, n_batch, dtype) &&
         work_bytes >= syk::otoc_batched_bytes(hams[0], n_batch, dtype, opts)) {
         for (int r = 0; r < n_batch; ++r) {
             if (hams[r]->block_of_N || batch_stride < ((int64_t)1 << hams[r]->L)) return SYK_EINVAL;

@@ -1138,3 +1138,53 @@ def test_nonhermitian_closed_form_and_spin_chain(B, torch, dt):
         B.syk_apply_H(h3, to_dev(torch, v3), d_out)
         assert relerr(d_out.cpu().numpy(), ref3) <= TOL[dt], kind
     assert seen == {0, 1, 2, 3, 4}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# norm carrying in imaginary time (syk_krylov_opts.renormalize / syk_stats.log_norm)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_renormalize_evolve_and_otoc(B, torch, propagators, dt):
+    """renormalize = 1: the returned vector keeps the norm of the input and exp(log_norm) x vector is the oracle's
+    result (one-pass, two-pass, several sub-steps); OTOC and Green function are unchanged by it; and at a beta whose
+    growth exp(beta |E_0|) leaves the fp32 range the complex64 pipeline still matches the oracle (PAPER.md:363 runs
+    beta = 20 at N = 64 in single precision)."""
+    N = 16
+    q, J, prop = propagators(N, None)
+    D = 1 << (N // 2)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    psi = (2.5 * inputs.gaussian_state(D, 17, npdtype(dt))).astype(npdtype(dt))
+    h = B.syk_build_from_terms(N, q, J)
+    for o in ({"krylov_dim": 20, "renormalize": 1}, {"krylov_dim": 6, "renormalize": 1, "two_pass": 1}):
+        wk = work(torch, B.syk_krylov_workspace_bytes(h, code, o))
+        for tau in ((0.0, -30.0), (2.0, -7.5), (3.0, 0.0)):
+            d = to_dev(torch, psi)
+            st = B.syk_krylov_evolve(h, d, tau[0], tau[1], wk, o)
+            ref = prop.apply(complex(*tau), psi.astype(np.complex128))
+            got = d.cpu().numpy().astype(np.complex128)
+            assert abs(np.linalg.norm(got) / np.linalg.norm(psi) - 1.0) <= (1e-12 if dt == "c128" else 1e-5)
+            assert relerr(got * math.exp(st["log_norm"]), ref) <= TOL[dt], (o, tau)
+            assert abs(st["log_norm"] - math.log(np.linalg.norm(ref) / np.linalg.norm(psi))) <= (1e-10 if dt == "c128" else 1e-5)
+    # OTOC / Green: same values with and without; large beta in complex64
+    psi1 = orng.random_state(N, 0, 0).astype(npdtype(dt))
+    t_grid = np.array([0.0, 1.0, 2.5])
+    o0, o1 = {"krylov_dim": 20}, {"krylov_dim": 20, "renormalize": 1}
+    wk = work(torch, B.syk_otoc_workspace_bytes(h, code, o1))
+    ref = ootoc.otoc_same_psi(prop, N, 0, 1, 5.0, t_grid, psi1.astype(np.complex128))
+    F1, st1 = B.syk_otoc(h, 0, 1, 5.0, t_grid, to_dev(torch, psi1), wk, o1)
+    F0, _ = B.syk_otoc(h, 0, 1, 5.0, t_grid, to_dev(torch, psi1), wk, o0)
+    assert np.max(np.abs(F1 - ref)) / abs(ref[0]) <= TOL[dt] and np.max(np.abs(F1 - F0)) / abs(ref[0]) <= 2 * TOL[dt]
+    assert st1["log_norm"] != 0.0
+    refG = ogreen.green_same_psi(prop, N, 3, 4.0, t_grid, psi1.astype(np.complex128))
+    G1, _ = B.syk_green(h, 3, 4.0, t_grid, to_dev(torch, psi1), wk, o1)
+    assert np.max(np.abs(G1 - refG)) / abs(refG[0]) <= TOL[dt]
+    beta = 200.0                                             # exp(beta |E_0|) ~ 1e60 and more: beyond fp32
+    E0 = prop.eigenvalues()[0]
+    assert beta * abs(E0) > 130.0
+    refB = ootoc.otoc_same_psi(prop, N, 0, 1, beta, t_grid, psi1.astype(np.complex128))
+    FB, _ = B.syk_otoc(h, 0, 1, beta, t_grid, to_dev(torch, psi1), wk, o1)
+    assert np.all(np.isfinite(FB))
+    assert np.max(np.abs(FB - refB)) / abs(refB[0]) <= (1e-9 if dt == "c128" else 5e-5), np.abs(FB - refB) / abs(refB[0])
+    if dt == "c64":                                          # without norm carrying the same call leaves the fp32 range
+        Fplain, _ = B.syk_otoc(h, 0, 1, beta, t_grid, to_dev(torch, psi1), wk, o0)
+        assert not np.all(np.isfinite(Fplain)) or np.max(np.abs(Fplain - refB)) / abs(refB[0]) > 1e-3
