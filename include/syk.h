@@ -319,6 +319,11 @@ int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes,
  * tiles shared between neighbouring output tiles are still in L2.  epoch_len = 0 lets the CTAs run free.
  * Default (8, 1).  Used only for vectors larger than L2.  0 <= lag <= 30. */
 int syk_set_lockstep(int epoch_len, int lag);
+/* Latency path of the Krylov driver (process-wide switch, default on; results do not depend on it): for vectors of at most
+ * 8 MB one Lanczos round (norm, m fused apply_H + m fused vector kernels, final norm) is captured once per (handle, dtype,
+ * m, buffers) into a CUDA graph and replayed with one launch per round; a per-thread cache holds the 24 most recent
+ * graphs.  Off while syk_profile_enable is on.  Replayed kernels count in syk_launch_count. */
+int syk_set_cuda_graphs(int on);
 /* Number of kernels launched by this library on the calling thread since the last reset. */
 int64_t syk_launch_count(int reset);
 /* Per-kernel device timing for the benchmark's roofline line.  While enabled, every apply_H launch made by the

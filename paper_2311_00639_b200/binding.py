@@ -99,6 +99,7 @@ _SIGNATURES = {
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
     "syk_set_apply_H_kernel": (_i, [_vp, _i]),
     "syk_set_lockstep": (_i, [_i, _i]),
+    "syk_set_cuda_graphs": (_i, [_i]),
     "syk_apply_H_layout": (_i, [_vp, _i, _P(_i), _P(_i), _P(_u32), _P(_u32)]),
     "syk_launch_count": (_i64, [_i]),
     "syk_microbench_workspace_bytes": (_sz, []),
@@ -537,6 +538,10 @@ def syk_apply_H_layout(h, dtype):
 
 def syk_set_lockstep(epoch_len, lag):
     _check(_lib.syk_set_lockstep(int(epoch_len), int(lag)), "syk_set_lockstep")
+
+
+def syk_set_cuda_graphs(on):
+    _check(_lib.syk_set_cuda_graphs(1 if on else 0), "syk_set_cuda_graphs")
 
 
 def syk_launch_count(reset=False):

@@ -105,6 +105,8 @@ struct syk_ham {
     int sector = -1;                           // parity block: 0 even / 1 odd popcount sector
     bool generic = false;                      // built from caller-supplied Pauli strings (no Majorana meaning)
     bool hermitian = true;                     // false: complex couplings / strings with a non-Hermitian coefficient (Arnoldi)
+    uint64_t uid = 0;                          // unique per handle (never reused): key of cached CUDA graphs
+    mutable uint64_t table_epoch = 0;          // bumped whenever the kernel tables are dropped (layout change)
     int forced_kernel = -1;                    // syk_set_apply_H_kernel
     mutable int dense_representable = -1;      // dense-table kernel: -1 not checked yet, 0 / 1
     mutable syk::DeviceTables dev;             // created on first device use
@@ -150,6 +152,8 @@ void set_cuda_error(cudaError_t e, const char* what);
 
 void count_launch(int n = 1);
 // benchmark timing of apply_H launches (syk_profile_*): no-ops unless enabled
+bool profile_enabled();
+uint64_t next_handle_uid();
 void profile_begin(cudaStream_t st);
 void profile_end(cudaStream_t st);
 int num_sms();                                 // SM count of the current device (cached); <= 0 on error
@@ -281,6 +285,7 @@ int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, vo
                                double tau_re, double tau_im, const syk_krylov_opts* opts, void* d_work,
                                size_t work_bytes, syk_stats* stats, bool* tables_uploaded, cudaStream_t stream);
 int resolve_krylov_dim(const syk_ham* h, const syk_krylov_opts* o);
+void set_graphs(int on);
 // the same call for a non-Hermitian operator: Arnoldi + host exponential of the Hessenberg matrix (arnoldi.cu)
 int arnoldi_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, double tau_im, const syk_krylov_opts* opts,
                         void* d_work, size_t work_bytes, syk_stats* stats, cudaStream_t stream);

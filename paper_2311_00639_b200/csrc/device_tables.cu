@@ -1,5 +1,6 @@
 // Device copy of the term tables of one Hamiltonian (created on first device use) plus library-wide plumbing:
 // error text, launch counter, SM count.
+#include <atomic>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -28,6 +29,13 @@ struct ProfileState {
 };
 static thread_local ProfileState g_prof;
 constexpr size_t kMaxProfileEvents = 2 * 65536;
+
+bool profile_enabled() { return g_prof.on; }
+
+uint64_t next_handle_uid() {
+    static std::atomic<uint64_t> counter{0};
+    return ++counter;
+}
 
 void profile_begin(cudaStream_t st) {
     ProfileState& p = g_prof;
@@ -170,6 +178,7 @@ void invalidate_kernel_tables(const syk_ham* h) {
     free_scatter_tables(h);
     free_dense_tables(h);
     h->dense_representable = -1;
+    ++h->table_epoch;
 }
 
 }  // namespace syk

@@ -15,6 +15,7 @@
 //             y += c_j v_j into psi's own buffer as soon as u_1 is no longer needed.  Replaces the restarted
 //             scheme of PAPER.md:301 as the bounded-memory mode (PAPER.md:249 counts v+3 vectors; this is 3).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <complex>
 #include <cstddef>
@@ -132,6 +133,108 @@ int run_recurrence(const Ctx& c, int n_steps, bool with_y) {
         SYK_TRY(launch_axpy_norm(c.dtype, c.D, c.buf(j + 1), c.buf(j), j, c.sc, y, j == 2, c.st));
         if (c.stats) c.stats->n_matvec += 1;
     }
+    return SYK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Latency path for small vectors ("hard parts": configs[0], [1] are launch bound): the
+// 2 n + 2 launches of one Lanczos round have the same arguments every time they are issued for the same (handle, buffers),
+// so the round is captured ONCE into a CUDA graph (on an internal stream) and replayed with one cudaGraphLaunch on the
+// caller's stream.  Keyed by everything that is baked into the kernel arguments; a small per-thread LRU cache.
+// ---------------------------------------------------------------------------------------------------------
+struct GraphKey {
+    uint64_t uid, epoch;
+    int dtype, n_steps, with_y, finalize, forced;
+    const void* psi;
+    const void* work;
+    bool operator==(const GraphKey& o) const {
+        return uid == o.uid && epoch == o.epoch && dtype == o.dtype && n_steps == o.n_steps && with_y == o.with_y &&
+               finalize == o.finalize && forced == o.forced && psi == o.psi && work == o.work;
+    }
+};
+struct GraphEntry {
+    GraphKey key;
+    cudaGraphExec_t exec = nullptr;   // nullptr: capture failed for this key, use direct launches
+    int n_kernels = 0;
+    uint64_t last_use = 0;
+    int device = -1;
+};
+struct GraphCache {
+    std::vector<GraphEntry> e;
+    cudaStream_t cap = nullptr;
+    int cap_device = -1;
+    uint64_t clock = 0;
+    ~GraphCache() {   // process exit: the context may be gone, do not touch CUDA
+    }
+};
+thread_local GraphCache g_graphs;
+constexpr size_t kMaxGraphs = 24;
+constexpr size_t kGraphMaxVectorBytes = (size_t)8 << 20;   // larger vectors are not launch bound
+std::atomic<int> g_graphs_on{1};
+
+int run_recurrence_direct(const Ctx& c, int n_steps, bool with_y, bool finalize) {
+    SYK_TRY(run_recurrence(c, n_steps, with_y));
+    if (finalize) SYK_TRY(launch_finalize_nrm(n_steps + 1, c.sc, c.st));
+    return SYK_OK;
+}
+
+// the round of run_recurrence (+ finalize_nrm) through a cached graph when the vector is small; else direct launches
+int run_round(const Ctx& c, int n_steps, bool with_y, bool finalize) {
+    if (!g_graphs_on.load() || c.vbytes > kGraphMaxVectorBytes || profile_enabled())
+        return run_recurrence_direct(c, n_steps, with_y, finalize);
+    int dev = 0;
+    SYK_CUDA(cudaGetDevice(&dev));
+    GraphCache& gc = g_graphs;
+    const GraphKey key{c.h->uid, c.h->table_epoch, c.dtype, n_steps, with_y ? 1 : 0, finalize ? 1 : 0, c.h->forced_kernel,
+                       c.psi, c.vecs};
+    GraphEntry* hit = nullptr;
+    for (GraphEntry& g : gc.e)
+        if (g.key == key && g.device == dev) hit = &g;
+    if (!hit) {
+        SYK_TRY(ensure_device_tables(c.h));   // allocations cannot happen inside a capture
+        if (apply_h_kernel_kind(c.h, c.dtype) == 4) SYK_TRY(prepare_dense_tables(c.h, c.dtype));
+        if (gc.cap && gc.cap_device != dev) {
+            cudaStreamDestroy(gc.cap);
+            gc.cap = nullptr;
+        }
+        if (!gc.cap) {
+            SYK_CUDA(cudaStreamCreateWithFlags(&gc.cap, cudaStreamNonBlocking));
+            gc.cap_device = dev;
+        }
+        if (gc.e.size() >= kMaxGraphs) {   // evict the least recently used
+            size_t lru = 0;
+            for (size_t i = 1; i < gc.e.size(); ++i)
+                if (gc.e[i].last_use < gc.e[lru].last_use) lru = i;
+            if (gc.e[lru].exec) cudaGraphExecDestroy(gc.e[lru].exec);
+            gc.e.erase(gc.e.begin() + (long)lru);
+        }
+        GraphEntry ne;
+        ne.key = key;
+        ne.device = dev;
+        Ctx cc = c;
+        cc.st = gc.cap;
+        cc.stats = nullptr;
+        const int64_t before = syk_launch_count(0);
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(gc.cap, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+            const int rc = run_recurrence_direct(cc, n_steps, with_y, finalize);
+            const cudaError_t e = cudaStreamEndCapture(gc.cap, &graph);
+            if (rc == SYK_OK && e == cudaSuccess && graph) {
+                if (cudaGraphInstantiate(&ne.exec, graph, 0) != cudaSuccess) ne.exec = nullptr;
+            }
+            if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();
+        ne.n_kernels = (int)(syk_launch_count(0) - before);
+        count_launch(-ne.n_kernels);   // nothing ran during the capture
+        gc.e.push_back(ne);
+        hit = &gc.e.back();
+    }
+    hit->last_use = ++gc.clock;
+    if (!hit->exec) return run_recurrence_direct(c, n_steps, with_y, finalize);
+    SYK_CUDA(cudaGraphLaunch(hit->exec, c.st));
+    count_launch(hit->n_kernels);
+    if (c.stats) c.stats->n_matvec += n_steps;
     return SYK_OK;
 }
 
@@ -270,8 +373,7 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
     int n_sub = 0;
     while (remaining > 1e-15 * len) {
         ++n_sub;
-        SYK_TRY(run_recurrence(c, m, false));
-        SYK_TRY(launch_finalize_nrm(m + 1, c.sc, st));
+        SYK_TRY(run_round(c, m, false, true));
         SYK_TRY(fetch_scalars(c, m, alpha.data(), nrm.data()));
         if (!(nrm[1] > 0.0)) return SYK_OK;   // zero vector stays zero
         const StepChoice ch = choose_step(m, alpha.data(), nrm.data(), dir, tol, len, remaining, eps_break,
@@ -293,7 +395,7 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
             if (me == 1) {
                 SYK_TRY(launch_axpy_coef(dtype, c.D, c.psi, nullptr, 1, 1, c.sc, st));
             } else {
-                SYK_TRY(run_recurrence(c, me - 1, true));
+                SYK_TRY(run_round(c, me - 1, true, false));
                 SYK_TRY(launch_axpy_coef(dtype, c.D, c.psi, c.buf(me), me, me == 2, c.sc, st));
             }
             if (stats) stats->model_bytes += (m + me - 1) * ((Dx + 3.0) * V + 3.0 * V) + 2.0 * V + 2.0 * me * V;
@@ -311,6 +413,7 @@ int krylov_evolve_impl(const syk_ham* h, int dtype, void* d_psi, double tau_re, 
 // finish.
 // ---------------------------------------------------------------------------------------------------------
 int resolve_krylov_dim(const syk_ham* h, const syk_krylov_opts* o) { return resolve_dim(h, o); }
+void set_graphs(int on) { g_graphs_on.store(on); }
 
 size_t krylov_batched_bytes(const syk_ham* h0, int nb, int dtype, int m) {
     const size_t v = ((size_t)1 << h0->L) * elem_bytes(dtype);
@@ -449,6 +552,11 @@ int krylov_evolve_batched_impl(const syk_ham* const* hams, int nb, int dtype, vo
 }  // namespace syk
 
 extern "C" {
+
+int syk_set_cuda_graphs(int on) {
+    syk::set_graphs(on != 0);
+    return SYK_OK;
+}
 
 int syk_krylov_workspace_bytes_batched(const syk_ham* h, int n_batch, int dtype, const syk_krylov_opts* opts,
                                        size_t* bytes) {

@@ -61,6 +61,7 @@ int compile(int N, int gamma_norm, std::vector<RawTerm>& raw, syk_ham** out) {
     h->N = N;
     h->L = N / 2;
     h->gamma_norm = gamma_norm;
+    h->uid = syk::next_handle_uid();
     try {
         for (size_t t = 0; t < raw.size(); ++t) {
             const RawTerm& r = raw[t];

@@ -1,6 +1,7 @@
 """On-chip peaks of this GPU for the roofline of the apply_H kernels (include/syk.h `syk_microbench`).
 
-    python -m paper_2311_00639_b200.microbench [--json]
+    python -m paper_2311_00639_b200.microbench [--json] [--quick]
+    python -m paper_2311_00639_b200.microbench --sweep       (streaming rate against the size of the source buffer)
 
 Prints a markdown table (or one JSON object): L2 -> SM and DRAM -> SM streaming rates of 148 persistent CTAs through the
 shared-memory ring of the scatter-tile kernel, the shared-memory read rate of its inner loop, both at once, and the issue
@@ -54,9 +55,36 @@ def measure(quick=False):
     return out
 
 
+def sweep():
+    """L2 / DRAM -> SM streaming rate (alone and with 1, 2 LDS passes per chunk) against the size of the buffer the 148 CTAs
+    walk through: where the working set leaves L2, and that multi-GB buffers (TLB reach) do not cost bandwidth."""
+    import torch
+    from . import binding as B
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    wk = torch.empty(B.syk_microbench_workspace_bytes(), dtype=torch.uint8, device="cuda")
+    free, _ = torch.cuda.mem_get_info()
+    print("| buffer | load only B/clk/SM (TB/s) | with 1 LDS pass | with 2 LDS passes |")
+    print("|---|---|---|---|")
+    for gb in (1 / 32, 1 / 16, 1 / 8, 1 / 4, 1, 8, 32, 64, 128):
+        n = int(gb * (1 << 30))
+        if n + (4 << 30) > free:
+            break
+        buf = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        B.syk_microbench(0, 2048, 0, buf, wk)
+        cells = []
+        for kind, terms in ((0, 0), (2, 1), (2, 2)):
+            r = B.syk_microbench(kind, 16384, terms, buf, wk)
+            cells.append(f"{r['units'] / sms / r['cycles']:.1f} ({r['units'] / (r['ms'] * 1e-3) / 1e12:.2f})")
+        print(f"| {gb * 1024:.0f} MiB | " + " | ".join(cells) + " |", flush=True)
+        del buf
+        torch.cuda.empty_cache()
+
+
 def main():
     import torch
     assert torch.cuda.is_available(), "needs a CUDA device"
+    if "--sweep" in sys.argv:
+        return sweep()
     res = measure(quick="--quick" in sys.argv)
     if "--json" in sys.argv:
         print(json.dumps(res))

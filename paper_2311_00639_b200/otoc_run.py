@@ -2,6 +2,7 @@
 
     python -m paper_2311_00639_b200.otoc_run --N 56 --k 4 --beta 5 --tmax 8 --nt 9 [--dtype c128|c64]
            [--krylov-dim 16] [--two-pass] [--tol 1e-10] [--block] [--green] [--seed 0] [--realization 0]
+           [--relabel] [--renormalize]
 
 Builds the sparse SYK Hamiltonian (Eq. 1), draws the Haar-random state on the device, runs syk_otoc
 (or, with --block, syk_otoc_block on both parity sectors of the same state and adds them) and prints one
@@ -32,6 +33,8 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="disorder realizations 0..batch-1 in lock step (syk_otoc_batched)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--realization", type=int, default=0)
+    ap.add_argument("--relabel", action="store_true", help="qubit layout chosen per Hamiltonian (syk_ham_optimize_layout)")
+    ap.add_argument("--renormalize", action="store_true", help="carry the norm separately (large beta in complex64)")
     args = ap.parse_args()
 
     import torch
@@ -43,7 +46,8 @@ def main():
     tdt = torch.complex128 if args.dtype == "c128" else torch.complex64
     code = B.SYK_C128 if args.dtype == "c128" else B.SYK_C64
     p = 1.0 if args.k == 0 else inputs.bernoulli_p(N, args.k)
-    opts = {"krylov_dim": args.krylov_dim, "two_pass": int(args.two_pass), "tol": args.tol}
+    opts = {"krylov_dim": args.krylov_dim, "two_pass": int(args.two_pass), "tol": args.tol,
+            "renormalize": int(args.renormalize)}
     t_grid = np.linspace(0.0, args.tmax, args.nt)
     iW, jV = N - 1, N - 2
 
@@ -57,8 +61,11 @@ def main():
     stats_tot = {"n_matvec": 0, "n_substeps": 0}
     torch.cuda.reset_peak_memory_stats()
     if not args.block:
+        if args.relabel:
+            B.syk_ham_optimize_layout(h, code)
+        B.syk_ham_prepare(h, code)
         psi = torch.empty(1 << L, dtype=tdt, device="cuda")
-        B.syk_random_state(N, args.seed, args.realization, psi, scratch)
+        B.syk_random_state_h(h, args.seed, args.realization, psi, scratch)
         wk = torch.empty(B.syk_otoc_workspace_bytes(h, code, opts), dtype=torch.uint8, device="cuda")
         torch.cuda.synchronize()
         t1 = time.perf_counter()
@@ -72,6 +79,9 @@ def main():
         # the two sector components of the random state are drawn directly as two independent normalised Gaussian
         # vectors with weight 1/2 each (the Haar ensemble up to O(D^-1/2) fluctuations of the sector weights)
         he, ho = B.syk_build_parity_block(h, 0), B.syk_build_parity_block(h, 1)
+        if args.relabel:                                       # one layout for both blocks (a gamma maps between them)
+            perm = B.syk_ham_optimize_layout(he, code)["perm"]
+            B.syk_ham_set_layout(ho, perm)
         half = 1 << (L - 1)
         ps = torch.empty(half, dtype=tdt, device="cuda")       # one sector at a time: N = 66 needs all of the memory
         wk = torch.empty(B.syk_otoc_workspace_bytes(he, code, opts), dtype=torch.uint8, device="cuda")
@@ -79,7 +89,7 @@ def main():
         t1 = time.perf_counter()
         F = 0
         for s in (0, 1):
-            B.syk_random_state(N - 2, args.seed, 2 * args.realization + s, ps, scratch)      # norm 1
+            B.syk_random_state_h(he, args.seed, 2 * args.realization + s, ps, scratch)      # norm 1
             if args.green:
                 Fs, st = B.syk_green_block(he, ho, s, iW, args.beta, t_grid, ps, wk, opts)
             else:
@@ -91,7 +101,7 @@ def main():
     t2 = time.perf_counter()
     ratio = F / F[0]
     out = {"what": "green" if args.green else "otoc", "N": N, "k": args.k, "beta": args.beta, "dtype": args.dtype,
-           "parity_blocks": args.block, "krylov_dim": args.krylov_dim, "two_pass": args.two_pass,
+           "parity_blocks": args.block, "relabelled": args.relabel, "krylov_dim": args.krylov_dim, "two_pass": args.two_pass,
            "n_terms": info["n_terms"], "n_xmasks": info["n_xmasks"], "t": t_grid.tolist(),
            "F_re": F.real.tolist(), "F_im": F.imag.tolist(), "ratio_re": ratio.real.tolist(),
            "seconds_setup": t1 - t0, "seconds_curve": t2 - t1, "seconds_per_point": (t2 - t1) / len(t_grid),

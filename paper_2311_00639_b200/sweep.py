@@ -1,6 +1,6 @@
 """Matvec bandwidth sweep of BASELINE.json configs[3] (SURVEY 8(d) "Sweep for config 4"), through the C ABI.
 
-    python -m paper_2311_00639_b200.sweep [--quick] > profiles/<round>_sweep.md
+    python -m paper_2311_00639_b200.sweep [--quick] [--relabel] > profiles/<round>_sweep.md
 
 Times plain `syk_apply_H` (CUDA events, 2 warm-up + 5 timed launches, minimum and median) for
   (i)   sparsity k in {1, 2, 4, 8, 16} at N = 56 complex128 -- PAPER.md:327 expects time ~ linear in k;
@@ -16,13 +16,16 @@ import sys
 import numpy as np
 
 
-def time_apply(B, torch, h, tdt, N, reps=5):
+def time_apply(B, torch, h, tdt, N, reps=5, relabel=False):
     D = 1 << (N // 2)
     code = B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64
+    if relabel:
+        B.syk_ham_optimize_layout(h, code)
+    B.syk_ham_prepare(h, code)
     scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
     a = torch.empty(D, dtype=tdt, device="cuda")
     b = torch.empty(D, dtype=tdt, device="cuda")
-    B.syk_random_state(N, 0, 0, a, scratch)
+    B.syk_random_state_h(h, 0, 0, a, scratch)
     for _ in range(2):
         B.syk_apply_H(h, a, b)
     torch.cuda.synchronize()
@@ -49,6 +52,7 @@ def time_apply(B, torch, h, tdt, N, reps=5):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--quick", action="store_true", help="N <= 48 only (a few seconds)")
+    ap.add_argument("--relabel", action="store_true", help="qubit layout chosen per Hamiltonian (syk_ham_optimize_layout)")
     ap.add_argument("--lockstep", action="store_true",
                     help="instead: sweep syk_set_lockstep(epoch, lag) for the two headline workloads and tile kernels")
     args = ap.parse_args()
@@ -62,7 +66,7 @@ def main():
     rows = []
 
     def run(label, N, h, tdt):
-        r = time_apply(B, torch, h, tdt, N)
+        r = time_apply(B, torch, h, tdt, N, relabel=args.relabel)
         rows.append((label, N, "c128" if tdt == torch.complex128 else "c64", r))
         print(f"# {label} N={N}: {r['ms_min']:.3f} ms", file=sys.stderr, flush=True)
 

@@ -1188,3 +1188,46 @@ def test_renormalize_evolve_and_otoc(B, torch, propagators, dt):
     if dt == "c64":                                          # without norm carrying the same call leaves the fp32 range
         Fplain, _ = B.syk_otoc(h, 0, 1, beta, t_grid, to_dev(torch, psi1), wk, o0)
         assert not np.all(np.isfinite(Fplain)) or np.max(np.abs(Fplain - refB)) / abs(refB[0]) > 1e-3
+
+
+def test_cuda_graph_latency_path(B, torch):
+    """The Krylov driver replays one captured CUDA graph per Lanczos round for small vectors (syk_set_cuda_graphs): bitwise
+    the same results as direct launches (one-pass, two-pass, OTOC over several buffers and handles), same kernel count,
+    and the graph survives a change of layout / kernel choice of the handle (new key)."""
+    N = 16
+    D = 256
+    q, J = couplings(N, None)
+    psi = inputs.gaussian_state(D, 4)
+    t_grid = np.array([0.0, 0.5, 1.5, 3.0])
+    outs = {}
+    for on in (1, 0, 1):
+        B.syk_set_cuda_graphs(on)
+        try:
+            h = B.syk_build_from_terms(N, q, J)
+            res = []
+            for o in ({"krylov_dim": 12}, {"krylov_dim": 7, "two_pass": 1}):
+                wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+                d = to_dev(torch, psi)
+                B.syk_launch_count(reset=True)
+                st = B.syk_krylov_evolve(h, d, 3.0, -1.0, wk, o)
+                n_k = B.syk_launch_count(reset=True)
+                res.append((d.cpu().numpy().copy(), st["n_matvec"], st["n_substeps"], n_k))
+                F, _ = B.syk_otoc(h, 0, 1, 5.0, t_grid, to_dev(torch, psi), wk, o)
+                res.append(F.copy())
+                B.syk_set_apply_H_kernel(h, 0)                       # another kernel for the same handle: a new graph
+                d2 = to_dev(torch, psi)
+                B.syk_krylov_evolve(h, d2, 3.0, -1.0, wk, o)
+                B.syk_set_apply_H_kernel(h, -1)
+                res.append(d2.cpu().numpy().copy())
+            outs.setdefault(on, []).append(res)
+        finally:
+            B.syk_set_cuda_graphs(1)
+    ref = outs[0][0]
+    for res in outs[1]:
+        for a, b in zip(res, ref):
+            if isinstance(a, tuple):
+                assert np.array_equal(a[0], b[0]) and a[1:] == b[1:]
+            else:
+                assert np.array_equal(a, b)
+    prop = oev.ExactPropagator(N, q, J)
+    assert relerr(ref[0][0], prop.apply(3.0 - 1.0j, psi)) <= 1e-10
