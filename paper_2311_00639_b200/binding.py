@@ -565,11 +565,12 @@ def syk_microbench_workspace_bytes():
 
 def syk_microbench(kind, arg0, arg1, d_buf, d_work, stream=None):
     """One on-chip peak measurement (include/syk.h); returns {"ms", "cycles", "units", "lds_bytes"}."""
-    res = (ctypes.c_double * 4)()
+    res = (ctypes.c_double * 6)()
     nb = 0 if d_buf is None else d_buf.numel() * d_buf.element_size()
     _check(_lib.syk_microbench(int(kind), int(arg0), int(arg1), 0 if d_buf is None else _dptr(d_buf), nb, _dptr(d_work),
                                d_work.numel() * d_work.element_size(), res, _stream(stream)), "syk_microbench")
-    return {"ms": res[0], "cycles": res[1], "units": res[2], "lds_bytes": res[3]}
+    return {"ms": res[0], "cycles": res[1], "units": res[2], "lds_bytes": res[3], "cycles_even": res[4],
+            "cycles_odd": res[5]}
 
 
 def syk_version():

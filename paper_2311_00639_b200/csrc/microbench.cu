@@ -31,6 +31,9 @@ struct MbParams {
     int n_chunks;                 // chunks streamed per CTA
     int terms_per_chunk;          // LDS passes over every staged chunk
     int load;                     // 0: the producer only signals, nothing is copied
+    int small_log2;               // > 0: odd CTAs walk only the first 2^small_log2 bytes (an L2-resident region) and stream
+                                  // `small_mult` times as many chunks, even CTAs walk the whole buffer (kind 5)
+    int small_mult;
     double2* sink;                // [grid * 256]
     unsigned long long* cycles;   // [grid]
 };
@@ -50,7 +53,9 @@ __global__ void __launch_bounds__(kMbThreads, 1) mb_stream_kernel(const MbParams
     for (uint32_t i = (uint32_t)tid; i < kMbRing * kMbChunk / 16u; i += kMbThreads)
         reinterpret_cast<uint4*>(smem)[i] = make_uint4(0u, 0u, 0u, 0u);   // defined values when nothing is copied
     __syncthreads();
-    const uint64_t mask = ((uint64_t)1 << p.buf_log2) - 1;
+    const bool small_grp = p.small_log2 > 0 && (blockIdx.x & 1);
+    const uint64_t mask = ((uint64_t)1 << (small_grp ? p.small_log2 : p.buf_log2)) - 1;
+    const int n_chunks = small_grp ? p.n_chunks * p.small_mult : p.n_chunks;
     if (warp >= kMbConsumerWarps) {
         if (warp != kMbConsumerWarps || lane != 0) return;
         int pos = 0;
@@ -58,7 +63,7 @@ __global__ void __launch_bounds__(kMbThreads, 1) mb_stream_kernel(const MbParams
         const uint32_t stage0 = smem_u32(smem);
         // every CTA walks its own sequence of 64 KiB chunks through the buffer (odd multiplier: all chunks are visited)
         uint64_t at = ((uint64_t)blockIdx.x * 0x9E3779B1ull) * kMbChunk;
-        for (int c = 0; c < p.n_chunks; ++c) {
+        for (int c = 0; c < n_chunks; ++c) {
             mbar_wait(bar_empty + 8 * pos, phase ^ 1u);
             if (p.load) {
                 mbar_arrive_expect_tx(bar_full + 8 * pos, kMbChunk);
@@ -84,7 +89,7 @@ __global__ void __launch_bounds__(kMbThreads, 1) mb_stream_kernel(const MbParams
             ai[r] = 0.0;
         }
         const unsigned long long t0 = clock64();
-        for (int c = 0; c < p.n_chunks; ++c) {
+        for (int c = 0; c < n_chunks; ++c) {
             mbar_wait(bar_full + 8 * pos, phase);
             const unsigned char* cp = smem + (size_t)pos * kMbChunk;
             for (int t = 0; t < p.terms_per_chunk; ++t) {
@@ -189,8 +194,11 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
     SYK_CUDA(cudaEventCreate(&e1));
     double units = 0.0, units2 = 0.0;
     int rc = SYK_OK;
-    if (kind >= 0 && kind <= 2) {
+    double cyc_even = 0.0, cyc_odd = 0.0;
+    if ((kind >= 0 && kind <= 2) || kind == 5) {
         // 0: loads only; 1: LDS + FMA only; 2: both.  arg0 = chunks per CTA, arg1 = terms per chunk
+        // 5: loads only, two groups: even CTAs walk the whole buffer (DRAM), odd CTAs its first 32 MB (L2) with arg1 times
+        //    as many chunks
         int buf_log2 = 0;
         while (((size_t)2 << buf_log2) <= buf_bytes) ++buf_log2;
         if (kind != 1 && (!d_buf || buf_log2 < 17 || ((uintptr_t)d_buf & 127))) rc = SYK_EINVAL;
@@ -200,8 +208,10 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
             p.buf = (const unsigned char*)d_buf;
             p.buf_log2 = buf_log2;
             p.n_chunks = arg0;
-            p.terms_per_chunk = kind == 0 ? 0 : arg1;
+            p.terms_per_chunk = (kind == 0 || kind == 5) ? 0 : arg1;
             p.load = kind != 1;
+            p.small_log2 = kind == 5 ? 25 : 0;
+            p.small_mult = kind == 5 ? (arg1 > 0 ? arg1 : 1) : 1;
             p.sink = (double2*)d_sink;
             p.cycles = d_cycles;
             const size_t smem = (size_t)kMbRing * kMbChunk + 2 * kMbRing * 8 + 64;
@@ -218,6 +228,10 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
             }
             units = p.load ? (double)sms * arg0 * (double)kMbChunk : 0.0;                       // bytes L2/DRAM -> smem
             units2 = (double)sms * arg0 * (double)p.terms_per_chunk * (double)kMbChunk;         // bytes read by LDS
+            if (kind == 5) {   // bytes of the even (whole buffer) and of the odd (L2-resident region) group
+                units = (double)((sms + 1) / 2) * arg0 * (double)kMbChunk;
+                units2 = (double)(sms / 2) * arg0 * (double)p.small_mult * (double)kMbChunk;
+            }
             count_launch();
         }
     } else if (kind == 3 || kind == 4) {
@@ -248,10 +262,16 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
             rc = SYK_ECUDA;
         } else {
             const unsigned long long cmax = *std::max_element(cyc.begin(), cyc.end());
+            for (int i = 0; i < sms; ++i) {
+                double& dst = (i & 1) ? cyc_odd : cyc_even;
+                dst = std::max(dst, (double)cyc[(size_t)i]);
+            }
             result[0] = ms;
             result[1] = (double)cmax;
             result[2] = units;
             result[3] = units2;
+            result[4] = cyc_even;
+            result[5] = cyc_odd;
         }
     }
     cudaEventDestroy(e0);

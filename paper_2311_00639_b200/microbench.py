@@ -45,6 +45,16 @@ def measure(quick=False):
         big = torch.zeros(big_bytes, dtype=torch.uint8, device="cuda")
         out["dram_to_sm"] = stream(0, n, 0, big)
         out["dram_and_lds_2"] = stream(2, n // 2, 2, big)
+        # do the two supplies overlap?  74 CTAs stream from DRAM while 74 stream from an L2-resident region
+        for mult in (1, 3):
+            B.syk_microbench(5, n // 16, mult, big, wk)
+            r = B.syk_microbench(5, n // 2, mult, big, wk)
+            out[f"dram_half_and_l2_half_x{mult}"] = {
+                "ms": r["ms"], "cycles": r["cycles"], "sm_mhz_effective": r["cycles"] / (r["ms"] * 1e-3) / 1e6,
+                "dram_group_TB_per_s": r["units"] / r["cycles_even"] * (r["cycles"] / (r["ms"] * 1e-3)) / 1e12,
+                "l2_group_TB_per_s": r["lds_bytes"] / r["cycles_odd"] * (r["cycles"] / (r["ms"] * 1e-3)) / 1e12,
+                "dram_group_B_per_clk_per_SM": r["units"] / ((sms + 1) // 2) / r["cycles_even"],
+                "l2_group_B_per_clk_per_SM": r["lds_bytes"] / (sms // 2) / r["cycles_odd"]}
         del big
     iters = 4000 if quick else 20000
     for name, kind in (("fp64_add", 3), ("dense_term_sequence", 4)):
@@ -93,6 +103,10 @@ def main():
     print("|---|---|---|---|---|---|---|---|")
     for k, v in res.items():
         if not isinstance(v, dict):
+            continue
+        if "dram_group_TB_per_s" in v:
+            print(f"| {k} | {v['ms']:.3f} | DRAM half: {v['dram_group_B_per_clk_per_SM']:.1f} | {v['dram_group_TB_per_s']:.2f} | "
+                  f"L2 half: {v['l2_group_B_per_clk_per_SM']:.1f} (load) | {v['l2_group_TB_per_s']:.2f} |  | {v['sm_mhz_effective']:.0f} |")
             continue
         f = lambda key, fmt: (fmt % v[key]) if key in v else ""
         print(f"| {k} | {v['ms']:.3f} | {f('load_B_per_clk_per_SM', '%.1f')} | {f('load_TB_per_s', '%.2f')} | "
