@@ -36,7 +36,7 @@
 // reproducible.  ~100 warp instructions per (term, chunk of 16 slices) instead of ~150 with a per-slice sign walk; what
 // the launch is bound by is the supply of tiles (DRAM phases and L2 phases of the lock-stepped CTAs do not overlap; L2
 // prefetching by the TMA unit or by prefetch.global.L2, of every load or only of the loads that must miss, 1..12 loads
-// ahead, made every configuration slower: profiles/r2_apply_h_experiments.md).
+// ahead, made every configuration slower: DESIGN.md section 6).
 //
 // Fused Lanczos epilogue (a-3 part 1) as in apply_h.cu: out = acc/|u_j| - (|u_j|/|u_{j-1}|) prev, per-CTA fp64
 // partial sums of Re<in|out>.  The tile of `in` and of `prev` are staged through the same ring after the last

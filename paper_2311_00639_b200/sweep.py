@@ -6,7 +6,8 @@ Times plain `syk_apply_H` (CUDA events, 2 warm-up + 5 timed launches, minimum an
   (i)   sparsity k in {1, 2, 4, 8, 16} at N = 56 complex128 -- PAPER.md:327 expects time ~ linear in k;
   (ii)  structured mask sets of equal size at N = 56: all X bits below bit 5 (warp-local), below bit 11
         (tile-local: no second source tile), only above bit 22 (every mask is a separate DRAM stream);
-  (iii) N = 40 .. 56 at k = 4 (where the vector leaves L2), and N = 64 complex64 at k in {1, 2, 4}.
+  (iii) N = 40 .. 56 at k = 4 (where the vector leaves L2), and N = 64 complex64 at k in {1, 2, 4};
+  (iv)  pure regimes with one term per load (Hamming-code mask sets): all loads L2 hits, all loads DRAM passes, mixtures.
 and prints one markdown table.  "model GB/s" = (D_x + 2) V / time; loads / passes are the
 tile layout the kernel chose (syk_apply_H_layout).  Argument marshalling only: every number is a kernel time.
 """
@@ -65,8 +66,8 @@ def main():
         return lockstep_sweep(B, torch, inputs, args.quick)
     rows = []
 
-    def run(label, N, h, tdt):
-        r = time_apply(B, torch, h, tdt, N, relabel=args.relabel)
+    def run(label, N, h, tdt, relabel=None):
+        r = time_apply(B, torch, h, tdt, N, relabel=args.relabel if relabel is None else relabel)
         rows.append((label, N, "c128" if tdt == torch.complex128 else "c64", r))
         print(f"# {label} N={N}: {r['ms_min']:.3f} ms", file=sys.stderr, flush=True)
 
@@ -83,6 +84,21 @@ def main():
     if not args.quick:
         for k in (1, 2, 4):
             run(f"(iii) k={k}", 64, B.syk_build_hamiltonian(64, inputs.bernoulli_p(64, k), 0, 0), c64)
+    # (iv) pure regimes of the tile kernel with ONE term per load: X strings whose masks are the 15 non-zero words of the
+    # Hamming(7,4) code on a 7-bit field (any two differ in >= 3 bits, so the kernel's 2 free tile bits cannot merge loads):
+    # field inside the L2 window -> every load after the first hits in L2; field on the top bits -> every load is a DRAM pass;
+    # products of the two -> runs of 15 (or 4) loads per DRAM pass
+    G = (0b1000110, 0b0100101, 0b0010011, 0b0001111)
+    code = sorted({(a * G[0]) ^ (b * G[1]) ^ (c * G[2]) ^ (d * G[3]) for a in (0, 1) for b in (0, 1) for c in (0, 1)
+                   for d in (0, 1)} - {0})
+    lo, hi = 13, L - 7
+    for name, terms in (("15 masks in the window", [(w << lo, 0, 0.01) for w in code]),
+                        ("15 masks on the top bits", [(w << hi, 0, 0.01) for w in code]),
+                        ("15 window x 4 top", [((w1 << lo) | (w2 << hi), 0, 0.01) for w1 in code for w2 in code[:4]]),
+                        ("15 window x 15 top", [((w1 << lo) | (w2 << hi), 0, 0.01) for w1 in code for w2 in code])):
+        h = B.syk_build_from_pauli_strings(L, terms)
+        B.syk_set_apply_H_kernel(h, 3)
+        run(f"(iv) {name}", Nbig, h, c128, relabel=False)   # canonical layout: the fields are placed for it
 
     print("| case | N | dtype | T | D_x | kernel | loads | passes | ms (min) | ms (median) | model GB/s | ms per X-mask |")
     print("|---|---|---|---|---|---|---|---|---|---|---|---|")

@@ -506,3 +506,35 @@ def test_P16_complex_syk_hamiltonian():
     assert np.allclose(Hc, sum(Jt * M for Jt, M in zip(Jc, [hamiltonian.dense_hamiltonian(N, [qq], [1.0]) for qq in q])), atol=1e-14)
     Hi = onh.complex_syk_hamiltonian(N, q, 1j * J)
     assert np.allclose(Hi, -Hi.conj().T, atol=1e-15)
+
+
+def test_paper_statements_fixture_is_what_the_oracle_uses():
+    """tests/golden/paper_statements.txt lists values the paper prints, each with its PAPER.md line.  The ones that are
+    numbers or tables are read here and compared with what the oracle computes with: the <bits> encoding of the four site
+    operators against oracle/alg1.py, the coupling variance 3/(8 p N^3) against the sample
+    variance of oracle/rng.py's couplings, k = (p/N) C(N,4) against the mean number of kept terms, and the two Clifford
+    normalisations against the Kronecker-built gammas."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_statements.txt")
+    stm = {}
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        key, rest = line.split("=", 1)
+        value, cite = rest.rsplit(";", 1)
+        assert "PAPER.md:" in cite, line
+        stm[key.strip()] = value.strip()
+    enc = dict(tok.split("=") for tok in stm["encoding"].split())
+    assert {int(k[1]): int(v, 2) for k, v in enc.items()} == alg1._CODE
+    assert stm["coupling_variance"].replace(" ", "") == "3/(8pN^3)"
+    N, k = 24, 6.0
+    p = k * N / math.comb(N, 4)
+    Js = np.concatenate([rng.sample_couplings(N, p, 11, r)[1] for r in range(400)])
+    var = eval(stm["coupling_variance"].replace("^", "**").replace("8 p N", "8*p*N"), {"p": p, "N": N})
+    assert abs(np.var(Js) / var - 1.0) < 0.03
+    assert stm["sparsity"].replace(" ", "") == "k=(p/N)C(N,4)"
+    assert abs(len(Js) / 400.0 - (p / N) * math.comb(N, 4) * N) < 0.05 * k * N          # mean kept terms = k N
+    for key, gn, scale in (("clifford_main_text", majorana.GAMMA_HALF, 1.0), ("clifford_supplement", majorana.GAMMA_PAULI, 2.0)):
+        assert ("2 delta" in stm[key]) == (scale == 2.0)
+        g = majorana.jw_gammas(6, gn)
+        assert np.allclose(g[1] @ g[1] + g[1] @ g[1], scale * np.eye(8)) and np.allclose(g[0] @ g[3] + g[3] @ g[0], 0)
