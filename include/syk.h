@@ -18,7 +18,8 @@
  *     <= ~8 MB for dense N=48) and, for the dense-table kernel on vectors with fewer tiles than SMs, a scratch
  *     buffer of partial sums (<= 64 vectors of <= 2^19 amplitudes).  syk_ham_prepare allocates and uploads all
  *     of it; after that no compute call allocates.  A handle that was not prepared does the same lazily inside
- *     its first compute call (one synchronous cudaMalloc + copy).
+ *     its first compute call (one synchronous cudaMalloc + copy).  (The CUDA graphs of the latency path for small
+ *     vectors, syk_set_cuda_graphs, are instantiated by the driver on first use, which may take device memory of its own.)
  *   - A handle is not thread-safe and must not be used by two launches that are in flight at the same time
  *     (different streams or threads): the lazily built table caches, the split scratch and the pacing counters
  *     of the tile kernels belong to the handle.  Different handles are independent.

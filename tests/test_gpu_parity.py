@@ -1231,3 +1231,49 @@ def test_cuda_graph_latency_path(B, torch):
                 assert np.array_equal(a, b)
     prop = oev.ExactPropagator(N, q, J)
     assert relerr(ref[0][0], prop.apply(3.0 - 1.0j, psi)) <= 1e-10
+
+
+def test_no_device_allocation_after_prepare(B, torch):
+    """include/syk.h: after syk_ham_prepare no compute call on the handle allocates device memory (the
+    memory discipline is part of the method).  cudaMemGetInfo (which sees the library's own cudaMalloc calls) must not move
+    across apply_H / Lanczos / Krylov / OTOC calls, for a sparse handle (tile kernels), a dense handle in the split form of
+    the dense-table kernel (scratch of partial sums) and a relabelled handle; an UNPREPARED dense handle does allocate in
+    its first call, which is what the check is able to see.  (CUDA graphs of the latency path off: instantiating a graph
+    is the driver's allocation.)"""
+    B.syk_set_cuda_graphs(0)
+    try:
+        N = 28
+        D = 1 << (N // 2)
+        o = {"krylov_dim": 6}
+        psi = inputs.gaussian_state(D, 3)
+        cases = []
+        q, J = couplings(N, 4, seed=3)
+        cases.append(("sparse", B.syk_build_from_terms(N, q, J)))
+        hr = B.syk_build_from_terms(N, q, J)
+        B.syk_ham_set_layout(hr, list(range(N // 2 - 1, -1, -1)))
+        cases.append(("relabelled", hr))
+        qd, Jd = couplings(N, None, seed=3)
+        cases.append(("dense", B.syk_build_from_terms(N, qd, Jd)))
+        for name, h in cases:
+            wk = work(torch, B.syk_otoc_workspace_bytes(h, B.SYK_C128, o))
+            d_in, d_out = to_dev(torch, psi), torch.empty(D, dtype=torch.complex128, device="cuda")
+            B.syk_ham_prepare(h, B.SYK_C128)
+            if name == "dense":
+                assert B.syk_apply_H_kernel_kind(h, B.SYK_C128) == 4 and B.syk_apply_H_dense_info(h, B.SYK_C128)["split"] > 1
+            torch.cuda.synchronize()
+            free0 = torch.cuda.mem_get_info()[0]
+            B.syk_apply_H(h, d_in, d_out)
+            B.syk_lanczos_run(h, d_in, 4, wk)
+            B.syk_krylov_evolve(h, d_in, 0.3, -0.1, wk, o)
+            B.syk_otoc(h, 0, 1, 1.0, [0.0, 0.2], d_in, wk, o)
+            torch.cuda.synchronize()
+            assert torch.cuda.mem_get_info()[0] == free0, name
+        hd = B.syk_build_from_terms(N, qd, Jd)                      # not prepared: the first call creates the tables + scratch
+        d_in, d_out = to_dev(torch, psi), torch.empty(D, dtype=torch.complex128, device="cuda")
+        torch.cuda.synchronize()
+        free0 = torch.cuda.mem_get_info()[0]
+        B.syk_apply_H(hd, d_in, d_out)
+        torch.cuda.synchronize()
+        assert torch.cuda.mem_get_info()[0] < free0
+    finally:
+        B.syk_set_cuda_graphs(1)
