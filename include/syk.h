@@ -290,6 +290,12 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
                      const double* t_grid, int n_t, void* d_psi, int64_t batch_stride, double* F_out,
                      const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats, void* stream);
 
+/* The Green function of gamma_n for a batch of realizations, same two modes, buffers and work-space query
+ * (syk_otoc_batched_workspace_bytes) as syk_otoc_batched; G_out[r][n_t][2]. */
+int syk_green_batched(const syk_ham* const* hams, int n_batch, int dtype, int n, double beta, const double* t_grid, int n_t,
+                      void* d_psi, int64_t batch_stride, double* G_out, const syk_krylov_opts* opts, void* d_work,
+                      size_t work_bytes, syk_stats* stats, void* stream);
+
 /* ------------------------------------------------------------------------------------------------------------
  * Introspection for tests and the benchmark. */
 /* Which apply_H kernel a handle would use for `dtype`: 0 = generic gather, 1 = TMA-pipelined 16 KiB-tile gather,

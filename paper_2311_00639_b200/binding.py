@@ -96,6 +96,8 @@ _SIGNATURES = {
     "syk_otoc_batched_workspace_bytes": (_i, [_vp, _i, _i, _P(syk_krylov_opts), _P(_sz)]),
     "syk_otoc_batched": (_i, [_P(_vp), _i, _i, _i, _i, _d, _vp, _i, _vp, _i64, _vp, _P(syk_krylov_opts), _vp, _sz,
                               _P(syk_stats), _vp]),
+    "syk_green_batched": (_i, [_P(_vp), _i, _i, _i, _d, _vp, _i, _vp, _i64, _vp, _P(syk_krylov_opts), _vp, _sz,
+                               _P(syk_stats), _vp]),
     "syk_apply_H_kernel_kind": (_i, [_vp, _i]),
     "syk_set_apply_H_kernel": (_i, [_vp, _i]),
     "syk_set_lockstep": (_i, [_i, _i]),
@@ -518,6 +520,18 @@ def syk_otoc_batched(hams, i_W, j_V, beta, t_grid, d_psi, batch_stride, d_work, 
                                  d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
            "syk_otoc_batched")
     return F[..., 0] + 1j * F[..., 1], st.as_dict()
+
+
+def syk_green_batched(hams, n, beta, t_grid, d_psi, batch_stride, d_work, opts=None, stream=None):
+    t = np.ascontiguousarray(t_grid, dtype=np.float64)
+    G = np.zeros((len(hams), len(t), 2), dtype=np.float64)
+    arr = (ctypes.c_void_p * len(hams))(*[_h(h).value for h in hams])
+    st = syk_stats()
+    _check(_lib.syk_green_batched(arr, len(hams), dtype_code(d_psi), int(n), float(beta), t.ctypes.data, len(t),
+                                  _dptr(d_psi), int(batch_stride), G.ctypes.data, _opts(opts), _dptr(d_work),
+                                  d_work.numel() * d_work.element_size(), ctypes.byref(st), _stream(stream)),
+           "syk_green_batched")
+    return G[..., 0] + 1j * G[..., 1], st.as_dict()
 
 
 # ---- introspection -------------------------------------------------------------------------------------------

@@ -164,10 +164,12 @@ static size_t otoc_batched_bytes(const syk_ham* h0, int nb, int dtype, const syk
     return 2 * (size_t)nb * v + krylov_batched_bytes(h0, nb, dtype, resolve_krylov_dim(h0, opts));
 }
 
+// green = true: the Green function of gamma_{i_W} (j_V unused), same buffers: l = E(-ib/2) psi, phi = g l, per grid point both
+// advance by E(dt) and G = <l | g phi>
 static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int i_W, int j_V, double beta,
                              const double* t_grid, int n_t, void* d_psi, size_t psi_stride, double* F_out,
                              const syk_krylov_opts* opts, void* d_work, size_t work_bytes, syk_stats* stats,
-                             cudaStream_t st) {
+                             cudaStream_t st, bool green = false) {
     const syk_ham* h0 = hams[0];
     const uint64_t D = 1ull << h0->L;
     const size_t v = (size_t)D * elem_bytes(dtype);
@@ -203,9 +205,14 @@ static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int 
         return launch_gamma_h(h0, n, dtype, in, out, st, b);   // one layout for the whole batch (batched_apply_ok)
     };
     std::vector<double> dots((size_t)2 * nb);
-    SYK_TRY(evolve(l, psi_stride, 0.0, -beta / 8.0));
-    SYK_TRY(gamma(j_V, l, psi_stride, phi, v));
-    SYK_TRY(evolve(phi, v, 0.0, -beta / 4.0));
+    if (green) {
+        SYK_TRY(evolve(l, psi_stride, 0.0, -beta / 2.0));
+        SYK_TRY(gamma(i_W, l, psi_stride, phi, v));
+    } else {
+        SYK_TRY(evolve(l, psi_stride, 0.0, -beta / 8.0));
+        SYK_TRY(gamma(j_V, l, psi_stride, phi, v));
+        SYK_TRY(evolve(phi, v, 0.0, -beta / 4.0));
+    }
     double t_prev = 0.0;
     for (int k = 0; k < n_t; ++k) {
         const double t = t_grid[k], dt = t - t_prev;
@@ -215,10 +222,12 @@ static int otoc_batched_impl(const syk_ham* const* hams, int nb, int dtype, int 
         }
         t_prev = t;
         SYK_TRY(gamma(i_W, phi, v, r, v));
-        SYK_TRY(evolve(r, v, -t, -beta / 4.0));
-        SYK_TRY(gamma(j_V, r, v, r, v));
-        SYK_TRY(evolve(r, v, t, -beta / 4.0));
-        SYK_TRY(gamma(i_W, r, v, r, v));
+        if (!green) {
+            SYK_TRY(evolve(r, v, -t, -beta / 4.0));
+            SYK_TRY(gamma(j_V, r, v, r, v));
+            SYK_TRY(evolve(r, v, t, -beta / 4.0));
+            SYK_TRY(gamma(i_W, r, v, r, v));
+        }
         Batch b;
         b.n = nb;
         b.s.a = psi_stride;
@@ -348,6 +357,39 @@ int syk_otoc_batched(const syk_ham* const* hams, int n_batch, int dtype, int i_W
             return SYK_EINVAL;
         int rc = syk::otoc_one(syk::full_space(hams[r]), dtype, i_W, j_V, beta, t_grid, n_t, psi, F_out + (size_t)r * 2 * n_t, opts,
                                d_work, work_bytes, stats, (cudaStream_t)stream);
+        if (rc == SYK_ENOCONV) rc_soft = rc;
+        else if (rc != SYK_OK) return rc;
+    }
+    return rc_soft;
+}
+
+int syk_green_batched(const syk_ham* const* hams, int n_batch, int dtype, int n, double beta, const double* t_grid, int n_t,
+                      void* d_psi, int64_t batch_stride, double* G_out, const syk_krylov_opts* opts, void* d_work,
+                      size_t work_bytes, syk_stats* stats, void* stream) {
+    if (!hams || n_batch < 1 || !hams[0]) return SYK_EINVAL;
+    if (stats) *stats = syk_stats{};
+    const int other = n == 0 ? 1 : 0;   // otoc_args_ok wants two different operator indices
+    const bool lockstep = n_batch >= 2 && !(opts && (opts->two_pass || opts->renormalize)) &&
+                          syk::batched_apply_ok(hams, n_batch, dtype) &&
+                          work_bytes >= syk::otoc_batched_bytes(hams[0], n_batch, dtype, opts);
+    for (int r = 0; r < n_batch; ++r) {
+        if (!hams[r] || hams[r]->N != hams[0]->N || hams[r]->block_of_N || batch_stride < ((int64_t)1 << hams[r]->L) ||
+            n < 0 || n >= hams[r]->N)
+            return SYK_EINVAL;
+        char* psi = (char*)d_psi + (size_t)r * (size_t)batch_stride * syk::elem_bytes(dtype);
+        if (!syk::otoc_args_ok(hams[r], dtype, n, other, beta, t_grid, n_t, psi, G_out, d_work)) return SYK_EINVAL;
+    }
+    if (lockstep) {
+        if (((size_t)batch_stride * syk::elem_bytes(dtype)) % 16) return SYK_EINVAL;
+        return syk::otoc_batched_impl(hams, n_batch, dtype, n, other, beta, t_grid, n_t, d_psi,
+                                      (size_t)batch_stride * syk::elem_bytes(dtype), G_out, opts, d_work, work_bytes, stats,
+                                      (cudaStream_t)stream, true);
+    }
+    int rc_soft = SYK_OK;
+    for (int r = 0; r < n_batch; ++r) {
+        char* psi = (char*)d_psi + (size_t)r * (size_t)batch_stride * syk::elem_bytes(dtype);
+        int rc = syk::green_one(syk::full_space(hams[r]), dtype, n, beta, t_grid, n_t, psi, G_out + (size_t)r * 2 * n_t, opts,
+                                d_work, work_bytes, stats, (cudaStream_t)stream);
         if (rc == SYK_ENOCONV) rc_soft = rc;
         else if (rc != SYK_OK) return rc;
     }

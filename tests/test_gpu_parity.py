@@ -1277,3 +1277,31 @@ def test_no_device_allocation_after_prepare(B, torch):
         assert torch.cuda.mem_get_info()[0] < free0
     finally:
         B.syk_set_cuda_graphs(1)
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_green_batched_vs_oracle(B, torch, dt):
+    """syk_green_batched in lock-step mode and back to back: each realization against its own oracle."""
+    N, nb = 24, 3
+    D = 1 << (N // 2)
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    p = inputs.bernoulli_p(N, 4)
+    t_grid = np.array([0.0, 0.7, 2.0])
+    hams = [B.syk_build_hamiltonian(N, p, 3, r) for r in range(nb)]
+    psis = np.stack([orng.random_state(N, 3, r) for r in range(nb)]).astype(npdtype(dt))
+    o = {"krylov_dim": 14}
+    wk = work(torch, B.syk_otoc_batched_workspace_bytes(hams[0], nb, code, o))
+    B.syk_launch_count(reset=True)
+    G, _ = B.syk_green_batched(hams, 5, 3.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk, o)
+    n_lock = B.syk_launch_count(reset=True)
+    wk1 = work(torch, B.syk_otoc_workspace_bytes(hams[0], code, o))
+    G1, _ = B.syk_green_batched(hams, 5, 3.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk1, o)
+    n_seq = B.syk_launch_count(reset=True)
+    assert n_lock * 2 < n_seq
+    for r in range(nb):
+        q, J, _ = orng.sample_couplings(N, p, 3, r)
+        ref = ogreen.green_same_psi(oev.ExactPropagator(N, q, J), N, 5, 3.0, t_grid, psis[r].astype(np.complex128))
+        assert np.max(np.abs(G[r] - ref)) / abs(ref[0]) <= TOL[dt], r
+        assert np.max(np.abs(G1[r] - ref)) / abs(ref[0]) <= TOL[dt], r
+    with pytest.raises(B.SykError):
+        B.syk_green_batched(hams, N, 3.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk, o)
