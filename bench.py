@@ -16,7 +16,7 @@ alone, timed with CUDA events around each of its launches inside the timed regio
 
 The default run times BASELINE.json's first headline config (N=56, k=4, complex128) as the JSON line itself and then its
 second one (N=64, k=2, complex64, two-pass Lanczos) for 3 steps, embedded under `second_headline` (skipped with a stated
-reason when less than 175 GB of device memory is free).  On-chip peaks (L2 -> SM, shared-memory reads, DRAM -> SM through
+reason when less than 140 GB of device memory is free).  On-chip peaks (L2 -> SM, shared-memory reads, DRAM -> SM through
 the TMA ring) are measured in the same run with `syk_microbench` and the roofline reports one fraction per unit.
 
 N > 1 (torchrun): realizations are independent, so each rank runs its own realization with no
@@ -565,12 +565,13 @@ def run_ours(args, wl, name):
     if name == "N56_k4_c128" and not args.no_second:
         name2 = "N64_k2_c64"
         free, _ = torch.cuda.mem_get_info()
-        ok = torch.tensor([1 if free >= 175 * 2 ** 30 else 0], device="cuda")
+        need = 4 * (8 << 32) + (2 << 30)          # l, r and two Krylov work vectors of 2^32 complex64 amplitudes + headers
+        ok = torch.tensor([1 if free >= need else 0], device="cuda")
         if world > 1:
             dist.all_reduce(ok, op=dist.ReduceOp.MIN)
         if int(ok[0]) == 0:
-            second = {"workload": name2, "skipped": "needs 175 GB of free device memory (5 vectors of 34.4 GB); free: %.1f GB"
-                      % (free / 2 ** 30)}
+            second = {"workload": name2, "skipped": "needs %.0f GB of free device memory (4 resident vectors of 34.4 GB); free: %.1f GB"
+                      % (need / 1e9, free / 1e9)}
         else:
             l2 = measure_workload(args, WORKLOADS[name2], name2, 3, 1, world, rank, local, dist, False, False, peaks)
             if l2 is not None:
