@@ -63,7 +63,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep needs a CUDA device: the library has no CPU path")
     if args.lockstep:
-        return lockstep_sweep(B, torch, inputs, args.quick)
+        return lockstep_sweep(B, torch, inputs, args.quick, args.relabel)
     rows = []
 
     def run(label, N, h, tdt, relabel=None):
@@ -114,7 +114,7 @@ def main():
         print(f"\nAffine fit of (i): time = {icpt:.3f} ms + {slope:.4f} ms x D_x, worst relative residual {resid:.3f}")
 
 
-def lockstep_sweep(B, torch, inputs, quick):
+def lockstep_sweep(B, torch, inputs, quick, relabel=False):
     """Pacing of the persistent CTAs (syk_set_lockstep): plain syk_apply_H, minimum of 3 launches in ms, for the
     register-tile (kind 2) and scatter-tile (kind 3) kernels; outputs are checked to be bitwise equal across settings."""
     settings = [(0, 0), (1, 1), (2, 1), (2, 2), (4, 1), (4, 2), (8, 1), (8, 2), (16, 1), (32, 1)]
@@ -125,10 +125,12 @@ def lockstep_sweep(B, torch, inputs, quick):
         for N, k, tdt in cases:
             D = 1 << (N // 2)
             h = B.syk_build_hamiltonian(N, inputs.bernoulli_p(N, k), 0, 0)
+            if relabel:
+                B.syk_ham_optimize_layout(h, B.SYK_C128 if tdt == torch.complex128 else B.SYK_C64)
             scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
             a = torch.empty(D, dtype=tdt, device="cuda")
             b = torch.empty(D, dtype=tdt, device="cuda")
-            B.syk_random_state(N, 0, 0, a, scratch)
+            B.syk_random_state_h(h, 0, 0, a, scratch)
             for kind in (2, 3):
                 B.syk_set_apply_H_kernel(h, kind)
                 cells, ref = [], None
