@@ -27,7 +27,8 @@
  *     where they hand back host scalars (syk_krylov_evolve, syk_otoc, syk_lanczos_run, *_host): those
  *     synchronise that stream only.
  *   - There is no CPU fallback: a compute call on a machine without a CUDA device returns SYK_ECUDA.
- *   - Results are bitwise reproducible run to run: no atomics on data, fixed reduction trees.
+ *   - Results are bitwise reproducible run to run on the same GPU model: no atomics on data, fixed reduction trees
+ *     (per-CTA partial sums and, in the large-vector kernel, a per-CTA order of the terms: both fixed by the SM count).
  */
 #ifndef SYK_B200_H
 #define SYK_B200_H

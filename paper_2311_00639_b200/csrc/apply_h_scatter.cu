@@ -34,7 +34,8 @@
 // by a uniform branch on the two low slice bits of z (accumulate_chunk).  Per-term data comes from the __grid_constant__
 // table (constant bank), the next entry fetched one term ahead.  No atomics on data, one write per output: bitwise
 // reproducible.  ~100 warp instructions per (term, chunk of 16 slices) instead of ~150 with a per-slice sign walk; what
-// the launch is bound by is the supply of tiles (DRAM phases and L2 phases of the lock-stepped CTAs do not overlap; L2
+// the launch is bound by is the supply of tiles (DRAM phases and L2 phases of the lock-stepped CTAs hardly overlap; a
+// staggered start of the CTAs -- each walks the list rotated by a few places -- spreads the misses: -6 % at N = 64; L2
 // prefetching by the TMA unit or by prefetch.global.L2, of every load or only of the loads that must miss, 1..12 loads
 // ahead, made every configuration slower: DESIGN.md section 6).
 //
@@ -70,6 +71,7 @@ constexpr int kSmemLimit = 232448;                 // 227 KiB opt-in maximum per
 constexpr int kMiscBytes = 2 * kMaxRing * 8 + 40 * 8 + 128;
 constexpr uint32_t kRingAlign = 4096;              // alignment of the ring inside the shared window
 constexpr int kWindowBits = 7;                     // ~log2(148 tiles in flight)
+constexpr int kStagger = 8;                        // spread of the per-CTA rotation of the load list, in loads
 constexpr int kFixedR = 3;                         // r bits 0..2 sit at index bits 8..10: a chunk is one contiguous run
 
 template <typename T>
@@ -84,6 +86,7 @@ struct StParams {
     uint32_t* sync;   // lock-step counters (device_utils.cuh lockstep_gate); nullptr = free running
     int epoch_len;
     int lag;
+    int stagger;      // CTA i walks the load list of its tiles rotated by (37 i) mod stagger places (0 = all in phase)
 };
 
 __device__ __forceinline__ void st_fused_scalars(LanczosScalars* sc, int j, double* red, double& s_in, double& s_prev) {
@@ -247,6 +250,13 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
 
     const uint32_t n_tiles = 1u << tab.n_outer;
     const int nring = p.nring, n_loads = tab.n_loads, n_outer = tab.n_outer;
+    // Staggered start (round 2): the CTAs walk the same load list in lock step, so the loads that must come from DRAM (the
+    // first of each run of masks that agree outside tile + window bits) would reach all of them at once.  Rotating the list
+    // by a few places per CTA spreads those misses over time while every tile is still re-read within a few loads of its
+    // first use (measured: -6 % at N = 64, neutral at N = 56; rotations beyond ~12 places lose the L2 reuse).  The order in
+    // which the terms of an output are added then depends on the CTA that owns its tile: results are reproducible for a
+    // given grid size, and equal across kernels only to rounding.
+    const int rot = p.stagger > 0 ? (int)((blockIdx.x * 37u) % (uint32_t)p.stagger) % n_loads : 0;
     double dot = 0.0;
 
     if (warp >= kConsumerWarps) {
@@ -260,7 +270,9 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             uint32_t base = 0;
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
-            for (int l = 0; l < n_loads; ++l) {
+            for (int li = 0; li < n_loads; ++li) {
+                int l = li + rot;
+                if (l >= n_loads) l -= n_loads;
                 if (p.sync) {
                     if (until_epoch == 0) {
                         lockstep_gate(p.sync, g / (uint32_t)p.epoch_len, (uint32_t)p.lag);
@@ -329,7 +341,9 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 ar[r] = 0;
                 ai[r] = 0;
             }
-            for (int l = 0; l < n_loads; ++l) {
+            for (int li = 0; li < n_loads; ++li) {
+                int l = li + rot;
+                if (l >= n_loads) l -= n_loads;
                 const int t0 = tab.load_t0[l], t1 = tab.load_t0[l + 1];
                 for (uint32_t c = 0; c < (uint32_t)NC; ++c) {
                     mbar_wait(bar_full + 8 * pos, phase);
@@ -645,6 +659,8 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
     p.sync = nullptr;
     p.epoch_len = epoch_len;
     p.lag = lag;
+    p.stagger = (((uint64_t)sizeof(C) << h->L) > ((uint64_t)64 << 20) && n_tiles >= 4 * (uint64_t)grid && tab.n_loads >= 2 * kStagger)
+                    ? kStagger : 0;
     if (epoch_len > 0 && ((uint64_t)sizeof(C) << h->L) > ((uint64_t)64 << 20) && n_tiles >= 4 * (uint64_t)grid) {
         p.sync = h->dev.sync;
         SYK_CUDA(cudaMemsetAsync(p.sync, 0, kSyncRing * sizeof(uint32_t), stream));
