@@ -1050,6 +1050,12 @@ def test_nonhermitian_syk_complex_couplings(B, torch, dt):
         exact = onh.expm_propagate(H, tau, v)
         assert relerr(d.cpu().numpy(), exact) <= TOL[dt], (tau, st)
         assert st["n_matvec"] >= 2 and st["err_est"] <= TOL[dt]
+    # norm carrying on the Arnoldi path: the vector keeps its norm, exp(log_norm) restores the result
+    d = to_dev(torch, v)
+    st = B.syk_krylov_evolve(h, d, 1.0, -2.5, wk, {"krylov_dim": 20, "renormalize": 1})
+    got = d.cpu().numpy().astype(np.complex128)
+    assert abs(np.linalg.norm(got) / np.linalg.norm(v) - 1.0) <= (1e-12 if dt == "c128" else 1e-5)
+    assert relerr(got * math.exp(st["log_norm"]), onh.expm_propagate(H, 1.0 - 2.5j, v)) <= TOL[dt]
     # group law through the library itself
     a, b = to_dev(torch, v), to_dev(torch, v)
     B.syk_krylov_evolve(h, a, 0.4, -0.1, wk, o)
