@@ -87,7 +87,13 @@ struct StParams {
     int epoch_len;
     int lag;
     int stagger;      // CTA i walks the load list of its tiles rotated by (37 i) mod stagger places (0 = all in phase)
+    // diagnostic timeline (syk_apply_H_trace; nullptr otherwise): CTA trace_cta records, for its trace_round-th tile, three
+    // clock64 stamps per ring chunk v = list position * NC + chunk: [v] producer issue, [n + v] consumer before the wait for
+    // the chunk, [2 n + v] after it, n = n_loads * NC
+    unsigned long long* trace;
+    int trace_cta, trace_round;
 };
+
 
 __device__ __forceinline__ void st_fused_scalars(LanczosScalars* sc, int j, double* red, double& s_in, double& s_prev) {
     double n2 = reduce_partials(sc->partial_nrm, sc->n_partial_nrm, red);
@@ -212,7 +218,7 @@ __device__ __forceinline__ void dispatch_chunk(uint32_t oc, uint32_t variant, ui
     }
 }
 
-template <typename T, int NR, int LRC, bool FUSED>
+template <typename T, int NR, int LRC, bool FUSED, bool TRACE = false>
 __global__ void __launch_bounds__(kThreads, 1)
 apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p) {
     using C = typename Cx<T>::type;
@@ -270,6 +276,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             uint32_t base = 0;
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
+            const bool tr = TRACE && p.trace && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
             for (int li = 0; li < n_loads; ++li) {
                 int l = li + rot;
                 if (l >= n_loads) l -= n_loads;
@@ -285,6 +292,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     mbar_wait(bar_empty + 8 * pos, phase ^ 1u);
+                    if constexpr (TRACE) if (tr) p.trace[li * NC + c] = clock64();
                     mbar_arrive_expect_tx(bar_full + 8 * pos, CHUNK_BYTES);
 #pragma unroll
                     for (int u = 0; u < RC / kRun; ++u)
@@ -335,6 +343,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
             const uint32_t bt = base | ((uint32_t)tid << (TB - 8));   // index of the element's first amplitude, r bits 0
             const uint32_t stage_base = smem_u32(smem), tid16 = (uint32_t)tid << 4;
+            const bool tr = TRACE && p.trace && tid == 0 && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
             T ar[R * PAIR], ai[R * PAIR];
 #pragma unroll
             for (int r = 0; r < R * PAIR; ++r) {
@@ -346,7 +355,9 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 if (l >= n_loads) l -= n_loads;
                 const int t0 = tab.load_t0[l], t1 = tab.load_t0[l + 1];
                 for (uint32_t c = 0; c < (uint32_t)NC; ++c) {
+                    if constexpr (TRACE) if (tr) p.trace[(n_loads + li) * NC + c] = clock64();
                     mbar_wait(bar_full + 8 * pos, phase);
+                    if constexpr (TRACE) if (tr) p.trace[(2 * n_loads + li) * NC + c] = clock64();
                     const uint32_t cp = stage_base + (uint32_t)pos * CHUNK_BYTES + tid16;
                     uint4 e = tab.term[t0];
                     for (int t = t0; t < t1; ++t) {
@@ -656,6 +667,9 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
     // lock-step only where it pays: the vector does not fit in L2 and there are several rounds of tiles
     int epoch_len = 0, lag = 0;
     get_lockstep(&epoch_len, &lag);
+    p.trace = fa.trace;
+    p.trace_cta = fa.trace_cta;
+    p.trace_round = fa.trace_round;
     p.sync = nullptr;
     p.epoch_len = epoch_len;
     p.lag = lag;
@@ -669,6 +683,10 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
         SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, true>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         apply_h_scatter_kernel<T, NR, LRC, true><<<grid, kThreads, smem, stream>>>(tab, p);
+    } else if (fa.trace) {   // diagnostic build of the plain kernel (syk_apply_H_trace): clock stamps per ring chunk
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false, true>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_scatter_kernel<T, NR, LRC, false, true><<<grid, kThreads, smem, stream>>>(tab, p);
     } else {
         SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -719,6 +737,48 @@ int scatter_tile_bits(int dtype) {
     return kStTB[k] + kStNR[k];
 }
 int scatter_window_bits() { return kWindowBits; }
+
+// syk_apply_H_trace (include/syk.h): one plain product with the timeline of one CTA and the load list it walked
+int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, uint64_t* clk,
+                  int clk_capacity, int32_t* load_terms, uint32_t* load_xo, int load_capacity, int* n_loads, int* rot,
+                  cudaStream_t stream) {
+    const StTable* tab = get_st_table(h, dtype);
+    if (!tab) return SYK_EINVAL;
+    const int k = dtype == SYK_C128 ? 1 : 0;
+    const int nc = 1 << (kStNR[k] - kStLRC[k]);
+    const int n = tab->n_loads * nc;
+    const int sms = num_sms();
+    if (sms <= 0) return SYK_ECUDA;
+    const uint64_t n_tiles = 1ull << tab->n_outer;
+    const uint64_t grid = n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms;
+    if (cta < 0 || (uint64_t)cta >= grid || round < 0 || (uint64_t)round * grid + (uint64_t)cta >= n_tiles ||
+        clk_capacity < 3 * n || load_capacity < tab->n_loads)
+        return SYK_EINVAL;
+    unsigned long long* d_trace = nullptr;
+    SYK_CUDA(cudaMalloc(&d_trace, (size_t)3 * n * sizeof(unsigned long long)));
+    cudaMemsetAsync(d_trace, 0, (size_t)3 * n * sizeof(unsigned long long), stream);
+    FusedArgs fa;
+    fa.trace = d_trace;
+    fa.trace_cta = cta;
+    fa.trace_round = round;
+    int rc = launch_apply_h_scatter(h, dtype, d_in, d_out, fa, stream);
+    if (rc == SYK_OK && cudaMemcpyAsync(clk, d_trace, (size_t)3 * n * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                                        stream) != cudaSuccess)
+        rc = SYK_ECUDA;
+    if (cudaStreamSynchronize(stream) != cudaSuccess) rc = SYK_ECUDA;
+    cudaFree(d_trace);
+    SYK_TRY(rc);
+    for (int l = 0; l < tab->n_loads; ++l) {
+        load_terms[l] = (int32_t)tab->load_t0[l + 1] - (int32_t)tab->load_t0[l];
+        load_xo[l] = tab->load_xo[l];
+    }
+    *n_loads = tab->n_loads;
+    // the rotation launch_st gives this CTA (same conditions)
+    const bool big = ((uint64_t)elem_bytes(dtype) << h->L) > ((uint64_t)64 << 20) && n_tiles >= 4 * grid;
+    const int stagger = big && tab->n_loads >= 2 * kStagger ? kStagger : 0;
+    *rot = stagger > 0 ? (int)(((uint32_t)cta * 37u) % (uint32_t)stagger) % tab->n_loads : 0;
+    return SYK_OK;
+}
 
 void free_scatter_tables(const syk_ham* h) {
     for (int k = 0; k < 2; ++k) {

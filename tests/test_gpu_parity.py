@@ -1311,3 +1311,44 @@ def test_green_batched_vs_oracle(B, torch, dt):
         assert np.max(np.abs(G1[r] - ref)) / abs(ref[0]) <= TOL[dt], r
     with pytest.raises(B.SykError):
         B.syk_green_batched(hams, N, 3.0, t_grid, to_dev(torch, psis.reshape(-1)), D, wk, o)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# diagnostic: syk_apply_H_trace (timeline of one persistent CTA of the scatter-tile kernel)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_apply_H_trace_matches_apply_H(B, torch, dt):
+    """The traced launch is the plain scatter-tile product (vs the oracle, and bitwise equal to syk_apply_H); its clock
+    stamps are ordered (issue <= got, asked <= got, chunks in list order) and its load list is the layout's."""
+    N = 30
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    q, J = couplings(N, 4, seed=5)
+    h = B.syk_build_from_terms(N, q, J)
+    B.syk_set_apply_H_kernel(h, 3)
+    assert B.syk_apply_H_kernel_kind(h, code) == 3
+    rs = np.random.default_rng(11)
+    v = (rs.standard_normal(1 << (N // 2)) + 1j * rs.standard_normal(1 << (N // 2))).astype(npdtype(dt))
+    d_in = to_dev(torch, v)
+    d_ref, d_out = torch.empty_like(d_in), torch.empty_like(d_in)
+    B.syk_apply_H(h, d_in, d_ref)
+    lay = B.syk_apply_H_layout(h, code)
+    n_tiles = (1 << (N // 2)) >> bin(lay["tile_mask"]).count("1")
+    for cta in (0, n_tiles - 1):
+        d_out.fill_(float("nan"))
+        tr = B.syk_apply_H_trace(h, d_in, d_out, cta=cta, round=0)
+        assert torch.equal(d_out, d_ref)
+        assert tr["n_loads"] == lay["n_loads"] and tr["rot"] == 0
+        assert int(tr["load_terms"].sum()) == len(J) and (tr["load_terms"] >= 1).all()
+        assert (tr["issue"] > 0).all() and (tr["after_wait"] >= tr["before_wait"]).all()
+        assert (tr["after_wait"] >= tr["issue"]).all()
+        assert (np.diff(tr["before_wait"]) > 0).all() and (np.diff(tr["issue"]) > 0).all()
+    ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
+    assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt]
+    # a CTA / round that does not exist, a handle on another kernel
+    with pytest.raises(B.SykError):
+        B.syk_apply_H_trace(h, d_in, d_out, cta=n_tiles, round=0)
+    with pytest.raises(B.SykError):
+        B.syk_apply_H_trace(h, d_in, d_out, cta=0, round=1)
+    B.syk_set_apply_H_kernel(h, 1)
+    with pytest.raises(B.SykError):
+        B.syk_apply_H_trace(h, d_in, d_out)
