@@ -471,6 +471,9 @@ def measure_workload(args, wl, name, steps, warmup, world, rank, local, dist, wi
         #   dram_traffic_vs_hbm ncu DRAM bytes per launch (committed capture)   / DRAM -> SM streaming peak
         #   l2_to_sm            (n_loads + 2) V: every load moves the vector once from L2 into the SMs / L2 -> SM peak
         #   lds                 n_terms V: every term reads the staged vector once from shared memory   / LDS peak
+        #   smem_path           (n_terms + n_loads + 2) V: the reads above plus the TMA fills of the ring, which go through the
+        #                       same banks / the LDS rate per clock measured by syk_microbench x the SM clock sampled during
+        #                       this run (profiles/r2_chunk_trace.md: this is the unit that binds the headline launches)
         sec = avg_ms * 1e-3
         fr = {"model_vs_hbm": roofline["frac"]}
         l2_bytes = (layout["n_loads"] + 2) * V
@@ -485,6 +488,12 @@ def measure_workload(args, wl, name, steps, warmup, world, rank, local, dist, wi
                 fr["dram_traffic_vs_hbm_copy_peak"] = roofline["traffic"] / sec / 1e9 / peak
             fr["l2_to_sm_vs_measured_peak"] = detail["l2_to_sm_TB_per_s"] / peaks["l2_to_sm"]["load_TB_per_s"]
             fr["lds_vs_measured_peak"] = detail["lds_TB_per_s"] / peaks["lds_only"]["lds_TB_per_s"]
+            mhz = (clocks or {}).get("sm_mhz") or peaks["lds_only"]["sm_mhz_effective"]
+            smem_bytes = (n_t + layout["n_loads"] + 2) * V
+            smem_peak = peaks["lds_only"]["lds_B_per_clk_per_SM"] * peaks["sms"] * mhz * 1e6
+            detail["smem_reads_plus_fills_bytes_per_launch"] = smem_bytes
+            detail["smem_reads_plus_fills_B_per_clk_per_SM"] = smem_bytes / sec / (peaks["sms"] * mhz * 1e6)
+            fr["smem_reads_plus_fills_vs_lds_rate_at_run_clock"] = smem_bytes / sec / smem_peak
             # supply model of the lock-stepped CTAs: DRAM phases and L2 phases do not overlap
             if roofline["traffic"]:
                 t_supply = (roofline["traffic"] / 1e12 / peaks["dram_to_sm"]["load_TB_per_s"] +

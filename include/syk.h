@@ -368,9 +368,12 @@ int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset);
  *           shift, XOR into the sign bit, FP64 add into one of 8 bin registers), 512 threads per SM.
  *   kind 5: as kind 0 in two groups at once: even CTAs walk the whole of d_buf (DRAM for a multi-GB buffer), odd CTAs only
  *           its first 32 MB (L2 resident) and stream arg1 times as many chunks: do the DRAM and the L2 supply overlap?
+ *   kind 6: do global loads share the shared-memory data path?  256 threads per SM; per iteration (arg0 of them) every
+ *           thread issues 16 LDG.128 (ld.global.cg, 64 KiB of d_buf per CTA and iteration; d_buf = NULL: none) and arg1 x 16
+ *           LDS.128 over a staged 64 KiB chunk, one FP64 FMA pair per value.
  * result[6]: [0] = device time in ms (CUDA events), [1] = SM cycles of the slowest CTA (clock64), [2] = bytes copied
- * into shared memory (kinds 0, 2; kind 5: by the even CTAs) or thread-level adds (kinds 3, 4), [3] = bytes read by LDS
- * (kinds 1, 2; kind 5: bytes copied by the odd CTAs), [4] / [5] = cycles of the slowest even / odd CTA.
+ * into shared memory (kinds 0, 2; kind 5: by the even CTAs), thread-level adds (kinds 3, 4) or bytes loaded by LDG (kind 6),
+ * [3] = bytes read by LDS (kinds 1, 2, 6; kind 5: bytes copied by the odd CTAs), [4] / [5] = cycles of the slowest even / odd CTA.
  * d_work: >= syk_microbench_workspace_bytes() of device memory; d_buf (kinds 0, 2): 128-byte aligned, buf_bytes >= 128 KiB
  * (rounded down to a power of two).  Synchronises. */
 size_t syk_microbench_workspace_bytes(void);

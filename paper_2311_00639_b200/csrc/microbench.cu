@@ -172,6 +172,68 @@ __global__ void __launch_bounds__(512, 1) mb_alu_kernel(int iters, int mode, dou
     if (tid == 0) cycles[blockIdx.x] = t1 - t0;
 }
 
+// Do global loads share the shared-memory data path?  256 threads per SM; per iteration every thread issues 16 LDG.128
+// (ld.global.cg: one 64 KiB stretch of an L2-resident buffer per CTA and iteration, coalesced) and `lds_passes` x 16
+// LDS.128 over a 64 KiB staged chunk (the consumers' access pattern), each value used by one FP64 FMA pair.
+__global__ void __launch_bounds__(256, 1) mb_ldg_kernel(const double2* __restrict__ g, uint32_t n_el_log2, int iters,
+                                                        int lds_passes, int with_ldg, double2* sink,
+                                                        unsigned long long* cycles) {
+    extern __shared__ __align__(128) unsigned char mb_smem[];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < 65536 / 16; i += 256) reinterpret_cast<double2*>(mb_smem)[i] = make_double2(1.0, 0.5);
+    __syncthreads();
+    const uint32_t sb = smem_u32(mb_smem) + (uint32_t)tid * 16u;
+    double ar[16], ai[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        ar[r] = 0.0;
+        ai[r] = 0.0;
+    }
+    const uint32_t mask = (1u << n_el_log2) - 1u;
+    uint32_t pos = (blockIdx.x * 4096u * 37u) & mask;
+    const unsigned long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+        double2 vg[16];
+        if (with_ldg) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const double2* q = g + ((pos + (uint32_t)r * 256u + (uint32_t)tid) & mask);
+                asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(vg[r].x), "=d"(vg[r].y) : "l"(q));
+            }
+            pos = (pos + 4096u * 149u) & mask;
+        }
+        for (int s = 0; s < lds_passes; ++s) {
+            double2 vs[16];
+#pragma unroll
+            for (int r = 0; r < 16; ++r)
+                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];"
+                             : "=d"(vs[r].x), "=d"(vs[r].y)
+                             : "r"(sb + (((uint32_t)r ^ ((uint32_t)(it + s) & 15u)) << 12)));
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                ar[r] = __fma_rn(1.0000001, vs[r].x, ar[r]);
+                ai[r] = __fma_rn(1.0000001, vs[r].y, ai[r]);
+            }
+        }
+        if (with_ldg) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                ar[r] = __fma_rn(1.0000001, vg[r].x, ar[r]);
+                ai[r] = __fma_rn(1.0000001, vg[r].y, ai[r]);
+            }
+        }
+    }
+    const unsigned long long t1 = clock64();
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        sr += ar[r];
+        si += ai[r];
+    }
+    sink[(size_t)blockIdx.x * 256 + tid] = make_double2(sr, si);
+    if (tid == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
 }  // namespace
 }  // namespace syk
 
@@ -246,6 +308,28 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
                 rc = SYK_ECUDA;
             }
             units = (double)sms * 512.0 * 64.0 * arg0;   // thread-level adds
+            count_launch();
+        }
+    } else if (kind == 6) {
+        // arg0 = iterations, arg1 = LDS passes per iteration (0 = global loads only); d_buf = NULL: LDS only
+        int buf_log2 = 0;
+        while (d_buf && ((size_t)2 << buf_log2) <= buf_bytes) ++buf_log2;
+        if (arg0 < 1 || arg1 < 0 || (!d_buf && arg1 < 1) || (d_buf && (buf_log2 < 17 || ((uintptr_t)d_buf & 127)))) rc = SYK_EINVAL;
+        if (rc == SYK_OK) {
+            cudaError_t e = cudaFuncSetAttribute(mb_ldg_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+            if (e == cudaSuccess) {
+                cudaEventRecord(e0, st);
+                mb_ldg_kernel<<<sms, 256, 65536, st>>>((const double2*)d_buf, d_buf ? (uint32_t)(buf_log2 - 4) : 0u, arg0, arg1,
+                                                       d_buf ? 1 : 0, (double2*)d_sink, d_cycles);
+                cudaEventRecord(e1, st);
+                e = cudaGetLastError();
+            }
+            if (e != cudaSuccess) {
+                set_cuda_error(e, "mb_ldg_kernel");
+                rc = SYK_ECUDA;
+            }
+            units = d_buf ? (double)sms * arg0 * 65536.0 : 0.0;       // bytes by global loads
+            units2 = (double)sms * arg0 * (double)arg1 * 65536.0;     // bytes by LDS
             count_launch();
         }
     } else {

@@ -56,6 +56,20 @@ def measure(quick=False):
                 "dram_group_B_per_clk_per_SM": r["units"] / ((sms + 1) // 2) / r["cycles_even"],
                 "l2_group_B_per_clk_per_SM": r["lds_bytes"] / (sms // 2) / r["cycles_odd"]}
         del big
+    # global loads against the shared-memory data path (kind 6): LDS alone, LDG alone (L2 hits), both
+    it6 = 1000 if quick else 4000
+    for name, buf, passes in (("lds_plain", None, 1), ("ldg_l2", small, 0), ("ldg_l2_and_lds_1", small, 1),
+                              ("ldg_l2_and_lds_2", small, 2), ("ldg_l2_and_lds_3", small, 3)):
+        B.syk_microbench(6, it6 // 8, passes, buf, wk)
+        r = B.syk_microbench(6, it6, passes, buf, wk)
+        d = {"ms": r["ms"], "cycles": r["cycles"], "sm_mhz_effective": r["cycles"] / (r["ms"] * 1e-3) / 1e6}
+        if r["units"]:
+            d["load_B_per_clk_per_SM"] = r["units"] / sms / r["cycles"]
+            d["load_TB_per_s"] = r["units"] / (r["ms"] * 1e-3) / 1e12
+        if r["lds_bytes"]:
+            d["lds_B_per_clk_per_SM"] = r["lds_bytes"] / sms / r["cycles"]
+            d["lds_TB_per_s"] = r["lds_bytes"] / (r["ms"] * 1e-3) / 1e12
+        out[name] = d
     iters = 4000 if quick else 20000
     for name, kind in (("fp64_add", 3), ("dense_term_sequence", 4)):
         B.syk_microbench(kind, iters // 8, 0, None, wk)
