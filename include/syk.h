@@ -303,8 +303,8 @@ int syk_green_batched(const syk_ham* const* hams, int n_batch, int dtype, int n,
  * 2 = TMA-pipelined register-tile gather (64 KiB tiles; sparse H with <= 1024 terms and D >= 2^22 / 2^23),
  * 3 = TMA-pipelined scatter-tile gather (128 KiB tiles on index bits chosen per Hamiltonian; sparse H with
  *     1..1024 terms and D >= 2^23 / 2^24),
- * 4 = dense-table kernel (many terms per X-mask: terms binned by the Walsh index of their Z-mask and transformed once per
- *     X-mask; chosen for > 1024 terms with >= 4 terms per X-mask and D >= 2^12; holds its own device table and, for
+ * 4 = dense-table kernel (many terms per X-mask: an X-mask whose Z-masks agree outside its own bits is one table lookup per
+ *     amplitude, the others have their terms binned by the Walsh index of the Z-mask and transformed once per X-mask; chosen for > 1024 terms with >= 4 terms per X-mask and D >= 2^12; holds its own device table and, for
  *     vectors with fewer tiles than SMs, a scratch buffer for partial sums). */
 int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
 /* Force the kernel choice for subsequent syk_apply_H calls on this handle: -1 = automatic, 0 / 1 / 2 / 3 / 4 as above
@@ -312,9 +312,11 @@ int syk_apply_H_kernel_kind(const syk_ham* h, int dtype);
 int syk_set_apply_H_kernel(syk_ham* h, int kind);
 /* Shape of the dense-table kernel's (kind 4) device table for this handle: n_loads source tiles per output tile,
  * n_chunks table chunks of <= 512 entries streamed per output tile, split = CTAs that share one output tile (1 = the
- * persistent one-CTA-per-tile form; > 1 = the split form for vectors with fewer tiles than SMs).  Builds the table if
- * needed.  Any output pointer may be NULL.  SYK_EINVAL if the handle cannot use kind 4. */
-int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split);
+ * persistent one-CTA-per-tile form; > 1 = the split form for vectors with fewer tiles than SMs), n_local_groups =
+ * X-masks whose terms are applied through ONE table of 2^popcount(x) values instead of term by term (their Z-masks agree
+ * outside the bits of x, popcount(x) <= 4, >= 4 terms: every four-qubit X-mask of a dense SYK Hamiltonian).  Builds the
+ * table if needed.  Any output pointer may be NULL.  SYK_EINVAL if the handle cannot use kind 4. */
+int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split, int* n_local_groups);
 /* Tile layout the scatter-tile kernel (kind 3) uses for this Hamiltonian in its current qubit layout: n_loads = source tiles fetched per
  * output tile (L2 -> SM transfers of the whole vector per product), n_passes = distinct X-masks outside tile and
  * L2-window bits (DRAM reads of the whole vector per product, if L2 reuse were perfect), tile_mask / window_mask =

@@ -69,7 +69,7 @@ _SIGNATURES = {
     "syk_random_state_h": (_i, [_vp, _u64, _u32, _i, _vp, _vp, _vp]),
     "syk_apply_gamma_h": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "syk_apply_gamma_block_h": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp]),
-    "syk_apply_H_dense_info": (_i, [_vp, _i, _P(_i), _P(_i), _P(_i)]),
+    "syk_apply_H_dense_info": (_i, [_vp, _i, _P(_i), _P(_i), _P(_i), _P(_i)]),
     "syk_apply_H": (_i, [_vp, _i, _vp, _vp, _vp]),
     "syk_apply_H_batched": (_i, [_P(_vp), _i, _i, _vp, _vp, _i64, _vp]),
     "syk_apply_H_host": (_i, [_vp, _i, _vp, _vp, _vp, _sz, _vp]),
@@ -314,10 +314,10 @@ def syk_ham_prepare(h, dtype):
 
 
 def syk_apply_H_dense_info(h, dtype):
-    nl, nc, sp = _i(), _i(), _i()
-    _check(_lib.syk_apply_H_dense_info(_h(h), int(dtype), ctypes.byref(nl), ctypes.byref(nc), ctypes.byref(sp)),
-           "syk_apply_H_dense_info")
-    return {"n_loads": nl.value, "n_chunks": nc.value, "split": sp.value}
+    nl, nc, sp, ng = _i(), _i(), _i(), _i()
+    _check(_lib.syk_apply_H_dense_info(_h(h), int(dtype), ctypes.byref(nl), ctypes.byref(nc), ctypes.byref(sp),
+                                       ctypes.byref(ng)), "syk_apply_H_dense_info")
+    return {"n_loads": nl.value, "n_chunks": nc.value, "split": sp.value, "n_local_groups": ng.value}
 
 
 # ---- a-2 ---------------------------------------------------------------------------------------------------

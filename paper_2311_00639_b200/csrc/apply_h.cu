@@ -651,9 +651,9 @@ int syk_ham_prepare(const syk_ham* h, int dtype) {
     return SYK_OK;
 }
 
-int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split) {
+int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split, int* n_local_groups) {
     if (!h || (dtype != SYK_C64 && dtype != SYK_C128) || !syk::dense_kernel_ok(h, true)) return SYK_EINVAL;
-    return syk::dense_tables_info(h, dtype, n_loads, n_chunks, split);
+    return syk::dense_tables_info(h, dtype, n_loads, n_chunks, split, n_local_groups);
 }
 
 int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,

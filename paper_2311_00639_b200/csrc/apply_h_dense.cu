@@ -51,6 +51,8 @@ constexpr int kMiscBytes = 2 * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, r
 // The consumers copy chunk k+1 into shared memory while they work on chunk k (double buffer), so every table read
 // in the inner loops is a broadcast LDS instead of a dependent global load.
 constexpr int kChunkEntries = 512;
+constexpr int kLocalMaxBits = 4;                   // x-local groups: popcount(x) <= 4 (a table of <= 16 values)
+constexpr int kLocalMinTerms = 4;                  // ... and at least this many terms (else the per-term walk is cheaper)
 struct DenseLoad { uint32_t hi, c0, c1, pad; };    // source tile = tile ^ hi; chunks [c0, c1)
 struct DenseChunk { uint32_t e0, ne, pad0, pad1; };// entries [e0, e0 + ne)
 
@@ -123,6 +125,73 @@ __device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// X-LOCAL groups.  If the Z-masks of a group agree outside the bits of its X-mask x (popcount(x) = k <= 4) -- true for every
+// group of a dense SYK Hamiltonian whose x has four bits: its 16 terms are the X / Y choices on the four flipped qubits, the
+// Jordan-Wigner strings are common -- then the whole group is ONE function of k bits of b:
+//     S_g(b) = (-1)^popcount(b & zb) F[pext(b, x)],   zb = the common part of z outside x,
+//     F[i]   = sum_t c_t (-1)^popcount(pdep(i, x) & z_t)                     (2^k complex numbers, summed on the host).
+// Per (group, amplitude) that is one table read and one complex multiply-add instead of one sign-accumulate per term: 16 terms
+// cost what ~3 cost before.  The table index of the thread's 8 amplitudes differs only through the r bits (index bits 9..11)
+// that x contains, XR = (x >> 9) & 7: 2^popcount(XR) table reads per thread (1.6 on average for random x), and the source
+// slice r ^ XR is a compile-time offset of the variant the (uniform) switch on XR selects.
+// Stream format of such a group: header A {x & (tile - 1), 1 + 2^k, 4, zb}, header B {.x = positions of the bits of x, 5 bits
+// each (unused: 9, an r bit, always 0 in the thread's base index), .y = index bit of r bit j in bits 2j..2j+1}, then F[0 .. 2^k)
+// as (re, im) doubles or floats at a 16-byte stride.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, int XR>
+__device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_t idx0, uint32_t mpos, uint32_t sgn0,
+                                            uint32_t zbr, const typename Cx<T>::type* pb, T (&ar)[kR], T (&ai)[kR]) {
+    using C = typename Cx<T>::type;
+    constexpr int ND = 1 << ((XR & 1) + ((XR >> 1) & 1) + ((XR >> 2) & 1));
+    T fr[ND], fi[ND];
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        // bits of d go to the index-bit positions of the r bits that x contains (ascending r bit)
+        uint32_t delta = 0;
+        int dj = 0;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            if (XR & (1 << j)) {
+                if (d & (1 << dj)) delta |= 1u << ((mpos >> (2 * j)) & 3u);
+                ++dj;
+            }
+        }
+        const uint4 e = F[idx0 ^ delta];
+        if constexpr (sizeof(T) == 8) {
+            fr[d] = __hiloint2double((int)e.y, (int)e.x);
+            fi[d] = __hiloint2double((int)e.w, (int)e.z);
+        } else {
+            fr[d] = __uint_as_float(e.x);
+            fi[d] = __uint_as_float(e.y);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        // which of the ND table values: the bits of r inside XR, compacted (compile time)
+        int d = 0, dj = 0;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            if (XR & (1 << j)) {
+                if (r & (1 << j)) d |= 1 << dj;
+                ++dj;
+            }
+        }
+        const uint32_t sg = sgn0 ^ ((uint32_t)__popc((uint32_t)r & zbr) << 31);
+        T a, bq;
+        if constexpr (sizeof(T) == 8) {
+            a = __hiloint2double(__double2hiint(fr[d]) ^ (int)sg, __double2loint(fr[d]));
+            bq = __hiloint2double(__double2hiint(fi[d]) ^ (int)sg, __double2loint(fi[d]));
+        } else {
+            a = __uint_as_float(__float_as_uint(fr[d]) ^ sg);
+            bq = __uint_as_float(__float_as_uint(fi[d]) ^ sg);
+        }
+        const C v = pb[(uint32_t)(r ^ XR) << kThreadBitsD];
+        ar[r] += a * v.x - bq * v.y;
+        ai[r] += a * v.y + bq * v.x;
+    }
+}
+
 // All groups of one staged table chunk applied to the thread's kR accumulators; `sp` = the staged source tile.
 template <typename T>
 __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uint32_t ne, const typename Cx<T>::type* sp,
@@ -132,6 +201,28 @@ __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uin
     while (i < ne) {
         const uint4 gh = ent[i];   // group header
         const uint32_t i_end = i + 1 + gh.y;
+        if (gh.z == 4u) {          // x-local group: one table value per amplitude
+            const uint4 hb = ent[i + 1];
+            const uint4* F = ent + i + 2;
+            uint32_t idx0 = 0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) idx0 |= ((bt >> ((hb.x >> (5 * k)) & 31u)) & 1u) << k;
+            const uint32_t sgn0 = (uint32_t)__popc(bt & gh.w) << 31;
+            const uint32_t zbr = (gh.w >> kThreadBitsD) & (uint32_t)(kR - 1);
+            const C* pbl = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
+            switch (gh.x >> kThreadBitsD) {
+                case 0: local_group<T, 0>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 1: local_group<T, 1>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 2: local_group<T, 2>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 3: local_group<T, 3>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 4: local_group<T, 4>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 5: local_group<T, 5>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 6: local_group<T, 6>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                default: local_group<T, 7>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+            }
+            i = i_end;
+            continue;
+        }
         T cr[kR], ci[kR];
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
@@ -417,6 +508,7 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
     std::vector<DenseChunk> chunks;
     std::vector<uint4> entries;
     entries.reserve(h->z.size() + ng);
+    int n_local = 0;
     for (size_t g = 0; g < ng; ++g) {
         const uint32_t x = (uint32_t)h->x[g];
         const uint32_t hi = x >> kTileLog2D;
@@ -427,8 +519,62 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
             if (!loads.empty()) loads.back().c1 = (uint32_t)chunks.size();
             loads.push_back(DenseLoad{hi, (uint32_t)chunks.size(), 0u, 0u});
         }
-        if (new_load || chunks.back().ne + nt + 1 > (uint32_t)kChunkEntries - 1)   // one spare entry: read-ahead
+        // x-local group (see local_group): all Z-masks agree outside x, popcount(x) <= 4, enough terms to pay for the table
+        const int kx = __builtin_popcount(x);
+        bool local = kx <= kLocalMaxBits && nt >= (uint32_t)kLocalMinTerms;
+        const uint32_t z_first = (uint32_t)h->z[h->group_off[g]];
+        for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1] && local; ++t)
+            if ((((uint32_t)h->z[t]) ^ z_first) & ~x) local = false;
+        const uint32_t n_follow = local ? 1u + (1u << kx) : nt;
+        if (new_load || chunks.back().ne + n_follow + 1 > (uint32_t)kChunkEntries - 1)   // one spare entry: read-ahead
             chunks.push_back(DenseChunk{(uint32_t)entries.size(), 0u, hi, 0u});
+        if (local) {
+            int pos[4] = {kThreadBitsD, kThreadBitsD, kThreadBitsD, kThreadBitsD};   // unused: an r bit (0 in the base index)
+            int np = 0;
+            for (int q = 0; q < 32; ++q)
+                if (x & (1u << q)) pos[np++] = q;
+            uint32_t mpos = 0;   // index bit of r bit j (index bit 9 + j of the vector), if x contains it
+            for (int j = 0; j < 3; ++j) {
+                const uint32_t bit = 1u << (kThreadBitsD + j);
+                if (x & bit) mpos |= (uint32_t)__builtin_popcount(x & (bit - 1u)) << (2 * j);
+            }
+            entries.push_back(make_uint4(x & (uint32_t)(kTile - 1), n_follow, 4u, z_first & ~x));
+            entries.push_back(make_uint4((uint32_t)pos[0] | (uint32_t)pos[1] << 5 | (uint32_t)pos[2] << 10 | (uint32_t)pos[3] << 15,
+                                         mpos, 0u, 0u));
+            for (uint32_t i = 0; i < (1u << kx); ++i) {
+                uint32_t dep = 0;   // pdep(i, x)
+                for (int q = 0; q < np; ++q)
+                    if (i & (1u << q)) dep |= 1u << pos[q];
+                double fr = 0.0, fi = 0.0;
+                for (uint32_t t = h->group_off[g]; t < h->group_off[g + 1]; ++t) {
+                    const std::complex<double> c = h->c[t];
+                    if (c.imag() != 0.0 && c.real() != 0.0) return SYK_EINVAL;
+                    double re = c.real(), im = c.imag();
+                    if (dtype != SYK_C128) {   // R-C64: coefficients rounded once to fp32, summed exactly enough in fp64
+                        re = (double)(float)re;
+                        im = (double)(float)im;
+                    }
+                    const double sg = (__builtin_popcount(dep & (uint32_t)h->z[t]) & 1) ? -1.0 : 1.0;
+                    fr += sg * re;
+                    fi += sg * im;
+                }
+                uint4 e = make_uint4(0u, 0u, 0u, 0u);
+                if (dtype == SYK_C128) {
+                    uint64_t b0, b1;
+                    std::memcpy(&b0, &fr, 8);
+                    std::memcpy(&b1, &fi, 8);
+                    e = make_uint4((uint32_t)b0, (uint32_t)(b0 >> 32), (uint32_t)b1, (uint32_t)(b1 >> 32));
+                } else {
+                    const float f0 = (float)fr, f1 = (float)fi;
+                    std::memcpy(&e.x, &f0, 4);
+                    std::memcpy(&e.y, &f1, 4);
+                }
+                entries.push_back(e);
+            }
+            chunks.back().ne += n_follow + 1;
+            ++n_local;
+            continue;
+        }
         uint32_t flags = 0, occ = 0;
         const size_t header_at = entries.size();
         entries.push_back(make_uint4(x & (uint32_t)(kTile - 1), nt, 0u, 0u));
@@ -493,6 +639,7 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
     dc.off_terms = off_e;
     dc.n_loads = (int)loads.size();
     dc.n_chunks = (int)chunks.size();
+    dc.n_local_groups = n_local;
     // small vectors: split the chunk list over several CTAs per tile (apply_h_dense_split_kernel)
     dc.split = 1;
     const int sms = num_sms();
@@ -621,12 +768,13 @@ int prepare_dense_tables(const syk_ham* h, int dtype) {
     return get_dense_tables(h, dtype, &dc);
 }
 
-int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split) {
+int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split, int* n_local_groups) {
     const DenseCache* dc = nullptr;
     SYK_TRY(get_dense_tables(h, dtype, &dc));
     if (n_loads) *n_loads = dc->n_loads;
     if (n_chunks) *n_chunks = dc->n_chunks;
     if (split) *split = dc->split;
+    if (n_local_groups) *n_local_groups = dc->n_local_groups;
     return SYK_OK;
 }
 

@@ -76,6 +76,7 @@ struct DenseCache {
     int device = -1;
     size_t off_groups = 0, off_terms = 0;   // byte offsets of the chunk list and of the entry stream
     int n_loads = 0, n_chunks = 0;
+    int n_local_groups = 0;                 // groups applied through a table of 2^popcount(x) values (x-local groups)
     // small vectors: `split` CTAs per tile, each with a range of chunks; partial sums in `partial` ([split][D], owned)
     int split = 1;
     void* partial = nullptr;
@@ -218,7 +219,7 @@ int launch_apply_h_dense(const syk_ham* h, int dtype, const void* d_in, void* d_
                          cudaStream_t stream);
 void free_dense_tables(const syk_ham* h);
 int prepare_dense_tables(const syk_ham* h, int dtype);   // builds / uploads the device table and the split scratch
-int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split);
+int dense_tables_info(const syk_ham* h, int dtype, int* n_loads, int* n_chunks, int* split, int* n_local_groups);
 
 // apply_H launcher shared by syk_apply_H and the Krylov driver (apply_h.cu)
 int launch_apply_h(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,

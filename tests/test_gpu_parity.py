@@ -1352,3 +1352,53 @@ def test_apply_H_trace_matches_apply_H(B, torch, dt):
     B.syk_set_apply_H_kernel(h, 1)
     with pytest.raises(B.SykError):
         B.syk_apply_H_trace(h, d_in, d_out)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# dense-table kernel: x-local groups (one table of 2^popcount(x) values per X-mask)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_dense_local_groups_canonical_and_relabelled(B, torch, dt):
+    """Dense p = 1 (Algorithm 1): every four-qubit X-mask is an x-local group (its 16 terms
+    differ in Z only on the flipped qubits), C(L,4) of them; two-qubit and diagonal masks are not.  apply_H against the
+    oracle in the canonical layout and with the qubits relabelled (the criterion is invariant under a permutation of bits);
+    a mixed Hamiltonian (dense on 12 Majoranas + sparse rest) has local and term-by-term groups in one chunk."""
+    from math import comb
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    rs = np.random.default_rng(21)
+    for N in (24, 26):
+        L, D = N // 2, 1 << (N // 2)
+        q, J, _ = orng.sample_couplings(N, 1.0, 2, 0)
+        v = (rs.standard_normal(D) + 1j * rs.standard_normal(D)).astype(npdtype(dt))
+        ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
+        for perm in (None, rs.permutation(L)):
+            h = B.syk_build_from_terms(N, q, J)
+            if perm is not None:
+                B.syk_ham_set_layout(h, perm)
+            assert B.syk_apply_H_kernel_kind(h, code) == 4
+            assert B.syk_apply_H_dense_info(h, code)["n_local_groups"] == comb(L, 4)
+            d_can = to_dev(torch, v)
+            d_in, d_out, d_back = torch.empty_like(d_can), torch.empty_like(d_can), torch.empty_like(d_can)
+            B.syk_permute_vector(h, True, d_can, d_in)
+            d_out.fill_(float("nan"))
+            B.syk_apply_H(h, d_in, d_out)
+            B.syk_permute_vector(h, False, d_out, d_back)
+            assert relerr(d_back.cpu().numpy(), ref) <= TOL[dt], (N, perm)
+    # mixed: all quartets on Majoranas 0..11 plus sparse quartets elsewhere; kind 4 forced
+    N, D = 28, 1 << 14
+    import itertools
+    qd = np.array(list(itertools.combinations(range(12), 4)), dtype=np.int32)
+    qs, Js = couplings(N, 4, seed=9)
+    qs = np.array([t for t in qs if max(t) >= 12], dtype=np.int32)
+    Js = Js[: len(qs)]
+    q = np.concatenate([qd, qs])
+    J = np.concatenate([rs.standard_normal(len(qd)) * 0.1, Js])
+    h = B.syk_build_from_terms(N, q, J)
+    B.syk_set_apply_H_kernel(h, 4)
+    assert B.syk_apply_H_kernel_kind(h, code) == 4
+    assert B.syk_apply_H_dense_info(h, code)["n_local_groups"] == comb(6, 4)
+    v = (rs.standard_normal(D) + 1j * rs.standard_normal(D)).astype(npdtype(dt))
+    d_in = to_dev(torch, v)
+    d_out = torch.empty_like(d_in)
+    B.syk_apply_H(h, d_in, d_out)
+    assert relerr(d_out.cpu().numpy(), ohm.matvec_sequential(N, q, J, v.astype(np.complex128))) <= TOL[dt]
