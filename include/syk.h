@@ -45,7 +45,8 @@ enum { SYK_OK = 0,
                              unaligned pointer, in == out where forbidden, unsorted quartet or t_grid */
        SYK_ENOMEM = -2,   /* work space too small (ask the *_workspace_bytes query) or host allocation failed */
        SYK_ECUDA = -3,    /* CUDA runtime error or no device; text via syk_last_cuda_error() */
-       SYK_ENOCONV = -4   /* Krylov sub-step limit reached; the result is written, stats->err_est says how bad */ };
+       SYK_ENOCONV = -4,  /* Krylov sub-step limit reached; the result is written, stats->err_est says how bad */
+       SYK_ELIMIT = -5    /* size beyond the fixed device scratch of a *_static entry point (syk_dot_static_max_N) */ };
 
 enum { SYK_C64 = 0, SYK_C128 = 1 };
 enum { SYK_GAMMA_PAULI = 0,  /* gamma_n = Pauli string, {g_m,g_n} = 2 delta; benchmark default */
@@ -174,6 +175,20 @@ int syk_random_state(int N, uint64_t seed, uint32_t realization, int dtype, void
 
 /* <a|b> = sum conj(a[k]) b[k] in fp64 (deterministic); synchronises; result to host re_im[2]. */
 int syk_dot(int N, int dtype, const void* d_a, const void* d_b, void* d_scratch, double* re_im, void* stream);
+
+/* The same inner product for callers that cannot allocate or synchronise (CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): d_result[0..1] (DEVICE memory, 8-byte aligned) <- (Re, Im) <a|b>, by two kernel launches on
+ * `stream`; no scratch argument, no cudaMalloc / cudaFree / allocating routine, no synchronisation, no host copy.  The
+ * per-CTA partial sums live in one file-scope __device__ array of 64 KiB that every GPU loading the library holds until
+ * exit; its device address is resolved once per device (syk_dot_static_prepare, or the first call on that device: call
+ * prepare before starting a capture).  Limit: 2^25 16-byte units, i.e. N <= syk_dot_static_max_N(dtype) = 50 (complex128) /
+ * 52 (complex64); larger N returns SYK_ELIMIT and launches nothing.  Every CTA sums a fixed stretch of the vector, so the
+ * result depends on the data only (bitwise equal on every GPU; equal to syk_dot to rounding).  All calls of a process on a
+ * device SHARE the array: calls that overlap on the GPU (two streams, independent graph branches) race and give wrong
+ * results -- order them.  Nothing in the array needs clearing between calls. */
+int syk_dot_static_max_N(int dtype);
+int syk_dot_static_prepare(void);
+int syk_dot_static(int N, int dtype, const void* d_a, const void* d_b, double* d_result, void* stream);
 
 /* ------------------------------------------------------------------------------------------------------------
  * a-3 / a-4  Lanczos and the Krylov exponential, PAPER.md:301 ("restarted Krylov subspace method for

@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsyk_b200.so")
 
-SYK_OK, SYK_EINVAL, SYK_ENOMEM, SYK_ECUDA, SYK_ENOCONV = 0, -1, -2, -3, -4
+SYK_OK, SYK_EINVAL, SYK_ENOMEM, SYK_ECUDA, SYK_ENOCONV, SYK_ELIMIT = 0, -1, -2, -3, -4, -5
 SYK_C64, SYK_C128 = 0, 1
 SYK_GAMMA_PAULI, SYK_GAMMA_HALF = 0, 1
 
@@ -77,6 +77,9 @@ _SIGNATURES = {
     "syk_reduce_scratch_bytes": (_sz, []),
     "syk_random_state": (_i, [_i, _u64, _u32, _i, _vp, _vp, _vp]),
     "syk_dot": (_i, [_i, _i, _vp, _vp, _vp, _P(_d), _vp]),
+    "syk_dot_static_max_N": (_i, [_i]),
+    "syk_dot_static_prepare": (_i, []),
+    "syk_dot_static": (_i, [_i, _i, _vp, _vp, _vp, _vp]),
     "syk_krylov_workspace_bytes": (_i, [_vp, _i, _P(syk_krylov_opts), _P(_sz)]),
     "syk_lanczos_run": (_i, [_vp, _i, _vp, _i, _vp, _vp, _vp, _sz, _P(syk_stats), _vp]),
     "syk_krylov_evolve": (_i, [_vp, _i, _vp, _d, _d, _P(syk_krylov_opts), _vp, _sz, _P(syk_stats), _vp]),
@@ -383,6 +386,21 @@ def syk_dot(N, d_a, d_b, d_scratch, stream=None):
     _check(_lib.syk_dot(int(N), dtype_code(d_a), _dptr(d_a), _dptr(d_b), _dptr(d_scratch), out, _stream(stream)),
            "syk_dot")
     return complex(out[0], out[1])
+
+
+def syk_dot_static_max_N(dtype):
+    return int(_lib.syk_dot_static_max_N(int(dtype)))
+
+
+def syk_dot_static_prepare():
+    _check(_lib.syk_dot_static_prepare(), "syk_dot_static_prepare")
+
+
+def syk_dot_static(N, d_a, d_b, d_result, stream=None):
+    """(Re, Im) <a|b> into the DEVICE tensor d_result (2 float64); allocation-free, asynchronous (include/syk.h)."""
+    _check(_lib.syk_dot_static(int(N), dtype_code(d_a), _dptr(d_a), _dptr(d_b), _dptr(d_result), _stream(stream)),
+           "syk_dot_static")
+    return d_result
 
 
 # ---- a-3 / a-4 ---------------------------------------------------------------------------------------------

@@ -6,7 +6,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["term_compiler.cpp", "device_tables.cu", "apply_h.cu", "apply_h_regtile.cu", "apply_h_scatter.cu", "apply_h_dense.cu", "vector_ops.cu", "krylov.cu", "arnoldi.cu", "otoc.cu", "microbench.cu"]
+SOURCES = ["term_compiler.cpp", "device_tables.cu", "apply_h.cu", "apply_h_regtile.cu", "apply_h_scatter.cu", "apply_h_dense.cu", "vector_ops.cu", "krylov.cu", "arnoldi.cu", "otoc.cu", "microbench.cu", "dot_static.cu"]
 LIB = os.path.join(HERE, "libsyk_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xcompiler", "-Wno-unknown-pragmas", "-cudart", "static"]

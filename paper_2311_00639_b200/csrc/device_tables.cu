@@ -192,6 +192,7 @@ const char* syk_strerror(int code) {
         case SYK_ENOMEM: return "work space too small or out of host memory";
         case SYK_ECUDA: return "CUDA error or no CUDA device (see syk_last_cuda_error)";
         case SYK_ENOCONV: return "Krylov sub-step limit reached";
+        case SYK_ELIMIT: return "size exceeds the fixed device scratch of a *_static entry point (see syk_dot_static_max_N)";
         default: return "unknown error code";
     }
 }
