@@ -434,6 +434,21 @@ def measure_workload(args, wl, name, steps, warmup, world, rank, local, dist, wi
     kind = B.syk_apply_H_kernel_kind(h0, code)
     layout = B.syk_apply_H_layout(h0, code) if kind == 3 else None
     perm = [int(x) for x in B.syk_ham_layout(h0)["perm"]]
+    dense_shape = None
+    if kind == 4:
+        # groups the dense-table kernel applies through one table lookup per amplitude (x-local groups) and the terms left
+        # to the term-by-term walk: the same criterion as csrc/apply_h_dense.cu, counted here on the exported tables
+        import numpy as np
+        tb = h0.tables()
+        gx, goff, tz = tb["x"].astype(np.uint64), tb["group_off"], tb["z"].astype(np.uint64)
+        n_local, walk_terms = 0, 0
+        for g in range(len(gx)):
+            zs = tz[goff[g]:goff[g + 1]]
+            if bin(int(gx[g])).count("1") <= 4 and len(zs) >= 4 and not np.any((zs ^ zs[0]) & ~gx[g]):
+                n_local += 1
+            else:
+                walk_terms += len(zs)
+        dense_shape = dict(B.syk_apply_H_dense_info(h0, code), walk_terms=walk_terms, local_by_tables=n_local)
     h0.close()
     del l, r, wk, scratch
     torch.cuda.empty_cache()
@@ -516,6 +531,19 @@ def measure_workload(args, wl, name, steps, warmup, world, rank, local, dist, wi
                          "peak_source": ("measured: syk_microbench kind 4 (the kernel's per-term instruction sequence, 512 "
                                          "threads per SM)" if peaks else "fallback: 12.1 adds/clk/SM x 148 SMs x 1.965 GHz"),
                          "model_GBs_for_reference": achieved})
+        if dense_shape and dense_shape["n_local_groups"] > 0 and apply_n:
+            # With x-local groups most terms are never walked: the arithmetic the launch cannot avoid is one complex
+            # multiply-add (4 FP64 FMA) per (X-mask, amplitude) plus one add per (walked term, thread).  Roofline = those
+            # FP64 issue slots / time against the FP64 issue rate of this box (syk_microbench kind 3: one DADD/DFMA per lane).
+            ops = 4.0 * n_x * D + dense_shape["walk_terms"] * (D / 8.0)
+            fp64_peak = peaks["fp64_add"]["adds_per_s"] if peaks else 63.9 * 148 * 1.965e9
+            roofline.update({"achieved": ops / (avg_ms * 1e-3) / 1e9, "peak": fp64_peak / 1e9,
+                             "unit": "G FP64 issue slots/s (FMA or add)", "frac": ops / (avg_ms * 1e-3) / fp64_peak,
+                             "peak_source": ("measured: syk_microbench kind 3 (FP64 add issue rate, 512 threads per SM)"
+                                             if peaks else "fallback: 63.9 /clk/SM x 148 SMs x 1.965 GHz"),
+                             "fp64_ops_per_launch": ops, "dense_table": dense_shape,
+                             "effective_term_adds_per_s": ach,
+                             "effective_term_adds_vs_term_sequence_peak": ach / alu_peak if ach else None})
 
     cpu = None
     if with_cpu:

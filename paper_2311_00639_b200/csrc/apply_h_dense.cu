@@ -85,6 +85,9 @@ __device__ __forceinline__ void dn_fused_scalars(LanczosScalars* sc, int j, doub
     }
 }
 
+__device__ __forceinline__ double dn_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float dn_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+
 // in-place Walsh-Hadamard transform: s[r] = sum_z c[z] (-1)^popcount(r & z)
 template <typename T>
 __device__ __forceinline__ void wht(T (&c)[kR]) {
@@ -136,12 +139,13 @@ __device__ __forceinline__ void walk_bins(const uint4* __restrict__ ent, uint32_
 // that x contains, XR = (x >> 9) & 7: 2^popcount(XR) table reads per thread (1.6 on average for random x), and the source
 // slice r ^ XR is a compile-time offset of the variant the (uniform) switch on XR selects.
 // Stream format of such a group: header A {x & (tile - 1), 1 + 2^k, 4, zb}, header B {.x = positions of the bits of x, 5 bits
-// each (unused: 9, an r bit, always 0 in the thread's base index), .y = index bit of r bit j in bits 2j..2j+1}, then F[0 .. 2^k)
+// each (unused: 9, an r bit, always 0 in the thread's base index), .y = index bit of r bit j in bits 2j..2j+1, .z = Walsh mask
+// of zb's r bits}, then F[0 .. 2^k)
 // as (re, im) doubles or floats at a 16-byte stride.
 // ---------------------------------------------------------------------------------------------------------
 template <typename T, int XR>
-__device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_t idx0, uint32_t mpos, uint32_t sgn0,
-                                            uint32_t zbr, const typename Cx<T>::type* pb, T (&ar)[kR], T (&ai)[kR]) {
+__device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_t idx0, uint32_t mpos, uint32_t W,
+                                            const typename Cx<T>::type* pb, T (&ar)[kR], T (&ai)[kR]) {
     using C = typename Cx<T>::type;
     constexpr int ND = 1 << ((XR & 1) + ((XR >> 1) & 1) + ((XR >> 2) & 1));
     T fr[ND], fi[ND];
@@ -177,18 +181,25 @@ __device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_
                 ++dj;
             }
         }
-        const uint32_t sg = sgn0 ^ ((uint32_t)__popc((uint32_t)r & zbr) << 31);
-        T a, bq;
+        // sign of amplitude r = bit r of W (Walsh function of r for the group's zb, times the thread's own sign), applied to
+        // the loaded source value in place: one shift and two LOP3 per amplitude; then four FMAs
+        const uint32_t sg = (W << (31 - r)) & 0x80000000u;
+        C v = pb[(uint32_t)(r ^ XR) << kThreadBitsD];
         if constexpr (sizeof(T) == 8) {
-            a = __hiloint2double(__double2hiint(fr[d]) ^ (int)sg, __double2loint(fr[d]));
-            bq = __hiloint2double(__double2hiint(fi[d]) ^ (int)sg, __double2loint(fi[d]));
+            v.x = __hiloint2double(__double2hiint(v.x) ^ (int)sg, __double2loint(v.x));
+            v.y = __hiloint2double(__double2hiint(v.y) ^ (int)sg, __double2loint(v.y));
+            ar[r] = __fma_rn(fr[d], v.x, ar[r]);
+            ar[r] = __fma_rn(-fi[d], v.y, ar[r]);
+            ai[r] = __fma_rn(fr[d], v.y, ai[r]);
+            ai[r] = __fma_rn(fi[d], v.x, ai[r]);
         } else {
-            a = __uint_as_float(__float_as_uint(fr[d]) ^ sg);
-            bq = __uint_as_float(__float_as_uint(fi[d]) ^ sg);
+            v.x = __uint_as_float(__float_as_uint(v.x) ^ sg);
+            v.y = __uint_as_float(__float_as_uint(v.y) ^ sg);
+            ar[r] = __fmaf_rn(fr[d], v.x, ar[r]);
+            ar[r] = __fmaf_rn(-fi[d], v.y, ar[r]);
+            ai[r] = __fmaf_rn(fr[d], v.y, ai[r]);
+            ai[r] = __fmaf_rn(fi[d], v.x, ai[r]);
         }
-        const C v = pb[(uint32_t)(r ^ XR) << kThreadBitsD];
-        ar[r] += a * v.x - bq * v.y;
-        ai[r] += a * v.y + bq * v.x;
     }
 }
 
@@ -207,18 +218,18 @@ __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uin
             uint32_t idx0 = 0;
 #pragma unroll
             for (int k = 0; k < 4; ++k) idx0 |= ((bt >> ((hb.x >> (5 * k)) & 31u)) & 1u) << k;
-            const uint32_t sgn0 = (uint32_t)__popc(bt & gh.w) << 31;
-            const uint32_t zbr = (gh.w >> kThreadBitsD) & (uint32_t)(kR - 1);
+            // hb.z = Walsh mask of the r bits of zb: bit r = parity(r & zb's bits 9..11); times the thread's own sign
+            const uint32_t W = hb.z ^ (0u - ((uint32_t)__popc(bt & gh.w) & 1u));
             const C* pbl = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
             switch (gh.x >> kThreadBitsD) {
-                case 0: local_group<T, 0>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 1: local_group<T, 1>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 2: local_group<T, 2>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 3: local_group<T, 3>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 4: local_group<T, 4>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 5: local_group<T, 5>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                case 6: local_group<T, 6>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
-                default: local_group<T, 7>(F, idx0, hb.y, sgn0, zbr, pbl, ar, ai); break;
+                case 0: local_group<T, 0>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 1: local_group<T, 1>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 2: local_group<T, 2>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 3: local_group<T, 3>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 4: local_group<T, 4>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 5: local_group<T, 5>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                case 6: local_group<T, 6>(F, idx0, hb.y, W, pbl, ar, ai); break;
+                default: local_group<T, 7>(F, idx0, hb.y, W, pbl, ar, ai); break;
             }
             i = i_end;
             continue;
@@ -241,16 +252,16 @@ __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uin
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                ar[r] += cr[r] * v.x;
-                ai[r] += cr[r] * v.y;
+                ar[r] = dn_fma(cr[r], v.x, ar[r]);
+                ai[r] = dn_fma(cr[r], v.y, ai[r]);
             }
         } else if (gh.z == 2u) {   // imaginary coefficients only
             wht(ci);
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                ar[r] -= ci[r] * v.y;
-                ai[r] += ci[r] * v.x;
+                ar[r] = dn_fma(-ci[r], v.y, ar[r]);
+                ai[r] = dn_fma(ci[r], v.x, ai[r]);
             }
         } else {
             wht(cr);
@@ -258,8 +269,8 @@ __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uin
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 const C v = pb[((uint32_t)r ^ xr) << kThreadBitsD];
-                ar[r] += cr[r] * v.x - ci[r] * v.y;
-                ai[r] += cr[r] * v.y + ci[r] * v.x;
+                ar[r] = dn_fma(-ci[r], v.y, dn_fma(cr[r], v.x, ar[r]));
+                ai[r] = dn_fma(ci[r], v.x, dn_fma(cr[r], v.y, ai[r]));
             }
         }
     }
@@ -538,9 +549,12 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
                 const uint32_t bit = 1u << (kThreadBitsD + j);
                 if (x & bit) mpos |= (uint32_t)__builtin_popcount(x & (bit - 1u)) << (2 * j);
             }
+            uint32_t walsh = 0;   // bit r = parity of r & (bits 9..11 of the common Z part)
+            for (uint32_t r = 0; r < (uint32_t)kR; ++r)
+                walsh |= (uint32_t)(__builtin_popcount(r & (((z_first & ~x) >> kThreadBitsD) & (uint32_t)(kR - 1))) & 1) << r;
             entries.push_back(make_uint4(x & (uint32_t)(kTile - 1), n_follow, 4u, z_first & ~x));
             entries.push_back(make_uint4((uint32_t)pos[0] | (uint32_t)pos[1] << 5 | (uint32_t)pos[2] << 10 | (uint32_t)pos[3] << 15,
-                                         mpos, 0u, 0u));
+                                         mpos, walsh, 0u));
             for (uint32_t i = 0; i < (1u << kx); ++i) {
                 uint32_t dep = 0;   // pdep(i, x)
                 for (int q = 0; q < np; ++q)
