@@ -34,10 +34,18 @@ namespace {
 // 16 warps, every thread a consumer (four warps per scheduler hide the dependent chain of a term: table LDS ->
 // popcount -> sign -> add; with 8 warps and 16 amplitudes per thread the schedulers were 35 % busy); thread 0 also
 // issues the bulk copies -- a source tile is consumed over ~10^5 cycles, so a plain double buffer is enough.
-constexpr int kThreadBitsD = 9;
+#ifndef SYK_DENSE_RBITS
+#define SYK_DENSE_RBITS 3
+#endif
+// Index bits of a tile inside a thread (amplitudes per thread = 2^kRBits; 2^(12 - kRBits) threads).  Measured at N = 48 dense
+// complex128 (plain product): 3 -> 170 ms (16 warps x 8 amplitudes), 2 -> 200 ms (32 warps x 4: twice the warps to hide the
+// per-group chain, but twice the per-group instructions per amplitude).
+constexpr int kRBits = SYK_DENSE_RBITS;
+static_assert(kRBits == 2 || kRBits == 3, "tested shapes: 1024 threads x 4 amplitudes, 512 threads x 8 amplitudes");
+constexpr int kThreadBitsD = 12 - kRBits;
 constexpr int kConsumerThreads = 1 << kThreadBitsD;
 constexpr int kThreads = kConsumerThreads;
-constexpr int kR = 8;                              // amplitudes per thread
+constexpr int kR = 1 << kRBits;                              // amplitudes per thread
 constexpr int kTileLog2D = 12;                     // 512 threads x 8
 constexpr int kTile = 1 << kTileLog2D;
 constexpr int kMiscBytes = 2 * 8 + 40 * 8 + 128 + 2 * 512 * 16;   // barriers, reduction scratch, table buffers
@@ -148,6 +156,7 @@ __device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_
                                             const typename Cx<T>::type* pb, T (&ar)[kR], T (&ai)[kR]) {
     using C = typename Cx<T>::type;
     constexpr int ND = 1 << ((XR & 1) + ((XR >> 1) & 1) + ((XR >> 2) & 1));
+    static_assert(XR < kR, "XR = the r bits of x");
     T fr[ND], fi[ND];
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
@@ -155,7 +164,7 @@ __device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_
         uint32_t delta = 0;
         int dj = 0;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
+        for (int j = 0; j < kRBits; ++j) {
             if (XR & (1 << j)) {
                 if (d & (1 << dj)) delta |= 1u << ((mpos >> (2 * j)) & 3u);
                 ++dj;
@@ -175,7 +184,7 @@ __device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_
         // which of the ND table values: the bits of r inside XR, compacted (compile time)
         int d = 0, dj = 0;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
+        for (int j = 0; j < kRBits; ++j) {
             if (XR & (1 << j)) {
                 if (r & (1 << j)) d |= 1 << dj;
                 ++dj;
@@ -203,6 +212,18 @@ __device__ __forceinline__ void local_group(const uint4* __restrict__ F, uint32_
     }
 }
 
+// uniform branch to the variant for XR = the r bits of x
+template <typename T, int XR>
+__device__ __forceinline__ void dispatch_local(uint32_t xr, const uint4* __restrict__ F, uint32_t idx0, uint32_t mpos,
+                                               uint32_t W, const typename Cx<T>::type* pb, T (&ar)[kR], T (&ai)[kR]) {
+    if constexpr (XR + 1 == kR) {
+        local_group<T, XR>(F, idx0, mpos, W, pb, ar, ai);
+    } else {
+        if (xr == (uint32_t)XR) local_group<T, XR>(F, idx0, mpos, W, pb, ar, ai);
+        else dispatch_local<T, XR + 1>(xr, F, idx0, mpos, W, pb, ar, ai);
+    }
+}
+
 // All groups of one staged table chunk applied to the thread's kR accumulators; `sp` = the staged source tile.
 template <typename T>
 __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uint32_t ne, const typename Cx<T>::type* sp,
@@ -221,16 +242,7 @@ __device__ __forceinline__ void process_chunk(const uint4* __restrict__ ent, uin
             // hb.z = Walsh mask of the r bits of zb: bit r = parity(r & zb's bits 9..11); times the thread's own sign
             const uint32_t W = hb.z ^ (0u - ((uint32_t)__popc(bt & gh.w) & 1u));
             const C* pbl = sp + ((uint32_t)tid ^ (gh.x & (uint32_t)(kConsumerThreads - 1)));
-            switch (gh.x >> kThreadBitsD) {
-                case 0: local_group<T, 0>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 1: local_group<T, 1>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 2: local_group<T, 2>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 3: local_group<T, 3>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 4: local_group<T, 4>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 5: local_group<T, 5>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                case 6: local_group<T, 6>(F, idx0, hb.y, W, pbl, ar, ai); break;
-                default: local_group<T, 7>(F, idx0, hb.y, W, pbl, ar, ai); break;
-            }
+            dispatch_local<T, 0>(gh.x >> kThreadBitsD, F, idx0, hb.y, W, pbl, ar, ai);
             i = i_end;
             continue;
         }
@@ -334,7 +346,8 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_split_kernel(const 
             }
             cur_hi = hi;
         }
-        tbuf[tid] = (uint32_t)tid < ne ? __ldg(p.entries + e0 + tid) : make_uint4(0, 0, 0, 0);
+        for (uint32_t t = (uint32_t)tid; t < (uint32_t)kChunkEntries; t += kThreads)
+            tbuf[t] = t < ne ? __ldg(p.entries + e0 + t) : make_uint4(0, 0, 0, 0);
         __syncthreads();
         if (new_tile) {
             mbar_wait(bar_full, n_loaded & 1u);
@@ -439,12 +452,21 @@ __global__ void __launch_bounds__(kThreads, 1) apply_h_dense_kernel(const DnPara
 
     // table stream: this thread's entry of the chunk being prefetched
     uint32_t ck = 0;                           // chunk whose copy sits in tbuf[ck & 1] after the next barrier
-    uint4 pre;
+    constexpr int kPre = (kChunkEntries + kThreads - 1) / kThreads;   // table entries per thread and chunk
+    uint4 pre[kPre];
     auto fetch = [&](uint32_t c) {             // global -> register (chunk c)
         const uint32_t e0 = __ldg(&p.chunks[c].e0), ne = __ldg(&p.chunks[c].ne);
-        pre = (uint32_t)tid < ne ? __ldg(p.entries + e0 + tid) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int k = 0; k < kPre; ++k) {
+            const uint32_t t = (uint32_t)tid + (uint32_t)k * kThreads;
+            pre[k] = t < ne ? __ldg(p.entries + e0 + t) : make_uint4(0, 0, 0, 0);
+        }
     };
-    auto stash = [&](uint32_t c) { tbuf[(c & 1u) * kChunkEntries + tid] = pre; };
+    auto stash = [&](uint32_t c) {
+#pragma unroll
+        for (int k = 0; k < kPre; ++k)
+            if (tid + k * kThreads < kChunkEntries) tbuf[(c & 1u) * kChunkEntries + tid + k * kThreads] = pre[k];
+    };
     fetch(0);
     stash(0);
     uint32_t g = 0;                            // loads consumed by this CTA: slot g & 1, parity (g >> 1) & 1
@@ -545,7 +567,7 @@ int build_dense_tables(const syk_ham* h, int dtype, DenseCache& dc) {
             for (int q = 0; q < 32; ++q)
                 if (x & (1u << q)) pos[np++] = q;
             uint32_t mpos = 0;   // index bit of r bit j (index bit 9 + j of the vector), if x contains it
-            for (int j = 0; j < 3; ++j) {
+            for (int j = 0; j < kRBits; ++j) {
                 const uint32_t bit = 1u << (kThreadBitsD + j);
                 if (x & bit) mpos |= (uint32_t)__builtin_popcount(x & (bit - 1u)) << (2 * j);
             }
