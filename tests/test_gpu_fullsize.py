@@ -337,3 +337,53 @@ def test_dense_table_kernel_multichunk_sampled(B, N, n_samples):
             rel = float(torch.linalg.vector_norm(a - b) / torch.linalg.vector_norm(a))
             assert rel <= (1e-13 if code == B.SYK_C128 else 2e-6), rel
         del d_in, d_out, wk
+
+
+@pytest.mark.parametrize("N,k,dt,need_gb", [(56, 4, "c128", 20), (64, 2, "c64", 112)])
+def test_fused_lanczos_fullsize_sampled_vs_oracle(B, N, k, dt, need_gb):
+    """The FUSED launches bench.py times (scatter-tile kernel, relabelled handle, epilogue out = H u_j/|u_j| - (|u_j|/|u_{j-1}|)
+    u_{j-1} with the operands staged through the ring) against the oracle's monomial rows at
+    the headline sizes: two fused Lanczos steps in the one-pass layout (u_2, u_3 = the two work vectors), sampled outputs
+    incl. the edges of the first / last tiles:
+        u_2 = H u_1/|u_1| - alpha_1 u_1/|u_1| ;   u_3 = H u_2/|u_2| - (|u_2|/|u_1|) u_1 - alpha_2 u_2/|u_2| ."""
+    import torch
+    if _free_gb() < need_gb:
+        pytest.skip(f"needs {need_gb} GB of device memory")
+    tdt = torch.complex128 if dt == "c128" else torch.complex64
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    tol = 1e-10 if dt == "c128" else 1e-5
+    D = 1 << (N // 2)
+    p = inputs.bernoulli_p(N, k)
+    q, J, _ = orng.sample_couplings(N, p, 0, 0)
+    h = B.syk_build_hamiltonian(N, p, 0, 0)
+    perm = list(B.syk_ham_optimize_layout(h, code)["perm"])
+    B.syk_ham_prepare(h, code)
+    assert B.syk_apply_H_kernel_kind(h, code) == 3
+    scratch = torch.empty(B.syk_reduce_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    m = 2
+    wk = torch.empty(B.syk_krylov_workspace_bytes(h, code, {"krylov_dim": m}), dtype=torch.uint8, device="cuda")
+    psi = torch.empty(D, dtype=tdt, device="cuda")
+    B.syk_random_state_h(h, 0, 0, psi, scratch)
+    alpha, beta, _ = B.syk_lanczos_run(h, psi, m, wk)
+    hdr = wk.numel() - m * D * psi.element_size()
+    vecs = wk[hdr:].view(tdt).view(m, D)
+    idx = inputs.sample_indices(D, 600, seed=23)
+    edge = np.array([0, 1, 8191, 8192, 16383, 16384, D // 2 - 1, D // 2, D - 16385, D - 16384, D - 8193, D - 1], dtype=np.uint64)
+    inv = np.argsort(np.array(perm))
+    idx = np.unique(np.concatenate([idx, edge, _storage_index(edge, inv)]))
+    sidx = torch.from_numpy(_storage_index(idx, perm).astype(np.int64)).cuda()
+    u1 = psi[sidx].cpu().numpy().astype(np.complex128)
+    u2 = vecs[0][sidx].cpu().numpy().astype(np.complex128)
+    u3 = vecs[1][sidx].cpu().numpy().astype(np.complex128)
+    Hu1 = _oracle_samples(N, q, J, idx, psi, perm)
+    ref2 = Hu1 / beta[0] - alpha[0] * u1 / beta[0]
+    assert np.linalg.norm(u2 - ref2) / np.linalg.norm(ref2) <= 2 * tol, (N, dt)
+    assert np.max(np.abs(u2 - ref2)) <= 20 * tol * np.sqrt(np.mean(np.abs(ref2) ** 2))
+    Hu2 = _oracle_samples(N, q, J, idx, vecs[0], perm)
+    ref3 = Hu2 / beta[1] - (beta[1] / beta[0]) * u1 - alpha[1] * u2 / beta[1]
+    assert np.linalg.norm(u3 - ref3) / np.linalg.norm(ref3) <= 4 * tol, (N, dt)
+    assert np.max(np.abs(u3 - ref3)) <= 40 * tol * np.sqrt(np.mean(np.abs(ref3) ** 2))
+    # Lanczos identities with the oracle-checked vectors: beta_2 = |u_2|, alpha_1 real part of <u_1|H u_1> / |u_1|^2
+    assert abs(beta[0] - 1.0) <= 1e-12 and beta[1] > 0.0
+    n2 = B.syk_dot(N, vecs[0], vecs[0], scratch).real
+    assert abs(np.sqrt(n2) / beta[1] - 1.0) <= (1e-12 if dt == "c128" else 1e-6)
