@@ -388,6 +388,9 @@ int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset);
  *   kind 6: do global loads share the shared-memory data path?  256 threads per SM; per iteration (arg0 of them) every
  *           thread issues 16 LDG.128 (ld.global.cg, 64 KiB of d_buf per CTA and iteration; d_buf = NULL: none) and arg1 x 16
  *           LDS.128 over a staged 64 KiB chunk, one FP64 FMA pair per value.
+ *   kind 7: distributed shared memory: clusters of two CTAs, 256 threads each; per iteration (arg0 of them) every thread reads 16
+ *           16-byte elements of a staged 64 KiB chunk through the shared::cluster window of its own CTA (arg1 = 0) or of the
+ *           peer CTA (arg1 = 1: SM-to-SM).  [3] = bytes read; rate per SM = [3] / SMs used (an even number) / [1].
  * result[6]: [0] = device time in ms (CUDA events), [1] = SM cycles of the slowest CTA (clock64), [2] = bytes copied
  * into shared memory (kinds 0, 2; kind 5: by the even CTAs), thread-level adds (kinds 3, 4) or bytes loaded by LDG (kind 6),
  * [3] = bytes read by LDS (kinds 1, 2, 6; kind 5: bytes copied by the odd CTAs), [4] / [5] = cycles of the slowest even / odd CTA.

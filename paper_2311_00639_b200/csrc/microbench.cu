@@ -234,6 +234,54 @@ __global__ void __launch_bounds__(256, 1) mb_ldg_kernel(const double2* __restric
     if (tid == 0) cycles[blockIdx.x] = t1 - t0;
 }
 
+// Distributed shared memory: clusters of two CTAs (two SMs); every thread reads 16-byte elements of a staged 64 KiB chunk with
+// the consumers' access pattern through the shared::cluster window -- of its OWN CTA (remote = 0) or of the PEER CTA (remote =
+// 1: SM-to-SM reads).  What a 2-CTA variant of the scatter-tile kernel (one 256 KiB tile pair per cluster) would pay for the
+// half of its reads that land in the peer's shared memory.
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(256, 1)
+mb_dsmem_kernel(int iters, int remote, double2* sink, unsigned long long* cycles) {
+    extern __shared__ __align__(128) unsigned char mb_smem[];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < 65536 / 16; i += 256) reinterpret_cast<double2*>(mb_smem)[i] = make_double2(1.0, 0.5);
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    const uint32_t local = smem_u32(mb_smem) + (uint32_t)tid * 16u;
+    uint32_t base;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(base) : "r"(local), "r"(remote ? rank ^ 1u : rank));
+    double ar[16], ai[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        ar[r] = 0.0;
+        ai[r] = 0.0;
+    }
+    const unsigned long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+        double2 v[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+            asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];"
+                         : "=d"(v[r].x), "=d"(v[r].y)
+                         : "r"(base + (((uint32_t)r ^ ((uint32_t)it & 15u)) << 12)));
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            ar[r] = __fma_rn(1.0000001, v[r].x, ar[r]);
+            ai[r] = __fma_rn(1.0000001, v[r].y, ai[r]);
+        }
+    }
+    const unsigned long long t1 = clock64();
+    // the peer may still be reading this CTA's shared memory
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        sr += ar[r];
+        si += ai[r];
+    }
+    sink[(size_t)blockIdx.x * 256 + tid] = make_double2(sr, si);
+    if (tid == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
 }  // namespace
 }  // namespace syk
 
@@ -330,6 +378,26 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
             }
             units = d_buf ? (double)sms * arg0 * 65536.0 : 0.0;       // bytes by global loads
             units2 = (double)sms * arg0 * (double)arg1 * 65536.0;     // bytes by LDS
+            count_launch();
+        }
+    } else if (kind == 7) {
+        // arg0 = iterations, arg1 = 0: own shared memory through the cluster window, 1: the peer CTA's (DSMEM)
+        if (arg0 < 1 || (arg1 != 0 && arg1 != 1)) rc = SYK_EINVAL;
+        if (rc == SYK_OK) {
+            const int grid = sms & ~1;   // whole clusters of two
+            cudaError_t e = cudaFuncSetAttribute(mb_dsmem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+            if (e == cudaSuccess) e = cudaMemsetAsync(d_cycles, 0, sizeof(unsigned long long) * (size_t)sms, st);
+            if (e == cudaSuccess) {
+                cudaEventRecord(e0, st);
+                mb_dsmem_kernel<<<grid, 256, 65536, st>>>(arg0, arg1, (double2*)d_sink, d_cycles);
+                cudaEventRecord(e1, st);
+                e = cudaGetLastError();
+            }
+            if (e != cudaSuccess) {
+                set_cuda_error(e, "mb_dsmem_kernel");
+                rc = SYK_ECUDA;
+            }
+            units2 = (double)grid * arg0 * 65536.0;   // bytes read through the cluster window
             count_launch();
         }
     } else {

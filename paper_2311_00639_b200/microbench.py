@@ -70,6 +70,14 @@ def measure(quick=False):
             d["lds_B_per_clk_per_SM"] = r["lds_bytes"] / sms / r["cycles"]
             d["lds_TB_per_s"] = r["lds_bytes"] / (r["ms"] * 1e-3) / 1e12
         out[name] = d
+    # distributed shared memory (kind 7): the consumers' reads from the own CTA and from the peer CTA of a 2-CTA cluster
+    for name, remote in (("dsmem_own_cta", 0), ("dsmem_peer_cta", 1)):
+        B.syk_microbench(7, it6 // 8, remote, None, wk)
+        r = B.syk_microbench(7, it6, remote, None, wk)
+        n_used = sms & ~1
+        out[name] = {"ms": r["ms"], "cycles": r["cycles"], "sm_mhz_effective": r["cycles"] / (r["ms"] * 1e-3) / 1e6,
+                     "lds_B_per_clk_per_SM": r["lds_bytes"] / n_used / r["cycles"],
+                     "lds_TB_per_s": r["lds_bytes"] / (r["ms"] * 1e-3) / 1e12}
     iters = 4000 if quick else 20000
     for name, kind in (("fp64_add", 3), ("dense_term_sequence", 4)):
         B.syk_microbench(kind, iters // 8, 0, None, wk)
