@@ -28,6 +28,31 @@ def string_matrix(L, x, z, c=1.0):
     return complex(c) * m
 
 
+def apply_string(L, x, z, c, v):
+    """c * (x)_q Z^{z_q} X^{x_q} applied to the vector v of 2^L amplitudes WITHOUT forming the 2^L x 2^L matrix: the vector is
+    viewed as an L-index tensor (index q = qubit q) and the 2 x 2 factor of every site is contracted with its own index --
+    the Kronecker product of PAPER.md:259 applied factor by factor (for vectors too long for `string_matrix`; pinned against
+    it in tests/test_oracle_pins.py)."""
+    t = np.asarray(v, dtype=np.complex128).reshape((2,) * L)      # C order: axis a = qubit L - 1 - a
+    for q in range(L):
+        site = I2
+        if (z >> q) & 1:
+            site = site @ SZ
+        if (x >> q) & 1:
+            site = site @ SX
+        if site is not I2:
+            t = np.moveaxis(np.tensordot(site, t, axes=([1], [L - 1 - q])), 0, L - 1 - q)
+    return complex(c) * t.reshape(-1)
+
+
+def apply_sum(L, terms, v):
+    """sum of apply_string over terms (x, z, c)."""
+    out = np.zeros(1 << L, dtype=np.complex128)
+    for x, z, c in terms:
+        out += apply_string(L, int(x), int(z), c, v)
+    return out
+
+
 def sum_matrix(L, terms):
     """terms: iterable of (x, z, c)."""
     H = np.zeros((1 << L, 1 << L), dtype=np.complex128)

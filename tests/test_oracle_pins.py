@@ -538,3 +538,22 @@ def test_paper_statements_fixture_is_what_the_oracle_uses():
         assert ("2 delta" in stm[key]) == (scale == 2.0)
         g = majorana.jw_gammas(6, gn)
         assert np.allclose(g[1] @ g[1] + g[1] @ g[1], scale * np.eye(8)) and np.allclose(g[0] @ g[3] + g[3] @ g[0], 0)
+
+
+def test_P15_apply_string_equals_string_matrix():
+    """pauli.apply_string (site factors contracted one by one) against the Kronecker-product matrix of the same string, for
+    every (x, z) on 3 qubits and random strings on 7 qubits; apply_sum against sum_matrix; Z X = iY on one site."""
+    rs = np.random.default_rng(5)
+    L = 3
+    v = rs.standard_normal(8) + 1j * rs.standard_normal(8)
+    for x in range(8):
+        for z in range(8):
+            assert np.allclose(pauli.apply_string(L, x, z, 0.5 - 2j, v), pauli.string_matrix(L, x, z, 0.5 - 2j) @ v, atol=1e-14)
+    L = 7
+    v = rs.standard_normal(128) + 1j * rs.standard_normal(128)
+    terms = [(int(rs.integers(0, 128)), int(rs.integers(0, 128)), complex(rs.standard_normal(), rs.standard_normal()))
+             for _ in range(12)]
+    assert np.allclose(pauli.apply_sum(L, terms, v), pauli.sum_matrix(L, terms) @ v, atol=1e-13)
+    e0, e1 = np.array([1.0, 0.0]), np.array([0.0, 1.0])
+    assert np.allclose(pauli.apply_string(1, 1, 1, 1.0, e0), -e1)            # Z X |0> = Z |1> = -|1> = (iY)|0>
+    assert np.allclose(pauli.apply_string(1, 1, 1, 1.0, e1), e0)             # Z X |1> = |0>     = (iY)|1>
