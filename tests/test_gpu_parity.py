@@ -1402,3 +1402,53 @@ def test_dense_local_groups_canonical_and_relabelled(B, torch, dt):
     d_out = torch.empty_like(d_in)
     B.syk_apply_H(h, d_in, d_out)
     assert relerr(d_out.cpu().numpy(), ohm.matvec_sequential(N, q, J, v.astype(np.complex128))) <= TOL[dt]
+
+
+@pytest.mark.parametrize("dt", ["c128", "c64"])
+def test_dense_local_groups_generic_pauli_strings(B, torch, dt):
+    """x-local groups beyond what SYK produces (generic Pauli sums): X-masks of 1, 2, 3 and 4 qubits placed on
+    thread bits, on the per-thread index bits 9..11 and above the 4096-amplitude tile, all or some of the 2^k Z-patterns on the
+    flipped qubits, one common Z-pattern elsewhere, real and imaginary coefficients in one group.  Groups with >= 4 terms go
+    through the table lookup, the others through the term-by-term walk; apply_H against the oracle's factor-by-factor
+    application of every string (oracle.pauli.apply_sum)."""
+    from oracle import pauli as opauli
+    code = B.SYK_C128 if dt == "c128" else B.SYK_C64
+    L, D = 14, 1 << 14
+    rs = np.random.default_rng(33)
+    masks = [0b1 << 3, 0b1 << 10, 0b1 << 13,                                            # one qubit (2 terms: walked)
+             (1 << 2) | (1 << 7), (1 << 5) | (1 << 9), (1 << 11) | (1 << 12), (1 << 10) | (1 << 11),
+             (1 << 0) | (1 << 4) | (1 << 8), (1 << 6) | (1 << 9) | (1 << 13), (1 << 9) | (1 << 10) | (1 << 11),
+             (1 << 1) | (1 << 3) | (1 << 5) | (1 << 7), (1 << 8) | (1 << 9) | (1 << 12) | (1 << 13),
+             (1 << 2) | (1 << 10) | (1 << 11) | (1 << 12), (1 << 9) | (1 << 10) | (1 << 11) | (1 << 13)]
+    terms, n_local = [], 0
+    for gi, x in enumerate(masks):
+        bits = [q for q in range(L) if (x >> q) & 1]
+        z_out = int(rs.integers(0, D)) & ~x
+        pats = list(range(1 << len(bits)))
+        if gi % 3 == 1 and len(pats) > 4:
+            pats = sorted(rs.choice(pats, size=len(pats) - 3, replace=False).tolist())   # an incomplete set of Z-patterns
+        if len(pats) >= 4:
+            n_local += 1
+        for pz in pats:
+            z = z_out | sum(1 << bits[j] for j in range(len(bits)) if (pz >> j) & 1)
+            a = float(rs.standard_normal())
+            terms.append((x, z, a * (1j if rs.integers(0, 2) else 1.0)))
+    # a second group on an X-mask of the list whose Z-patterns differ OUTSIDE x: not local, must be walked
+    x = masks[4]
+    for _ in range(6):
+        terms.append((x | (1 << 1), int(rs.integers(0, D)), float(rs.standard_normal())))
+    h = B.syk_build_from_pauli_strings(L, terms)
+    B.syk_set_apply_H_kernel(h, 4)
+    assert B.syk_apply_H_kernel_kind(h, code) == 4
+    assert B.syk_apply_H_dense_info(h, code)["n_local_groups"] == n_local
+    v = (rs.standard_normal(D) + 1j * rs.standard_normal(D)).astype(npdtype(dt))
+    d_in = to_dev(torch, v)
+    d_out = torch.full((D,), complex(float("nan"), float("nan")), dtype=d_in.dtype, device="cuda")
+    B.syk_apply_H(h, d_in, d_out)
+    ref = opauli.apply_sum(L, terms, v.astype(np.complex128))
+    assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt]
+    # the same operator term by term (generic kernel): the two CUDA paths agree as well
+    B.syk_set_apply_H_kernel(h, 0)
+    d_gen = torch.empty_like(d_out)
+    B.syk_apply_H(h, d_in, d_gen)
+    assert relerr(d_gen.cpu().numpy(), ref) <= TOL[dt]
