@@ -18,7 +18,11 @@
 // one, mbarrier completion); the table (a few MB, streamed once per output tile) is staged chunk by chunk in shared
 // memory by the threads themselves, double buffered, so the inner loops read it with broadcast LDS (read from global
 // with warp-uniform addresses, each term cost an exposed L2 latency: 1120 ms per N = 48 matvec).
-// History at N = 48 dense complex128: generic kernel 2390 ms; 8 warps x 16 amplitudes 692 ms; this shape 450 ms.
+// Groups whose Z-masks agree outside their own X-mask (every four-qubit X-mask of a dense SYK Hamiltonian) skip the binning
+// altogether: one table of 2^popcount(x) coefficient sums per group, one lookup and one complex multiply-add per amplitude
+// (local_group below).
+// History at N = 48 dense complex128: generic kernel 2390 ms; 8 warps x 16 amplitudes 692 ms; this shape 450 ms; with the
+// x-local groups 178 ms (0.24 of the FP64 issue rate: latency-bound, profiles/r2_N48_dense_c128.md).
 // No atomics on data, one write per output: bitwise reproducible.  Fused Lanczos epilogue as in apply_h.cu.
 #include <algorithm>
 #include <cstring>
