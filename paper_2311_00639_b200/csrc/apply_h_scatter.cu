@@ -34,7 +34,8 @@
 // by a uniform branch on the two low slice bits of z (accumulate_chunk).  Per-term data comes from the __grid_constant__
 // table (constant bank), the next entry fetched one term ahead.  No atomics on data, one write per output: bitwise
 // reproducible.  ~100 warp instructions per (term, chunk of 16 slices) instead of ~150 with a per-slice sign walk; what
-// the launch is bound by is the supply of tiles (DRAM phases and L2 phases of the lock-stepped CTAs hardly overlap; a
+// the launch is bound by is the shared-memory data path (every term reads the staged tile once, every load fills it once:
+// 134 B/clk/SM at N = 56; syk_apply_H_trace, profiles/r2_chunk_trace.md), plus waits for the loads that miss in L2 (a
 // staggered start of the CTAs -- each walks the list rotated by a few places -- spreads the misses: -6 % at N = 64; L2
 // prefetching by the TMA unit or by prefetch.global.L2, of every load or only of the loads that must miss, 1..12 loads
 // ahead, made every configuration slower: DESIGN.md section 6).
