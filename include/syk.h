@@ -376,7 +376,7 @@ int syk_profile_read(double* apply_h_ms, int64_t* apply_h_launches, int reset);
  * peak is known, the L2 -> SM, shared-memory and ALU-issue peaks of this box are not).  One launch of 1 CTA per SM:
  *   kind 0: every CTA streams arg0 chunks of 64 KiB from d_buf (walked pseudo-randomly; a buffer of <= 32 MB stays in
  *           L2, a multi-GB one streams from DRAM) into the 3-chunk shared-memory ring of the scatter-tile kernel with
- *           cp.async.bulk, no arithmetic;
+ *           cp.async.bulk, no arithmetic; arg1 > 0: only arg1 CTAs (SMs) stream (per-SM rate below the chip-wide L2 limit);
  *   kind 1: no copies; the 8 consumer warps make arg1 passes over each of arg0 staged chunks with the kernel's
  *           XOR-permuted LDS.128 + 2 FP64 FMA per element;
  *   kind 2: both at once (arg1 passes over every chunk that arrives);

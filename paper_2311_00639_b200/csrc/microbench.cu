@@ -313,6 +313,8 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
         while (((size_t)2 << buf_log2) <= buf_bytes) ++buf_log2;
         if (kind != 1 && (!d_buf || buf_log2 < 17 || ((uintptr_t)d_buf & 127))) rc = SYK_EINVAL;
         if (arg0 < 1 || arg1 < 0) rc = SYK_EINVAL;
+        // kind 0: arg1 > 0 limits the launch to arg1 CTAs (per-SM rate when only some SMs pull from L2)
+        const int grid = kind == 0 && arg1 > 0 && arg1 < sms ? arg1 : sms;
         if (rc == SYK_OK) {
             MbParams p;
             p.buf = (const unsigned char*)d_buf;
@@ -328,7 +330,8 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
             cudaError_t e = cudaFuncSetAttribute(mb_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e == cudaSuccess) {
                 cudaEventRecord(e0, st);
-                mb_stream_kernel<<<sms, kMbThreads, smem, st>>>(p);
+                cudaMemsetAsync(d_cycles, 0, sizeof(unsigned long long) * (size_t)sms, st);
+                mb_stream_kernel<<<grid, kMbThreads, smem, st>>>(p);
                 cudaEventRecord(e1, st);
                 e = cudaGetLastError();
             }
@@ -336,7 +339,7 @@ int syk_microbench(int kind, int arg0, int arg1, const void* d_buf, size_t buf_b
                 set_cuda_error(e, "mb_stream_kernel");
                 rc = SYK_ECUDA;
             }
-            units = p.load ? (double)sms * arg0 * (double)kMbChunk : 0.0;                       // bytes L2/DRAM -> smem
+            units = p.load ? (double)grid * arg0 * (double)kMbChunk : 0.0;                      // bytes L2/DRAM -> smem
             units2 = (double)sms * arg0 * (double)p.terms_per_chunk * (double)kMbChunk;         // bytes read by LDS
             if (kind == 5) {   // bytes of the even (whole buffer) and of the odd (L2-resident region) group
                 units = (double)((sms + 1) / 2) * arg0 * (double)kMbChunk;

@@ -36,6 +36,12 @@ def measure(quick=False):
         return d
 
     out["l2_to_sm"] = stream(0, n, 0, small)
+    for ctas in (74, 37, 8):                                                 # fewer SMs pulling: the per-SM limit
+        B.syk_microbench(0, 256, ctas, small, wk)
+        r = B.syk_microbench(0, n, ctas, small, wk)
+        out[f"l2_to_sm_{ctas}_ctas"] = {"ms": r["ms"], "cycles": r["cycles"], "load_B_per_clk_per_SM": r["units"] / ctas / r["cycles"],
+                                        "load_TB_per_s": r["units"] / (r["ms"] * 1e-3) / 1e12,
+                                        "sm_mhz_effective": r["cycles"] / (r["ms"] * 1e-3) / 1e6}
     out["lds_only"] = stream(1, n // 8, 8, None)
     for t in (1, 2, 3, 4):
         out[f"l2_and_lds_{t}"] = stream(2, n // 2, t, small)
