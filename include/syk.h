@@ -339,15 +339,18 @@ int syk_apply_H_dense_info(const syk_ham* h, int dtype, int* n_loads, int* n_chu
 int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,
                        uint32_t* window_mask);
 /* Diagnostic (measure, don't guess): one plain product out = H in through the scatter-tile kernel (kind 3, else SYK_EINVAL)
- * in which persistent CTA `cta` records, for the `round`-th output tile it owns, three SM-clock stamps per ring chunk:
+ * in which persistent CTA `cta` records, for the `round`-th output tile it owns, seven SM-clock stamps per ring chunk:
  * clk[v] = the producer issued the bulk copies of chunk v, clk[n + v] = the first consumer warp asked for chunk v,
- * clk[2 n + v] = it got it; v = list position * 2 + chunk, n = 2 * n_loads (clk_capacity >= 3 n).  So
+ * clk[2 n + v] = it got it, clk[3 n + v] = it had decoded the chunk's first term (the LDS stream follows), clk[4 n + v] = it
+ * had issued the first term, clk[5 n + v] = all terms, clk[6 n + v] = it had arrived on the chunk's empty-barrier;
+ * v = list position * 2 + chunk, n = 2 * n_loads (clk_capacity >= 7 n).  detail = 0 records the first three only (the others
+ * stay 0): every stamp costs the traced warp time, and the seven-stamp build lengthens a chunk by ~200 clocks.  So
  * clk[2n + v] - clk[n + v] is the time the consumers waited for data and clk[n + v + 1] - clk[2n + v] the time they
  * worked on chunk v.  List position li of this CTA holds load (li + rot) % n_loads; load_terms[l] / load_xo[l] = number of
  * terms / the part of the X-mask outside the tile bits of load l (load_capacity >= n_loads).  Unlike every other compute
  * call this one allocates (and frees) a small device buffer and synchronises `stream`.  Results of `out` are those of
  * syk_apply_H. */
-int syk_apply_H_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, uint64_t* clk,
+int syk_apply_H_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, int detail, uint64_t* clk,
                       int clk_capacity, int32_t* load_terms, uint32_t* load_xo, int load_capacity, int* n_loads, int* rot,
                       void* stream);
 /* Pacing of the register-tile / scatter-tile kernels' persistent CTAs (process-wide; a tuning knob, results do not depend on it):

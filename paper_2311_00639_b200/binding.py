@@ -106,7 +106,7 @@ _SIGNATURES = {
     "syk_set_lockstep": (_i, [_i, _i]),
     "syk_set_cuda_graphs": (_i, [_i]),
     "syk_apply_H_layout": (_i, [_vp, _i, _P(_i), _P(_i), _P(_u32), _P(_u32)]),
-    "syk_apply_H_trace": (_i, [_vp, _i, _vp, _vp, _i, _i, _vp, _i, _vp, _vp, _i, _P(_i), _P(_i), _vp]),
+    "syk_apply_H_trace": (_i, [_vp, _i, _vp, _vp, _i, _i, _i, _vp, _i, _vp, _vp, _i, _P(_i), _P(_i), _vp]),
     "syk_launch_count": (_i64, [_i]),
     "syk_microbench_workspace_bytes": (_sz, []),
     "syk_microbench": (_i, [_i, _i, _i, _vp, _sz, _vp, _sz, _P(_d), _vp]),
@@ -569,20 +569,21 @@ def syk_apply_H_layout(h, dtype):
     return {"n_loads": nl.value, "n_passes": npass.value, "tile_mask": tm.value, "window_mask": wm.value}
 
 
-def syk_apply_H_trace(h, d_in, d_out, cta=0, round=2, stream=None):
+def syk_apply_H_trace(h, d_in, d_out, cta=0, round=2, detail=0, stream=None):
     """One plain scatter-tile product with the timeline of one persistent CTA (include/syk.h).  Returns a dict with the
-    clock stamps per ring chunk (issue, before_wait, after_wait), the load list (terms, xo per load) and the CTA's rotation."""
+    clock stamps per ring chunk (issue, before_wait, after_wait, first_decoded, first_issued, all_issued, arrived), the load list (terms, xo per load) and the CTA's rotation."""
     n_loads_max = 1024
-    clk = np.zeros(3 * 2 * n_loads_max, dtype=np.uint64)
+    clk = np.zeros(7 * 2 * n_loads_max, dtype=np.uint64)
     terms = np.zeros(n_loads_max, dtype=np.int32)
     xo = np.zeros(n_loads_max, dtype=np.uint32)
     nl, rot = _i(), _i()
-    _check(_lib.syk_apply_H_trace(_h(h), dtype_code(d_in), _dptr(d_in), _dptr(d_out), int(cta), int(round),
+    _check(_lib.syk_apply_H_trace(_h(h), dtype_code(d_in), _dptr(d_in), _dptr(d_out), int(cta), int(round), int(detail),
                                   clk.ctypes.data, len(clk), terms.ctypes.data, xo.ctypes.data, n_loads_max,
                                   ctypes.byref(nl), ctypes.byref(rot), _stream(stream)), "syk_apply_H_trace")
     n = 2 * nl.value
     c = clk.astype(np.int64)
-    return {"n_loads": nl.value, "rot": rot.value, "issue": c[:n], "before_wait": c[n:2 * n], "after_wait": c[2 * n:3 * n],
+    return {"n_loads": nl.value, "rot": rot.value, "issue": c[:n], "before_wait": c[n:2 * n], "after_wait": c[2 * n:3 * n], "first_decoded": c[3 * n:4 * n], "first_issued": c[4 * n:5 * n], "all_issued": c[5 * n:6 * n],
+            "arrived": c[6 * n:7 * n],
             "load_terms": terms[:nl.value].copy(), "load_xo": xo[:nl.value].copy()}
 
 

@@ -662,7 +662,7 @@ int syk_apply_H_layout(const syk_ham* h, int dtype, int* n_loads, int* n_passes,
     return syk::scatter_layout_info(h, dtype, n_loads, n_passes, tile_mask, window_mask);
 }
 
-int syk_apply_H_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, uint64_t* clk,
+int syk_apply_H_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, int detail, uint64_t* clk,
                       int clk_capacity, int32_t* load_terms, uint32_t* load_xo, int load_capacity, int* n_loads, int* rot,
                       void* stream) {
     if (!h || !d_in || !d_out || !clk || !load_terms || !load_xo || !n_loads || !rot ||
@@ -674,7 +674,7 @@ int syk_apply_H_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out
     if (a < b + bytes && b < a + bytes) return SYK_EINVAL;
     if (syk::apply_h_kernel_kind(h, dtype) != 3) return SYK_EINVAL;
     SYK_TRY(syk::ensure_device_tables(h));
-    return syk::scatter_trace(h, dtype, d_in, d_out, cta, round, clk, clk_capacity, load_terms, load_xo, load_capacity,
+    return syk::scatter_trace(h, dtype, d_in, d_out, cta, round, detail != 0, clk, clk_capacity, load_terms, load_xo, load_capacity,
                               n_loads, rot, (cudaStream_t)stream);
 }
 

@@ -88,9 +88,10 @@ struct StParams {
     int epoch_len;
     int lag;
     int stagger;      // CTA i walks the load list of its tiles rotated by (37 i) mod stagger places (0 = all in phase)
-    // diagnostic timeline (syk_apply_H_trace; nullptr otherwise): CTA trace_cta records, for its trace_round-th tile, three
-    // clock64 stamps per ring chunk v = list position * NC + chunk: [v] producer issue, [n + v] consumer before the wait for
-    // the chunk, [2 n + v] after it, n = n_loads * NC
+    // diagnostic timeline (syk_apply_H_trace; nullptr otherwise): CTA trace_cta records, for its trace_round-th tile, seven
+    // clock64 stamps per ring chunk v = list position * NC + chunk (n = n_loads * NC): [v] producer issue; thread 0 of the
+    // consumers: [n + v] before the wait for the chunk, [2 n + v] after it, [3 n + v] first term decoded (its LDS stream is
+    // next), [4 n + v] first term issued, [5 n + v] all terms issued, [6 n + v] arrived on the empty-barrier
     unsigned long long* trace;
     int trace_cta, trace_round;
 };
@@ -219,7 +220,7 @@ __device__ __forceinline__ void dispatch_chunk(uint32_t oc, uint32_t variant, ui
     }
 }
 
-template <typename T, int NR, int LRC, bool FUSED, bool TRACE = false>
+template <typename T, int NR, int LRC, bool FUSED, int TRACE = 0>   // TRACE: 0 off, 1 three stamps per chunk, 2 seven
 __global__ void __launch_bounds__(kThreads, 1)
 apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p) {
     using C = typename Cx<T>::type;
@@ -277,7 +278,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             uint32_t base = 0;
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
-            const bool tr = TRACE && p.trace && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
+            const bool tr = TRACE != 0 && p.trace && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
             for (int li = 0; li < n_loads; ++li) {
                 int l = li + rot;
                 if (l >= n_loads) l -= n_loads;
@@ -293,7 +294,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     mbar_wait(bar_empty + 8 * pos, phase ^ 1u);
-                    if constexpr (TRACE) if (tr) p.trace[li * NC + c] = clock64();
+                    if constexpr (TRACE != 0) if (tr) p.trace[li * NC + c] = clock64();
                     mbar_arrive_expect_tx(bar_full + 8 * pos, CHUNK_BYTES);
 #pragma unroll
                     for (int u = 0; u < RC / kRun; ++u)
@@ -344,7 +345,7 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
             for (int i = 0; i < n_outer; ++i) base |= ((tile >> i) & 1u) << tab.outer_pos[i];
             const uint32_t bt = base | ((uint32_t)tid << (TB - 8));   // index of the element's first amplitude, r bits 0
             const uint32_t stage_base = smem_u32(smem), tid16 = (uint32_t)tid << 4;
-            const bool tr = TRACE && p.trace && tid == 0 && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
+            const bool tr = TRACE != 0 && p.trace && tid == 0 && (int)blockIdx.x == p.trace_cta && (int)(tile / gridDim.x) == p.trace_round;
             T ar[R * PAIR], ai[R * PAIR];
 #pragma unroll
             for (int r = 0; r < R * PAIR; ++r) {
@@ -356,9 +357,9 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                 if (l >= n_loads) l -= n_loads;
                 const int t0 = tab.load_t0[l], t1 = tab.load_t0[l + 1];
                 for (uint32_t c = 0; c < (uint32_t)NC; ++c) {
-                    if constexpr (TRACE) if (tr) p.trace[(n_loads + li) * NC + c] = clock64();
+                    if constexpr (TRACE != 0) if (tr) p.trace[(n_loads + li) * NC + c] = clock64();
                     mbar_wait(bar_full + 8 * pos, phase);
-                    if constexpr (TRACE) if (tr) p.trace[(2 * n_loads + li) * NC + c] = clock64();
+                    if constexpr (TRACE != 0) if (tr) p.trace[(2 * n_loads + li) * NC + c] = clock64();
                     const uint32_t cp = stage_base + (uint32_t)pos * CHUNK_BYTES + tid16;
                     uint4 e = tab.term[t0];
                     for (int t = t0; t < t1; ++t) {
@@ -376,11 +377,15 @@ apply_h_scatter_kernel(const __grid_constant__ StTable tab, const StParams<T> p)
                             variant |= (e.x & 1u) << 3;            // the mask flips index bit 0: the pair arrives swapped
                             aux = (e.y & 1u) << 31;                // second amplitude of the pair: index bit 0 set
                         }
+                        if constexpr (TRACE == 2) if (tr && t == t0) p.trace[(3 * n_loads + li) * NC + c] = clock64();
                         dispatch_chunk<T, R, RC, 0>(oc, variant, pb, xr & lo, (zr & lo) >> 2, aux, w, ar, ai);
+                        if constexpr (TRACE == 2) if (tr && t == t0) p.trace[(4 * n_loads + li) * NC + c] = clock64();
                         e = en;
                     }
+                    if constexpr (TRACE == 2) if (tr) p.trace[(5 * n_loads + li) * NC + c] = clock64();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_empty + 8 * pos);
+                    if constexpr (TRACE == 2) if (tr) p.trace[(6 * n_loads + li) * NC + c] = clock64();
                     if (++pos == nring) {
                         pos = 0;
                         phase ^= 1u;
@@ -684,10 +689,14 @@ int launch_st(const syk_ham* h, const StTable& tab, const void* d_in, void* d_ou
         SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, true>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         apply_h_scatter_kernel<T, NR, LRC, true><<<grid, kThreads, smem, stream>>>(tab, p);
-    } else if (fa.trace) {   // diagnostic build of the plain kernel (syk_apply_H_trace): clock stamps per ring chunk
-        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false, true>,
+    } else if (fa.trace && fa.trace_detail) {   // diagnostic builds of the plain kernel (syk_apply_H_trace): clock stamps per ring chunk
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false, 2>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        apply_h_scatter_kernel<T, NR, LRC, false, true><<<grid, kThreads, smem, stream>>>(tab, p);
+        apply_h_scatter_kernel<T, NR, LRC, false, 2><<<grid, kThreads, smem, stream>>>(tab, p);
+    } else if (fa.trace) {
+        SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false, 1>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        apply_h_scatter_kernel<T, NR, LRC, false, 1><<<grid, kThreads, smem, stream>>>(tab, p);
     } else {
         SYK_CUDA(cudaFuncSetAttribute(apply_h_scatter_kernel<T, NR, LRC, false>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -740,7 +749,7 @@ int scatter_tile_bits(int dtype) {
 int scatter_window_bits() { return kWindowBits; }
 
 // syk_apply_H_trace (include/syk.h): one plain product with the timeline of one CTA and the load list it walked
-int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, uint64_t* clk,
+int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, int detail, uint64_t* clk,
                   int clk_capacity, int32_t* load_terms, uint32_t* load_xo, int load_capacity, int* n_loads, int* rot,
                   cudaStream_t stream) {
     const StTable* tab = get_st_table(h, dtype);
@@ -753,17 +762,18 @@ int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, in
     const uint64_t n_tiles = 1ull << tab->n_outer;
     const uint64_t grid = n_tiles < (uint64_t)sms ? n_tiles : (uint64_t)sms;
     if (cta < 0 || (uint64_t)cta >= grid || round < 0 || (uint64_t)round * grid + (uint64_t)cta >= n_tiles ||
-        clk_capacity < 3 * n || load_capacity < tab->n_loads)
+        clk_capacity < 7 * n || load_capacity < tab->n_loads)
         return SYK_EINVAL;
     unsigned long long* d_trace = nullptr;
-    SYK_CUDA(cudaMalloc(&d_trace, (size_t)3 * n * sizeof(unsigned long long)));
-    cudaMemsetAsync(d_trace, 0, (size_t)3 * n * sizeof(unsigned long long), stream);
+    SYK_CUDA(cudaMalloc(&d_trace, (size_t)7 * n * sizeof(unsigned long long)));
+    cudaMemsetAsync(d_trace, 0, (size_t)7 * n * sizeof(unsigned long long), stream);
     FusedArgs fa;
     fa.trace = d_trace;
     fa.trace_cta = cta;
     fa.trace_round = round;
+    fa.trace_detail = detail;
     int rc = launch_apply_h_scatter(h, dtype, d_in, d_out, fa, stream);
-    if (rc == SYK_OK && cudaMemcpyAsync(clk, d_trace, (size_t)3 * n * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+    if (rc == SYK_OK && cudaMemcpyAsync(clk, d_trace, (size_t)7 * n * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
                                         stream) != cudaSuccess)
         rc = SYK_ECUDA;
     if (cudaStreamSynchronize(stream) != cudaSuccess) rc = SYK_ECUDA;

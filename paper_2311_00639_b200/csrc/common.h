@@ -189,7 +189,7 @@ struct FusedArgs {
     const void* prev = nullptr;     // u_{j-1}; may alias out; nullptr when j == 1
     int j = 0;
     unsigned long long* trace = nullptr;   // scatter-tile kernel only: timeline of one CTA (syk_apply_H_trace)
-    int trace_cta = 0, trace_round = 0;
+    int trace_cta = 0, trace_round = 0, trace_detail = 0;
 };
 
 // register-tile kernel (apply_h_regtile.cu): 0 if the handle cannot use it, else the tile_log2 it would use
@@ -204,7 +204,7 @@ void get_lockstep(int* epoch_len, int* lag);
 int scatter_tile_log2(const syk_ham* h, int dtype, bool forced);
 int launch_apply_h_scatter(const syk_ham* h, int dtype, const void* d_in, void* d_out, const FusedArgs& fa,
                            cudaStream_t stream);
-int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, uint64_t* clk,
+int scatter_trace(const syk_ham* h, int dtype, const void* d_in, void* d_out, int cta, int round, int detail, uint64_t* clk,
                   int clk_capacity, int32_t* load_terms, uint32_t* load_xo, int load_capacity, int* n_loads, int* rot,
                   cudaStream_t stream);
 int scatter_layout_info(const syk_ham* h, int dtype, int* n_loads, int* n_passes, uint32_t* tile_mask,

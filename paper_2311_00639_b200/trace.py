@@ -35,8 +35,23 @@ def analyse(tr, window_mask):
                 other_wait += int(wait[v]); n_other += 1
             if v + 1 < n_loads * nc:
                 by_nt.setdefault(int(tr["load_terms"][l]), []).append(int(work[v]))
+    if not tr["first_decoded"].any():        # three-stamp trace: no phases
+        return {"total": total, "wait": int(wait.sum()), "work": int(work.sum()), "by_nt": by_nt,
+                "first_wait": (first_wait, n_first), "other_wait": (other_wait, n_other), "nc": nc, "phases": {}}
+    # phases of a chunk as thread 0 of the consumers sees them (means over the chunks of loads with 1, 2, >= 4 terms)
+    nt_of = np.repeat(tr["load_terms"][(np.arange(n_loads) + rot) % n_loads], nc)
+    phases = {}
+    for name, sel in (("1", nt_of == 1), ("2", nt_of == 2), (">= 4", nt_of >= 4)):
+        idx = np.where(sel)[0]
+        idx = idx[idx + 1 < n_loads * nc]
+        if len(idx) == 0:
+            continue
+        phases[name] = [len(idx)] + [float(np.mean(b[idx] - a[idx])) for a, b in (
+            (before, after), (after, tr["first_decoded"]), (tr["first_decoded"], tr["first_issued"]),
+            (tr["first_issued"], tr["all_issued"]), (tr["all_issued"], tr["arrived"]))] + [
+            float(np.mean(before[idx + 1] - tr["arrived"][idx]))]
     return {"total": total, "wait": int(wait.sum()), "work": int(work.sum()), "by_nt": by_nt,
-            "first_wait": (first_wait, n_first), "other_wait": (other_wait, n_other), "nc": nc}
+            "first_wait": (first_wait, n_first), "other_wait": (other_wait, n_other), "nc": nc, "phases": phases}
 
 
 def main():
@@ -82,6 +97,8 @@ def main():
                   f"({100 * r['wait'] / r['total']:.1f} %) | {fw[0] / max(fw[1], 1):.0f} / {ow[0] / max(ow[1], 1):.0f} |")
             for nt, v in r["by_nt"].items():
                 merged.setdefault(nt, []).extend(v)
+        first_cta = int(args.cta.split(",")[0])
+        last_phases = analyse(B.syk_apply_H_trace(h, a, b, cta=first_cta, round=args.round, detail=1), lay["window_mask"])["phases"]
         chunk_bytes = 65536
         print("\n| terms of the load | chunks sampled | clocks worked per chunk (mean) | per term | shared-memory bytes read per clock |")
         print("|---|---|---|---|---|")
@@ -94,6 +111,14 @@ def main():
         coef, *_ = np.linalg.lstsq(A, ys, rcond=None)
         print(f"\nLeast-squares fit: clocks per chunk = {coef[0]:.0f} + {coef[1]:.0f} x terms "
               f"(an LDS pass over a 64 KiB chunk at 128 B/clk is 512 clocks).\n")
+        print(f"Phases of a chunk for thread 0 of the consumers (CTA {first_cta}, seven-stamp build of the kernel: the four extra stamps "
+              "lengthen a chunk by ~200 clocks, so read the proportions, not the sums; mean clocks):\n")
+        print("| terms of the load | chunks | wait for the chunk | decode of the first term | first term issued (16 LDS.128 + FMAs) | "
+              "other terms | last FMAs issued -> arrived on the empty-barrier | -> asks for the next chunk |")
+        print("|---|---|---|---|---|---|---|---|")
+        for name, ph in last_phases.items():
+            print(f"| {name} | {ph[0]} | " + " | ".join(f"{x:.0f}" for x in ph[1:]) + " |")
+        print()
         del a, b
         torch.cuda.empty_cache()
     return 0

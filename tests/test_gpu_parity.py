@@ -1342,6 +1342,12 @@ def test_apply_H_trace_matches_apply_H(B, torch, dt):
         assert (tr["issue"] > 0).all() and (tr["after_wait"] >= tr["before_wait"]).all()
         assert (tr["after_wait"] >= tr["issue"]).all()
         assert (np.diff(tr["before_wait"]) > 0).all() and (np.diff(tr["issue"]) > 0).all()
+        assert not tr["first_decoded"].any()                                  # three-stamp build
+        tr7 = B.syk_apply_H_trace(h, d_in, d_out, cta=cta, round=0, detail=1)    # seven stamps, in order within a chunk
+        assert torch.equal(d_out, d_ref)
+        for a, b in (("after_wait", "first_decoded"), ("first_decoded", "first_issued"), ("first_issued", "all_issued"),
+                     ("all_issued", "arrived")):
+            assert (tr7[b] >= tr7[a]).all() and (tr7[a] > 0).all(), (a, b)
     ref = ohm.matvec_sequential(N, q, J, v.astype(np.complex128))
     assert relerr(d_out.cpu().numpy(), ref) <= TOL[dt]
     # a CTA / round that does not exist, a handle on another kernel
